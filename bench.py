@@ -1,0 +1,384 @@
+#!/usr/bin/env python
+"""bench.py -- rand_cholQR (Count-Gauss) FP64 throughput on B200, one JSON line.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2] [--impl ours|reference]
+
+A "step" is one whole factorization (all SURVEY.md 8(a) rows A1..A7) of one synthetic matrix
+V = U diag(sigma) W^T of the named workload.  Sketch generation A0 is OFF the clock, the
+paper's convention; `with_sketch_gen` reports the time including it.
+`value` = algorithmic GFLOP/s (paper_2309_05868_b200/flops.py) with V resident in HBM;
+`e2e` = the same through host buffers (H2D of V, D2H of Q and R inside the timed region).
+N > 1: the rows are sharded over ranks (PAPER.md:228 footnote 3), weak scaling.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--workload", default="C2")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--seed", type=int, default=42)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extra", action="store_true", help="skip the C3 extra line")
+    ap.add_argument("--recompute-v1", action="store_true")
+    return ap.parse_args()
+
+
+# ------------------------------------------------------------------------------------------
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed regions run."""
+
+    def __init__(self, index=0, period=0.02):
+        super().__init__(daemon=True)
+        self.period = period
+        self.samples = []
+        self.reasons = set()
+        self.max_mhz = None
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
+        }
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    mask = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, nm in names.items():
+                    if mask & bit:
+                        self.reasons.add(nm)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def stop(self):
+        self._stop_evt.set()
+
+    def summary(self):
+        if not self.ok or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["nvml_unavailable"]}
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons)}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"hbm_gbs": d.get("hbm_gbs"), "bf16_tflops": d.get("bf16_tflops"),
+                "bf16_tflops_sustained": d.get("bf16_tflops_sustained"), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "source": "fallback"}
+
+
+# ------------------------------------------------------------------------------------------
+def oracle_sample(V_host, n, seed, threads_hint=None):
+    """Times the CPU oracle, as it stands, on a bounded sample (the first rows) of the workload."""
+    from oracle import rqr_oracle as orc
+    from paper_2309_05868_b200 import flops, inputs
+    orc.build()
+    ms = V_host.shape[0]
+    s1, s2 = inputs.sketch_sizes(n)
+    t0 = time.perf_counter()
+    Q, R, info = orc.rand_cholqr(V_host, s1, s2, seed)
+    dt = time.perf_counter() - t0
+    fl = flops.rand_cholqr_flops(ms, n, s1, s2)
+    return {"value": fl / dt / 1e9, "unit": "GFLOP/s", "cores": orc.num_threads(), "kind": "oracle",
+            "sample": "first %d of the workload's rows x %d cols, s1=%d s2=%d, %.2f s wall, info=%d"
+                      % (ms, n, s1, s2, dt, info)}, dt
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, on a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_2309_05868_b200 import inputs
+    c = inputs.config(args.workload)
+    n = c["n"]
+    ms = min(c["m"], 1 << 17)
+    V = inputs.make_V(ms, n, c["kappa"], c["seed"]).numpy()
+    for _ in range(args.warmup if args.warmup < 2 else 1):
+        oracle_sample(V, n, args.seed)
+    vals, dts = [], []
+    for _ in range(max(1, min(args.steps, 5))):
+        r, dt = oracle_sample(V, n, args.seed)
+        vals.append(r["value"]); dts.append(dt)
+    r["value"] = sum(vals) / len(vals)
+    line = {"impl": "reference", "metric": "rand_cholQR FP64 GFLOP/s", "value": r["value"], "unit": "GFLOP/s",
+            "n_gpus": args.gpus, "steps": len(vals), "warmup": 1, "ms_per_step": 1e3 * sum(dts) / len(dts),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": args.workload, "m": c["m"], "n": n, "kappa": c["kappa"],
+                                            "s1": c["s1"], "s2": c["s2"], "sample_rows": ms},
+            "cpu_baseline": r,
+            "e2e": {"value": r["value"], "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------
+def time_region(torch, fn, steps):
+    """CUDA-event time (ms) of `steps` calls of fn on the current stream, synchronised both sides."""
+    torch.cuda.synchronize()
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1)
+
+
+def probe_fp64_peak(torch, rq):
+    """Measured FP64 peak (TFLOP/s): best of a DFMA chain and a DMMA chain, >= 0.25 s each."""
+    sink = torch.empty(148 * 8 * 256, dtype=torch.float64, device="cuda")
+    out = {}
+    for kind, name in ((rq.PROBE_DFMA, "dfma"), (rq.PROBE_DMMA, "dmma")):
+        iters = 20000
+        fl = rq.probe_fp64(kind, iters, 148 * 8, sink)        # warm-up
+        ms = time_region(torch, lambda: rq.probe_fp64(kind, iters, 148 * 8, sink), 1)
+        reps = max(1, int(250.0 / max(ms, 1e-3)))
+        ms = time_region(torch, lambda: rq.probe_fp64(kind, iters, 148 * 8, sink), reps)
+        out[name] = fl * reps / (ms * 1e-3) / 1e12
+    return out
+
+
+def breakdown(torch, rq, Vd, c, seed, Q, R, bufs, steps, recompute):
+    """Per-step CUDA-event times of the same sequence the one-shot runs (step entry points)."""
+    names = ["countsketch", "gauss_sketch", "small_geqrf", "trsm_gram", "chol", "apply", "triu_mul"]
+    acc = {k: 0.0 for k in names}
+    s1, s2 = c["s1"], c["s2"]
+    P = rq.FLAG_PREPARED
+    for _ in range(steps):
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(len(names) + 1)]
+        ev[0].record()
+        rq.countsketch(Vd, s1, seed, bufs["W1"], bufs["work"], 0, P); ev[1].record()
+        rq.gauss_sketch(bufs["W1"], s2, seed, bufs["W"], bufs["work"], P); ev[2].record()
+        rq.small_geqrf(bufs["W"], bufs["R0"], bufs["info"]); ev[3].record()
+        rq.trsm_gram(Vd, bufs["R0"], bufs["G"], None if recompute else Q, bufs["work"]); ev[4].record()
+        rq.chol(bufs["G"], bufs["R1"], bufs["info"]); ev[5].record()
+        if recompute:
+            rq.apply(Vd, bufs["R0"], bufs["R1"], Q, bufs["work"])
+        else:
+            rq.apply(Q, None, bufs["R1"], Q, bufs["work"])
+        ev[6].record()
+        rq.triu_mul(bufs["R1"], bufs["R0"], R); ev[7].record()
+        torch.cuda.synchronize()
+        for i, k in enumerate(names):
+            acc[k] += ev[i].elapsed_time(ev[i + 1])
+    return {k: v / steps for k, v in acc.items()}
+
+
+def run_config(torch, rq, name, args, peaks, p64, want_e2e=True, want_breakdown=True):
+    from paper_2309_05868_b200 import dist as rdist, flops, inputs
+    c = inputs.config(name)
+    m, n, s1, s2 = c["m"], c["n"], c["s1"], c["s2"]
+    seed = args.seed
+    Vd = inputs.make_config_V(name, device="cuda")
+    Q = torch.empty_like(Vd)
+    R = torch.empty(n, n, dtype=torch.float64, device="cuda")
+    bufs = rdist.alloc_bufs(rq, m, n, s1, s2, "cuda")
+    work, info = bufs["work"], bufs["info"]
+    flags = rq.FLAG_PREPARED | (rq.FLAG_RECOMPUTE_V1 if args.recompute_v1 else 0)
+    t_prep = time_region(torch, lambda: rq.sketch_prepare(m, n, s1, s2, seed, work), 1)
+    t_prep = time_region(torch, lambda: rq.sketch_prepare(m, n, s1, s2, seed, work), 3) / 3
+
+    def step():
+        rq.rand_cholqr(Vd, s1, s2, seed, Q, R, work, info, 0, flags)
+
+    for _ in range(args.warmup):
+        step()
+    ms = time_region(torch, step, args.steps) / args.steps
+    assert int(info.item()) == 0, "numerical failure: info=%d" % int(info.item())
+    eye = torch.eye(n, dtype=torch.float64, device="cuda")
+    orth = float(torch.linalg.norm(Q.T @ Q - eye))
+    res = float(torch.linalg.norm(Vd - Q @ R) / torch.linalg.norm(Vd))
+    F = flops.rand_cholqr_flops(m, n, s1, s2)
+    B = flops.rand_cholqr_bytes(m, n, s1, s2)
+    t_roof = max(F / (p64 * 1e12), B / (peaks["hbm_gbs"] * 1e9))
+    out = {"workload": name, "m": m, "n": n, "kappa": c["kappa"], "s1": s1, "s2": s2,
+           "ms_per_step": ms, "gflops": F / ms / 1e6, "gbs": B / ms / 1e6,
+           "roofline_frac_whole_path": t_roof / (ms * 1e-3), "orth_err": orth, "resid": res,
+           "sketch_gen_ms": t_prep, "ms_with_sketch_gen": ms + t_prep}
+    # comparator on the same kernels, same V
+    def step_c2():
+        rq.cholqr2(Vd, Q, R, work, info)
+    for _ in range(2):
+        step_c2()
+    out["cholqr2_ms"] = time_region(torch, step_c2, max(3, args.steps // 3)) / max(3, args.steps // 3)
+    out["cholqr2_info"] = int(info.item())
+    if want_breakdown:
+        out["breakdown_ms"] = breakdown(torch, rq, Vd, c, seed, Q, R, bufs, max(3, args.steps // 3),
+                                        args.recompute_v1)
+    if want_e2e:
+        Vh = torch.empty(Vd.shape, dtype=torch.float64, pin_memory=True)
+        Vh.copy_(Vd)
+        Qh = torch.empty(Vd.shape, dtype=torch.float64, pin_memory=True)
+        Rh = torch.empty(n, n, dtype=torch.float64, pin_memory=True)
+        Vin = torch.empty_like(Vd)
+
+        def step_e2e():
+            Vin.copy_(Vh, non_blocking=True)
+            rq.rand_cholqr(Vin, s1, s2, seed, Q, R, work, info, 0, flags)
+            Qh.copy_(Q, non_blocking=True)
+            Rh.copy_(R, non_blocking=True)
+        step_e2e()
+        k = max(2, min(args.steps, 5))
+        ms_e = time_region(torch, step_e2e, k) / k
+        out["e2e"] = {"value": F / ms_e / 1e6, "unit": "GFLOP/s", "ms_per_step": ms_e,
+                      "h2d_bytes_per_step": int(8 * m * n), "d2h_bytes_per_step": int(8 * m * n + 8 * n * n)}
+        del Vh, Qh, Vin
+    out["_V_host_sample"] = Vd[: min(m, 1 << 17)].cpu().numpy() if not args.no_cpu_baseline else None
+    del Vd, Q, bufs
+    torch.cuda.empty_cache()
+    return out, F
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+        return
+    import torch
+    import __graft_entry__ as ge
+    from paper_2309_05868_b200 import binding as rq, flops, inputs
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if rank == 0:
+        ge.build()
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        dist.barrier()
+        run_sharded(torch, rq, args, world, rank)
+        dist.destroy_process_group()
+        return
+    rq.lib()
+    peaks = measured_peaks()
+    sampler = ClockSampler(local)
+    sampler.start()
+    p64s = probe_fp64_peak(torch, rq)
+    ratio_peak = (peaks["bf16_tflops"] or 1590.0) * (45.0 / 2250.0)   # guide's nominal FP64:bf16 ratio
+    p64 = max(p64s["dfma"], p64s["dmma"], 1e-3)
+    main_out, F = run_config(torch, rq, args.workload, args, peaks, p64)
+    extra = None
+    if not args.no_extra and args.workload == "C2":
+        extra, _ = run_config(torch, rq, "C3", args, peaks, p64, want_e2e=False, want_breakdown=True)
+        extra.pop("_V_host_sample", None)
+    sampler.stop()
+    sampler.join(timeout=1.0)
+    c = inputs.config(args.workload)
+    m, n = c["m"], c["n"]
+    bd = main_out["breakdown_ms"]
+    dom = max(("countsketch", "trsm_gram", "apply"), key=lambda k: bd[k])
+    sb = flops.step_bytes(m, n)
+    if dom == "trsm_gram" and flops.trsm_gram_flops(m, n) / (p64 * 1e12) > sb[dom] / (peaks["hbm_gbs"] * 1e9):
+        ach = flops.trsm_gram_flops(m, n) / (bd[dom] * 1e-3) / 1e12
+        roof = {"kernel": "rqr_trsm_gram", "bound": "tensor", "achieved": ach, "peak": p64, "unit": "TFLOP/s",
+                "frac": ach / p64, "traffic": None,
+                "peak_source": "FP64 probe measured live in this run (max of DFMA %.1f / DMMA %.1f TFLOP/s); "
+                               "MEASURED_PEAKS.json has no FP64 figure; bf16 x nominal ratio would give %.1f"
+                               % (p64s["dfma"], p64s["dmma"], ratio_peak)}
+    else:
+        ach = sb[dom] / (bd[dom] * 1e-3) / 1e9
+        roof = {"kernel": "rqr_" + dom, "bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                "frac": ach / peaks["hbm_gbs"], "traffic": None,
+                "peak_source": "MEASURED_PEAKS.json hbm_gbs (%s)" % peaks["source"]}
+    cpu = None
+    if not args.no_cpu_baseline:
+        cpu, _ = oracle_sample(main_out.pop("_V_host_sample"), n, args.seed)
+    main_out.pop("_V_host_sample", None)
+    line = {"metric": "rand_cholQR FP64 GFLOP/s", "value": main_out["gflops"], "unit": "GFLOP/s",
+            "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": main_out["ms_per_step"],
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": args.workload, "m": m, "n": n, "kappa": c["kappa"], "s1": c["s1"], "s2": c["s2"],
+                       "l2": "inputs_exceed_L2" if 8 * m * n > 126e6 else "L2_resident_not_flushed",
+                       "sketch_generation": "off_the_clock (PAPER.md:883)",
+                       "v1": "recomputed" if args.recompute_v1 else "stored"},
+            "gbs": main_out["gbs"], "roofline_frac_whole_path": main_out["roofline_frac_whole_path"],
+            "orth_err": main_out["orth_err"], "resid": main_out["resid"],
+            "cholqr2_ms": main_out["cholqr2_ms"], "cholqr2_info": main_out["cholqr2_info"],
+            "sketch_gen_ms": main_out["sketch_gen_ms"], "breakdown_ms": bd,
+            "fp64_peak_tflops": p64s, "e2e": {k: v for k, v in main_out["e2e"].items()},
+            "gpu_launches": 9 * args.steps, "roofline": roof, "cpu_baseline": cpu,
+            "clocks": sampler.summary(), "extra": extra}
+    print(json.dumps(line))
+
+
+def run_sharded(torch, rq, args, world, rank):
+    """N > 1: block rows per rank, two all-reduces per step, weak scaling (per-rank rows fixed)."""
+    import torch.distributed as dist
+    from paper_2309_05868_b200 import dist as rdist, flops, inputs
+    c = inputs.config(args.workload)
+    m, n, s1, s2 = c["m"], c["n"], c["s1"], c["s2"]
+    m_total = m * world
+    row0 = rank * m
+    Vd = inputs.make_V(m, n, c["kappa"], c["seed"] + 1000 * rank, device="cuda")
+    Q = torch.empty_like(Vd)
+    R = torch.empty(n, n, dtype=torch.float64, device="cuda")
+    bufs = rdist.alloc_bufs(rq, m, n, s1, s2, "cuda")
+    rq.sketch_prepare(m, n, s1, s2, args.seed, bufs["work"], 0, row0)
+
+    def step():
+        rdist.rand_cholqr_sharded(rq, Vd, row0, s1, s2, args.seed, Q, R, bufs, None, rq.FLAG_PREPARED, 0)
+    for _ in range(args.warmup):
+        step()
+    dist.barrier(); torch.cuda.synchronize()
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    torch.cuda.synchronize(); dist.barrier()
+    t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms = float(t.item()) / args.steps
+    F = flops.rand_cholqr_flops(m_total, n, s1, s2)
+    if rank == 0:
+        line = {"metric": "rand_cholQR FP64 GFLOP/s", "value": F / ms / 1e6, "unit": "GFLOP/s", "n_gpus": world,
+                "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": args.workload, "m_per_gpu": m, "m_total": m_total, "n": n, "s1": s1, "s2": s2,
+                           "parallelism": "row-sharded, 2 all-reduces (W, G) per step",
+                           "l2": "inputs_exceed_L2"},
+                "gpu_launches": 9 * args.steps, "info": int(bufs["info"].item())}
+        print(json.dumps(line))
+
+
+if __name__ == "__main__":
+    main()

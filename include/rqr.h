@@ -1,0 +1,149 @@
+/*
+ * rqr.h -- C ABI of librqr: the hot path of rand_cholQR with Count-Gauss multisketching
+ * (Higgins, Szyld, Boman, Yamazaki, arxiv 2309.05868; cited as PAPER.md:<line>) for one
+ * NVIDIA B200 (sm_100a).  Every step is a hand-written CUDA kernel; no cuBLAS / cuSOLVER /
+ * cuSPARSE, no CPU fallback.
+ *
+ * Letters follow BASELINE.json: V is m x n (m rows >> n columns), s1 = CountSketch rows,
+ * s2 = Gaussian sketch rows.  The paper writes V in R^{n x m}, S1 in R^{p1 x n},
+ * S2 in R^{p2 x p1}.
+ *
+ * Conventions common to every entry point
+ *  - All matrix pointers are DEVICE pointers to float64, ROW-MAJOR, with an element leading
+ *    dimension where one is given (ldv, ldq >= n).  Small matrices (W1, W, R0, G, R1, R) are
+ *    dense row-major with leading dimension n.  Bases must be 16-byte aligned.
+ *  - The caller owns every buffer.  The library allocates nothing; scratch comes from `work`,
+ *    a device buffer of at least rqr_workspace_bytes(...) bytes, 256-byte aligned.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = default stream).  Every call is
+ *    asynchronous on it, performs no synchronisation or allocation, and is CUDA-graph
+ *    capturable.
+ *  - Return value: RQR_OK, or -k if argument k (1-based) is invalid, or RQR_ERR_LAUNCH if a
+ *    kernel launch failed.  NUMERICAL status goes to a device int (`d_info`, may be NULL):
+ *      0                        success
+ *      RQR_INFO_NOT_SPD + j     Cholesky pivot j (1-based) not > 0 or NaN  (cholQR2 at
+ *                               kappa >~ u^-1/2)
+ *      RQR_INFO_SINGULAR + j    Householder column j has zero / non-finite norm: V is rank
+ *                               deficient for randQR
+ *    d_info is written only on failure (first failure wins); the caller zeroes it (the
+ *    one-shot drivers zero it themselves).  Outputs are undefined when *d_info != 0.
+ *  - Argument limits: 2 <= n <= 256, n <= s2 <= s1 <= m_total (eq. (20)),
+ *    s2 <= 512, s1 < 2^31, m < 2^31 per call.
+ *  - Thread safety: no global mutable state; calls on different streams with different
+ *    buffers are independent.
+ */
+#ifndef RQR_H
+#define RQR_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define RQR_OK 0
+#define RQR_ERR_LAUNCH (-1000)
+#define RQR_INFO_NOT_SPD 1000
+#define RQR_INFO_SINGULAR 2000
+
+/* CountSketch variants */
+#define RQR_VARIANT_SORTED 0  /* gather over the bucket-sorted row list (CSR form of S1, the
+                                 paper's SpMM form); deterministic            */
+#define RQR_VARIANT_SCATTER 1 /* stream V, hash on the fly, red.global.add.f64; the last
+                                 bits depend on the order of the atomics                    */
+
+/* flags */
+#define RQR_FLAG_PREPARED 1   /* `work` already holds the sketch state written by
+                                 rqr_sketch_prepare with the same (m, n, row0, s1, s2,
+                                 seed, variant): skip sketch generation (the paper's timing
+                                 convention).  Without it the call generates
+                                 what it needs first, on the same stream.                   */
+#define RQR_FLAG_RECOMPUTE_V1 2 /* one-shot drivers: do not store V1 = V R0^-1; re-form it in
+                                 the apply pass with bit-identical arithmetic (32mn bytes of
+                                 traffic instead of 40mn, 4mn^2 flops instead of 3mn^2)      */
+
+/* Size in bytes of the workspace every call below accepts for this problem shape. */
+size_t rqr_workspace_bytes(int64_t m, int n, int64_t s1, int s2, int variant);
+
+/* A0 -- sketch generation, off the paper's clock.  Writes into `work`:
+ * S2 (s2 x s1, entries N(0,1)/sqrt(s2)) from Philox4x32-10 stream 1 and, for
+ * RQR_VARIANT_SORTED, the rows [row0, row0+m) sorted by CountSketch bucket (stable, ascending
+ * row inside a bucket) with their signs, plus the s1+1 bucket offsets.  Bucket and sign of a
+ * row are a function of its GLOBAL index row0 + i (Philox stream 0; reading S1).  */
+int rqr_sketch_prepare(int64_t m, int n, int64_t row0, int64_t s1, int s2, uint64_t seed,
+                       int variant, void* work, void* stream);
+
+/* A1 -- CountSketch, Alg. 1 step 1 first half: W1 = S1 V,
+ * W1[h(i),:] += sigma(i) V[i,:], S1 unscaled.  W1 (s1 x n) is overwritten.   */
+int rqr_countsketch(const double* V, int64_t m, int n, int64_t ldv, int64_t row0, int64_t s1,
+                    uint64_t seed, double* W1, void* work, int variant, int flags, void* stream);
+
+/* A2 -- Gaussian sketch, Alg. 1 step 1 second half: W = S2 W1, W s2 x n.      */
+int rqr_gauss_sketch(const double* W1, int64_t s1, int n, int s2, uint64_t seed, double* W,
+                     void* work, int flags, void* stream);
+
+/* A3 -- R factor of the Householder QR of W (Alg. 1 step 2).  W (s2 x n) is
+ * destroyed.  R0 is n x n upper triangular with diag > 0 and exact zeros below.             */
+int rqr_small_geqrf(double* W, int s2, int n, double* R0, int* d_info, void* stream);
+
+/* A4 -- fused V1 = V R0^-1 (Alg. 1 step 3; row-wise substitution, eq. (42)
+ * PAPER.md:449-453) and Gram matrix G = V1^T V1 (Alg. 2 step 1), split over
+ * row tiles with a fixed-order reduction.  R0 == NULL means identity (plain Gram of V).
+ * G (n x n) is written full symmetric.  V1 != NULL: V1 (m x n, ld ldq) is also stored;
+ * V1 == V is allowed.                                                                        */
+int rqr_trsm_gram(const double* V, int64_t m, int n, int64_t ldv, const double* R0, double* G,
+                  double* V1, int64_t ldq, void* work, void* stream);
+
+/* A5 -- upper Cholesky factor, G + shift I = R1^T R1 (Alg. 2 step 2).          */
+int rqr_chol(const double* G, int n, double shift, double* R1, int* d_info, void* stream);
+
+/* A6 -- Q = (V R0^-1) R1^-1 (Alg. 2 step 3), never V (R0^-1 R1^-1).
+ * R0 == NULL: V already holds V1 (stored by rqr_trsm_gram) and Q = V R1^-1.  R0 != NULL: V1
+ * is re-formed with arithmetic bit-identical to rqr_trsm_gram's.  Q == V is allowed.         */
+int rqr_apply(const double* V, int64_t m, int n, int64_t ldv, const double* R0, const double* R1,
+              double* Q, int64_t ldq, void* work, void* stream);
+
+/* A7 -- R = R1 R0, upper x upper (Alg. 3 step 3).                              */
+int rqr_triu_mul(const double* R1, const double* R0, int n, double* R, void* stream);
+
+/* One-shot Alg. 3 rand_cholQR with Count-Gauss: Q (m x n, ld n), R (n x n).
+ * V has leading dimension n.  Q == V is allowed.                                             */
+int rqr_rand_cholqr(const double* V, int64_t m, int n, int64_t s1, int s2, uint64_t seed,
+                    double* Q, double* R, void* work, int* d_info, int variant, int flags,
+                    void* stream);
+
+/* Comparators on the same kernels.  Alg. 4 CholeskyQR2.                   */
+int rqr_cholqr2(const double* V, int64_t m, int n, double* Q, double* R, void* work, int* d_info,
+                void* stream);
+/* Shifted CholeskyQR3 (cited only; reading S9): shift =
+ * 11 (m n + n(n+1)) 2^-53 tr(V^T V).                                                         */
+int rqr_scholqr3(const double* V, int64_t m, int n, double* Q, double* R, void* work, int* d_info,
+                 void* stream);
+/* rand_cholQR with ONE dense Gaussian sketch S (s x m, N(0,1)/sqrt(s), Philox stream 3,
+ * generated on the fly).                                             */
+int rqr_gauss_randcholqr(const double* V, int64_t m, int n, int s, uint64_t seed, double* Q,
+                         double* R, void* work, int* d_info, void* stream);
+/* The dense sketch step alone: W (s x n) = S V for rows [row0, row0+m) of m_total.           */
+int rqr_dense_gauss_sketch(const double* V, int64_t m, int n, int64_t ldv, int64_t row0,
+                           int64_t m_total, int s, uint64_t seed, double* W, void* work,
+                           void* stream);
+
+/* Inspection helpers for parity tests (device outputs): bucket (uint32) and sign (int8, +-1)
+ * of rows [row0, row0+count); Gaussian stream entries z(first .. first+count-1).            */
+int rqr_debug_hash_sign(uint64_t seed, int64_t row0, int64_t count, int64_t s1, uint32_t* bucket,
+                        int8_t* sign, void* stream);
+int rqr_debug_gauss(uint64_t seed, uint32_t stream_id, uint64_t first, int64_t count, double* z,
+                    void* stream);
+/* Pointer to S2 (s2 x s1) inside a workspace prepared for (n, s1).                            */
+const double* rqr_workspace_S2(void* work, int n, int64_t s1);
+
+/* Test hook: on != 0 forces the generic (non-DMMA) kernels in rqr_trsm_gram / rqr_apply.       */
+void rqr_debug_force_generic(int on);
+
+/* Library version string. */
+const char* rqr_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RQR_H */

@@ -211,13 +211,18 @@ void orc_gauss_sketch(const double *W1, int64_t s1, int n, int s2, uint64_t seed
 {
     double *S2 = (double *)malloc(sizeof(double) * (size_t)s2 * (size_t)s1);
     orc_gauss_matrix(seed, s2, s1, S2);
+    /* loop nest r, c, j: every entry W[r,j] still receives its terms in ascending c (the
+     * stated order); only the memory walk is contiguous */
 #pragma omp parallel for schedule(static)
-    for (int r = 0; r < s2; ++r)
-        for (int j = 0; j < n; ++j) {
-            double acc = 0.0;
-            for (int64_t c = 0; c < s1; ++c) acc += S2[(int64_t)r * s1 + c] * W1[c * n + j];
-            W[(int64_t)r * n + j] = acc;
+    for (int r = 0; r < s2; ++r) {
+        double *w = W + (int64_t)r * n;
+        for (int j = 0; j < n; ++j) w[j] = 0.0;
+        for (int64_t c = 0; c < s1; ++c) {
+            const double a = S2[(int64_t)r * s1 + c];
+            const double *b = W1 + c * n;
+            for (int j = 0; j < n; ++j) w[j] += a * b[j];
         }
+    }
     free(S2);
 }
 

@@ -1,0 +1,125 @@
+// rqr_common.cuh -- shared device helpers of librqr (CUDA path only; the CPU oracle shares
+// nothing with this file).  sm_100a.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include "../../include/rqr.h"
+
+#define RQR_MAX_N 256
+#define RQR_MAX_S2 512
+#define RQR_MAX_GRAM_PARTIALS 304        // >= 2 CTAs per SM on 148 SMs
+#define RQR_GAUSS_PARTIAL_ROWS 16384     // ksplit * s2 <= this
+
+#define RQR_PHILOX_STREAM_COUNT 0u
+#define RQR_PHILOX_STREAM_S2 1u
+#define RQR_PHILOX_STREAM_DENSE 3u
+
+#define RQR_LAUNCH_CHECK()                                   \
+    do {                                                     \
+        if (cudaGetLastError() != cudaSuccess) return RQR_ERR_LAUNCH; \
+    } while (0)
+
+static inline size_t rqr_align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+// ---------------------------------------------------------------------------------------
+// Workspace layout.  Offsets of a region depend only on
+// arguments every user of that region has.
+//   [0,256)            header: counters / flags used inside single calls
+//   A  tall scratch    f(n)      Gram partials, small matrices of the one-shot drivers
+//   B  bucket offsets  f(s1)     (s1+1) u32 offsets, s1 u32 cursors
+//   C  S2 slot         f(s1)     sized for s2 = RQR_MAX_S2
+//   D  gauss partials  f(n)
+//   E  sorted rows     f(m)      m u32 (row | sign<<31)
+//   F  one-shot        W1 (s1 x n), W (s2max x n)
+// ---------------------------------------------------------------------------------------
+struct RqrLayout {
+    size_t hdr, A, A_small, B_off, B_cur, C, D, E, F_W1, F_W, total;
+};
+
+static inline RqrLayout rqr_layout(int64_t m, int n, int64_t s1)
+{
+    RqrLayout L;
+    size_t nn = (size_t)n * n * sizeof(double);
+    L.hdr = 0;
+    L.A = 256;
+    L.A_small = L.A + rqr_align256((size_t)RQR_MAX_GRAM_PARTIALS * nn);
+    L.B_off = L.A_small + rqr_align256(16 * nn);
+    L.B_cur = L.B_off + rqr_align256((size_t)(s1 + 1) * 4);
+    L.C = L.B_cur + rqr_align256((size_t)s1 * 4);
+    L.D = L.C + rqr_align256((size_t)RQR_MAX_S2 * (size_t)s1 * sizeof(double));
+    L.E = L.D + rqr_align256((size_t)RQR_GAUSS_PARTIAL_ROWS * n * sizeof(double));
+    L.F_W1 = L.E + rqr_align256((size_t)m * 4);
+    L.F_W = L.F_W1 + rqr_align256((size_t)s1 * n * sizeof(double));
+    L.total = L.F_W + rqr_align256((size_t)RQR_MAX_S2 * n * sizeof(double));
+    return L;
+}
+
+// small matrices inside A_small (each n*n doubles)
+enum { RQR_SM_R0 = 0, RQR_SM_R1 = 1, RQR_SM_G = 2, RQR_SM_RA = 3, RQR_SM_RB = 4, RQR_SM_RC = 5 };
+
+// ---------------------------------------------------------------------------------------
+// Philox4x32-10 (Salmon et al., SC'11).  Specification: DESIGN.md reading S1.
+// key = (seed lo, seed hi); counter = (idx lo, idx hi, stream, 0).
+// ---------------------------------------------------------------------------------------
+__host__ __device__ __forceinline__ void rqr_philox(uint64_t seed, uint64_t idx, uint32_t stream,
+                                                    uint32_t out[4])
+{
+    uint32_t c0 = (uint32_t)idx, c1 = (uint32_t)(idx >> 32), c2 = stream, c3 = 0u;
+    uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+#ifdef __CUDA_ARCH__
+        uint32_t h0 = __umulhi(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;
+        uint32_t h1 = __umulhi(0xCD9E8D57u, c2), l1 = 0xCD9E8D57u * c2;
+#else
+        uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
+        uint32_t h0 = (uint32_t)(p0 >> 32), l0 = (uint32_t)p0;
+        uint32_t h1 = (uint32_t)(p1 >> 32), l1 = (uint32_t)p1;
+#endif
+        uint32_t n0 = h1 ^ c1 ^ k0, n2 = h0 ^ c3 ^ k1;
+        c0 = n0; c1 = l1; c2 = n2; c3 = l0;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// CountSketch bucket and sign of GLOBAL row index i (reading S1/S2).
+__device__ __forceinline__ void rqr_hash_sign(uint64_t seed, uint64_t i, uint32_t s1,
+                                              uint32_t& bucket, uint32_t& neg)
+{
+    uint32_t o[4];
+    rqr_philox(seed, i, RQR_PHILOX_STREAM_COUNT, o);
+    bucket = __umulhi(o[0], s1);     // (uint64(o0) * s1) >> 32
+    neg = o[1] & 1u;
+}
+
+// Box-Muller pair q of a stream (reading S3): returns z_even, z_odd (standard normal).
+__device__ __forceinline__ void rqr_gauss_pair(uint64_t seed, uint64_t q, uint32_t stream,
+                                               double& z0, double& z1)
+{
+    uint32_t o[4];
+    rqr_philox(seed, q, stream, o);
+    uint64_t x1 = (((uint64_t)o[0] << 32) | o[1]) >> 12;
+    uint64_t x2 = (((uint64_t)o[2] << 32) | o[3]) >> 12;
+    double u1 = (double)(2 * x1 + 1) * 0x1p-53;      // exact: 2x+1 < 2^53
+    double u2 = (double)(2 * x2 + 1) * 0x1p-53;
+    double rho = sqrt(-2.0 * log(u1));
+    double s, c;
+    sincospi(2.0 * u2, &s, &c);
+    z0 = rho * c;
+    z1 = rho * s;
+}
+
+__device__ __forceinline__ double rqr_gauss_entry(uint64_t seed, uint64_t e, uint32_t stream)
+{
+    double z0, z1;
+    rqr_gauss_pair(seed, e >> 1, stream, z0, z1);
+    return (e & 1) ? z1 : z0;
+}
+
+// first-failure-wins numerical status
+__device__ __forceinline__ void rqr_set_info(int* d_info, int code)
+{
+    if (d_info) atomicCAS(d_info, 0, code);
+}

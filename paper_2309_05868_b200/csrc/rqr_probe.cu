@@ -1,0 +1,62 @@
+// rqr_probe.cu -- FP64 peak probes (include/rqr_probe.h).  Measurement only, not on the hot path.
+#include "rqr_common.cuh"
+#include "../../include/rqr_probe.h"
+
+__global__ void __launch_bounds__(256)
+k_probe_dfma(int iters, double* __restrict__ sink)
+{
+    double a = 1.0 + 1e-9 * threadIdx.x, b = 1e-9 * blockIdx.x;
+    double acc[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) acc[k] = (double)k;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) acc[k] = fma(acc[k], a, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) s += acc[k];
+    sink[(size_t)blockIdx.x * 256 + threadIdx.x] = s;
+}
+
+__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+__global__ void __launch_bounds__(256)
+k_probe_dmma(int iters, double* __restrict__ sink)
+{
+    double a = 1e-3 * (threadIdx.x & 31), b = 1e-3 * (blockIdx.x & 7);
+    double c[8][2];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) { c[k][0] = k; c[k][1] = -k; }
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) dmma884(c[k][0], c[k][1], a, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) s += c[k][0] + c[k][1];
+    sink[(size_t)blockIdx.x * 256 + threadIdx.x] = s;
+}
+
+extern "C" int rqr_probe_fp64(int kind, int iters, int blocks, double* d_sink, double* flops_out,
+                              void* stream)
+{
+    if (kind != RQR_PROBE_DFMA && kind != RQR_PROBE_DMMA) return -1;
+    if (iters < 1) return -2;
+    if (blocks < 1) return -3;
+    if (!d_sink) return -4;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (kind == RQR_PROBE_DFMA) {
+        k_probe_dfma<<<blocks, 256, 0, st>>>(iters, d_sink);
+        if (flops_out) *flops_out = (double)blocks * 256.0 * iters * 8.0 * 2.0;
+    } else {
+        k_probe_dmma<<<blocks, 256, 0, st>>>(iters, d_sink);
+        if (flops_out) *flops_out = (double)blocks * 8.0 /*warps*/ * iters * 8.0 * 512.0;
+    }
+    RQR_LAUNCH_CHECK();
+    return RQR_OK;
+}

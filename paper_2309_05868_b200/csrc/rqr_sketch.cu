@@ -1,0 +1,585 @@
+// rqr_sketch.cu -- A0 sketch generation, A1 CountSketch, A2 Gaussian sketch GEMM, and the
+// single dense Gaussian sketch comparator.  See include/rqr.h for the contracts and DESIGN.md
+// for the kernel designs.  sm_100a.
+#include "rqr_common.cuh"
+
+// =========================================================================================
+// A0: sketch generation (off the paper's clock)
+// =========================================================================================
+
+// S2[e] = z(e) / sqrt(s2), one Box-Muller pair per thread (entries 2q, 2q+1).
+__global__ void k_gen_S2(uint64_t seed, int s2, int64_t total, double* __restrict__ S2)
+{
+    const double d = sqrt((double)s2);
+    int64_t npairs = (total + 1) >> 1;
+    for (int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; q < npairs;
+         q += (int64_t)gridDim.x * blockDim.x) {
+        double z0, z1;
+        rqr_gauss_pair(seed, (uint64_t)q, RQR_PHILOX_STREAM_S2, z0, z1);
+        int64_t e = 2 * q;
+        S2[e] = z0 / d;
+        if (e + 1 < total) S2[e + 1] = z1 / d;
+    }
+}
+
+__global__ void k_bucket_hist(uint64_t seed, int64_t row0, int64_t m, uint32_t s1,
+                              uint32_t* __restrict__ hist)
+{
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < m;
+         i += (int64_t)gridDim.x * blockDim.x) {
+        uint32_t b, neg;
+        rqr_hash_sign(seed, (uint64_t)(row0 + i), s1, b, neg);
+        atomicAdd(&hist[b], 1u);
+    }
+}
+
+// single CTA: exclusive scan of hist[0..s1) -> off[0..s1]; cursor[b] = off[b]
+__global__ void k_bucket_scan(const uint32_t* hist, uint32_t s1, uint32_t* __restrict__ off,
+                              uint32_t* cursor)   // hist may alias cursor
+{
+    __shared__ uint32_t warp_tot[32];
+    __shared__ uint32_t carry;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    if (tid == 0) carry = 0;
+    __syncthreads();
+    for (uint32_t base = 0; base < s1; base += blockDim.x) {
+        uint32_t idx = base + tid;
+        uint32_t v = idx < s1 ? hist[idx] : 0u;
+        uint32_t x = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= o) x += y;
+        }
+        if (lane == 31) warp_tot[wid] = x;
+        __syncthreads();
+        if (wid == 0) {
+            uint32_t t = lane < (int)(blockDim.x >> 5) ? warp_tot[lane] : 0u;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                uint32_t y = __shfl_up_sync(0xffffffffu, t, o);
+                if (lane >= o) t += y;
+            }
+            warp_tot[lane] = t;   // inclusive scan of warp totals
+        }
+        __syncthreads();
+        uint32_t excl = carry + (wid ? warp_tot[wid - 1] : 0u) + x - v;
+        if (idx < s1) { off[idx] = excl; cursor[idx] = excl; }
+        __syncthreads();
+        if (tid == 0) carry += warp_tot[(blockDim.x >> 5) - 1];
+        __syncthreads();
+    }
+    if (tid == 0) off[s1] = carry;
+}
+
+__global__ void k_bucket_fill(uint64_t seed, int64_t row0, int64_t m, uint32_t s1,
+                              uint32_t* __restrict__ cursor, uint32_t* __restrict__ entries)
+{
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < m;
+         i += (int64_t)gridDim.x * blockDim.x) {
+        uint32_t b, neg;
+        rqr_hash_sign(seed, (uint64_t)(row0 + i), s1, b, neg);
+        uint32_t pos = atomicAdd(&cursor[b], 1u);
+        entries[pos] = (uint32_t)i | (neg << 31);
+    }
+}
+
+// One CTA per bucket (grid-stride): sort the bucket's entries by row (low 31 bits), so that the
+// list is the STABLE counting sort of the rows and W1 is reproducible run to run.  Bitonic
+// network in its all-ascending form, which tolerates virtual +inf padding, in shared memory
+// when the segment fits, else in place in global memory.
+#define RQR_SORT_SMEM_ENTRIES 8192
+__global__ void k_bucket_sort(const uint32_t* __restrict__ off, uint32_t s1,
+                              uint32_t* __restrict__ entries)
+{
+    __shared__ uint32_t sbuf[RQR_SORT_SMEM_ENTRIES];
+    for (uint32_t b = blockIdx.x; b < s1; b += gridDim.x) {
+        const uint32_t beg = off[b], len = off[b + 1] - beg;
+        if (len < 2) continue;
+        uint32_t* g = entries + beg;
+        const bool in_smem = len <= RQR_SORT_SMEM_ENTRIES;
+        uint32_t* a = in_smem ? sbuf : g;
+        if (in_smem) {
+            for (uint32_t i = threadIdx.x; i < len; i += blockDim.x) sbuf[i] = g[i];
+        }
+        __syncthreads();
+        uint32_t P = 1; while (P < len) P <<= 1;
+        for (uint32_t k = 2; k <= P; k <<= 1) {
+            for (uint32_t i = threadIdx.x; i < len; i += blockDim.x) {
+                uint32_t p = i ^ (k - 1);
+                if (p > i && p < len) {
+                    uint32_t x = a[i], y = a[p];
+                    if ((x & 0x7fffffffu) > (y & 0x7fffffffu)) { a[i] = y; a[p] = x; }
+                }
+            }
+            __syncthreads();
+            for (uint32_t j = k >> 2; j > 0; j >>= 1) {
+                for (uint32_t i = threadIdx.x; i < len; i += blockDim.x) {
+                    uint32_t p = i ^ j;
+                    if (p > i && p < len) {
+                        uint32_t x = a[i], y = a[p];
+                        if ((x & 0x7fffffffu) > (y & 0x7fffffffu)) { a[i] = y; a[p] = x; }
+                    }
+                }
+                __syncthreads();
+            }
+        }
+        if (in_smem) {
+            for (uint32_t i = threadIdx.x; i < len; i += blockDim.x) g[i] = sbuf[i];
+        }
+        __syncthreads();
+    }
+}
+
+static int launch_prepare_S2(int64_t s1, int s2, uint64_t seed, double* S2, cudaStream_t st)
+{
+    int64_t total = (int64_t)s2 * s1;
+    int64_t npairs = (total + 1) / 2;
+    int blocks = (int)((npairs + 255) / 256 < 148 * 16 ? (npairs + 255) / 256 : 148 * 16);
+    if (blocks < 1) blocks = 1;
+    k_gen_S2<<<blocks, 256, 0, st>>>(seed, s2, total, S2);
+    RQR_LAUNCH_CHECK();
+    return RQR_OK;
+}
+
+static int launch_prepare_sorted(int64_t m, int64_t row0, int64_t s1, uint64_t seed, uint32_t* off,
+                                 uint32_t* cursor, uint32_t* entries, cudaStream_t st)
+{
+    if (cudaMemsetAsync(cursor, 0, (size_t)s1 * 4, st) != cudaSuccess) return RQR_ERR_LAUNCH;
+    int blocks = (int)((m + 255) / 256 < 148 * 16 ? (m + 255) / 256 : 148 * 16);
+    if (blocks < 1) blocks = 1;
+    k_bucket_hist<<<blocks, 256, 0, st>>>(seed, row0, m, (uint32_t)s1, cursor);
+    RQR_LAUNCH_CHECK();
+    k_bucket_scan<<<1, 1024, 0, st>>>(cursor, (uint32_t)s1, off, cursor);
+    RQR_LAUNCH_CHECK();
+    k_bucket_fill<<<blocks, 256, 0, st>>>(seed, row0, m, (uint32_t)s1, cursor, entries);
+    RQR_LAUNCH_CHECK();
+    int sb = (int)(s1 < 148 * 8 ? s1 : 148 * 8);
+    k_bucket_sort<<<sb, 256, 0, st>>>(off, (uint32_t)s1, entries);
+    RQR_LAUNCH_CHECK();
+    return RQR_OK;
+}
+
+extern "C" int rqr_sketch_prepare(int64_t m, int n, int64_t row0, int64_t s1, int s2,
+                                  uint64_t seed, int variant, void* work, void* stream)
+{
+    if (m < 1 || m >= ((int64_t)1 << 31)) return -1;
+    if (n < 2 || n > RQR_MAX_N) return -2;
+    if (row0 < 0) return -3;
+    if (s1 < 1 || s1 >= ((int64_t)1 << 31)) return -4;
+    if (s2 < 1 || s2 > RQR_MAX_S2 || s2 > s1) return -5;
+    if (variant != RQR_VARIANT_SORTED && variant != RQR_VARIANT_SCATTER) return -7;
+    if (!work) return -8;
+    cudaStream_t st = (cudaStream_t)stream;
+    RqrLayout L = rqr_layout(m, n, s1);
+    char* w = (char*)work;
+    int rc = launch_prepare_S2(s1, s2, seed, (double*)(w + L.C), st);
+    if (rc != RQR_OK) return rc;
+    if (variant == RQR_VARIANT_SORTED)
+        rc = launch_prepare_sorted(m, row0, s1, seed, (uint32_t*)(w + L.B_off),
+                                   (uint32_t*)(w + L.B_cur), (uint32_t*)(w + L.E), st);
+    return rc;
+}
+
+// =========================================================================================
+// A1: CountSketch  W1[h(i),:] += sigma(i) V[i,:]   (PAPER.md:236, :240; S1 unscaled, :341)
+// =========================================================================================
+
+// SORTED / gather variant.  One CTA per bucket (grid-stride).  The CTA's threads form
+// R row-slots x LPR lanes-per-row; lane c of slot r owns VEC consecutive columns and sums the
+// bucket's rows r, r+R, r+2R, ... (4 loads in flight per thread), then the R slot sums are
+// added in slot order through shared memory.  Fixed mapping => bit-reproducible W1.
+// HBM-bound: every row of V is read exactly once, 8n contiguous bytes.
+template <int VEC>
+__global__ void __launch_bounds__(256)
+k_countsketch_gather(const double* __restrict__ V, int64_t ldv, int n,
+                     const uint32_t* __restrict__ off, const uint32_t* __restrict__ entries,
+                     uint32_t s1, double* __restrict__ W1)
+{
+    extern __shared__ double red[];                 // R * n doubles
+    const int lpr = (n + VEC - 1) / VEC;            // lanes per row
+    const int R = max(1, 256 / lpr);
+    const int slot = threadIdx.x / lpr;
+    const int col = (threadIdx.x % lpr) * VEC;
+    const bool active = slot < R && col < n;
+    for (uint32_t b = blockIdx.x; b < s1; b += gridDim.x) {
+        const uint32_t beg = off[b], end = off[b + 1];
+        double a0 = 0.0, a1 = 0.0;
+        if (active) {
+            uint32_t k = beg + slot;
+            // 4 rows in flight
+            for (; k + 3u * R < end; k += 4u * R) {
+                uint32_t e[4];
+                double x[4][2];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) e[u] = entries[k + u * R];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const double* p = V + (int64_t)(e[u] & 0x7fffffffu) * ldv + col;
+                    if (VEC == 2) {
+                        double2 t = __ldg(reinterpret_cast<const double2*>(p));
+                        x[u][0] = t.x; x[u][1] = t.y;
+                    } else {
+                        x[u][0] = __ldg(p); x[u][1] = 0.0;
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    if (e[u] >> 31) { a0 -= x[u][0]; a1 -= x[u][1]; }
+                    else            { a0 += x[u][0]; a1 += x[u][1]; }
+                }
+            }
+            for (; k < end; k += R) {
+                uint32_t e = entries[k];
+                const double* p = V + (int64_t)(e & 0x7fffffffu) * ldv + col;
+                double x0, x1 = 0.0;
+                if (VEC == 2) { double2 t = __ldg(reinterpret_cast<const double2*>(p)); x0 = t.x; x1 = t.y; }
+                else x0 = __ldg(p);
+                if (e >> 31) { a0 -= x0; a1 -= x1; } else { a0 += x0; a1 += x1; }
+            }
+            red[slot * n + col] = a0;
+            if (VEC == 2) red[slot * n + col + 1] = a1;
+        }
+        __syncthreads();
+        for (int c = threadIdx.x; c < n; c += blockDim.x) {
+            double s = red[c];
+            for (int r = 1; r < R; ++r) s += red[r * n + c];
+            W1[(int64_t)b * n + c] = s;
+        }
+        __syncthreads();
+    }
+}
+
+// SCATTER variant: stream V in row order, hash on the fly, red.global.add.f64 into W1 (which
+// lives in L2).  Order of the atomics is not fixed => last bits vary run to run.
+__global__ void __launch_bounds__(256)
+k_countsketch_scatter(const double* __restrict__ V, int64_t m, int64_t ldv, int n, int64_t row0,
+                      uint64_t seed, uint32_t s1, double* __restrict__ W1)
+{
+    const int lpr = n < 32 ? n : 32;                // lanes cooperating on one row
+    const int rows_per_warp = 32 / lpr;
+    const int lane = threadIdx.x & 31;
+    const int sub = lane / lpr, c0 = lane % lpr;
+    const int64_t warp_global = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
+    for (int64_t i = warp_global * rows_per_warp + sub; i < m; i += nwarps * rows_per_warp) {
+        if (sub >= rows_per_warp) continue;
+        uint32_t b, neg;
+        rqr_hash_sign(seed, (uint64_t)(row0 + i), s1, b, neg);
+        const double* src = V + i * ldv;
+        double* dst = W1 + (int64_t)b * n;
+        for (int c = c0; c < n; c += lpr) {
+            double x = __ldg(src + c);
+            atomicAdd(dst + c, neg ? -x : x);
+        }
+    }
+}
+
+extern "C" int rqr_countsketch(const double* V, int64_t m, int n, int64_t ldv, int64_t row0,
+                               int64_t s1, uint64_t seed, double* W1, void* work, int variant,
+                               int flags, void* stream)
+{
+    if (!V) return -1;
+    if (m < 1 || m >= ((int64_t)1 << 31)) return -2;
+    if (n < 2 || n > RQR_MAX_N) return -3;
+    if (ldv < n) return -4;
+    if (row0 < 0) return -5;
+    if (s1 < 1 || s1 >= ((int64_t)1 << 31)) return -6;
+    if (!W1) return -8;
+    if (variant != RQR_VARIANT_SORTED && variant != RQR_VARIANT_SCATTER) return -10;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (variant == RQR_VARIANT_SCATTER) {
+        if (cudaMemsetAsync(W1, 0, (size_t)s1 * n * sizeof(double), st) != cudaSuccess)
+            return RQR_ERR_LAUNCH;
+        int64_t want = (m + 7) / 8;
+        int blocks = (int)(want < 148 * 8 ? want : 148 * 8);
+        if (blocks < 1) blocks = 1;
+        k_countsketch_scatter<<<blocks, 256, 0, st>>>(V, m, ldv, n, row0, seed, (uint32_t)s1, W1);
+        RQR_LAUNCH_CHECK();
+        return RQR_OK;
+    }
+    if (!work) return -9;
+    RqrLayout L = rqr_layout(m, n, s1);
+    char* w = (char*)work;
+    uint32_t* off = (uint32_t*)(w + L.B_off);
+    uint32_t* cur = (uint32_t*)(w + L.B_cur);
+    uint32_t* ent = (uint32_t*)(w + L.E);
+    if (!(flags & RQR_FLAG_PREPARED)) {
+        int rc = launch_prepare_sorted(m, row0, s1, seed, off, cur, ent, st);
+        if (rc != RQR_OK) return rc;
+    }
+    const bool vec2 = (n % 2 == 0) && (ldv % 2 == 0) && (((uintptr_t)V & 15) == 0);
+    const int lpr = vec2 ? n / 2 : n;
+    const int R = 256 / lpr > 1 ? 256 / lpr : 1;
+    size_t smem = (size_t)R * n * sizeof(double);
+    int blocks = (int)(s1 < 148 * 8 ? s1 : 148 * 8);
+    if (vec2) k_countsketch_gather<2><<<blocks, 256, smem, st>>>(V, ldv, n, off, ent, (uint32_t)s1, W1);
+    else      k_countsketch_gather<1><<<blocks, 256, smem, st>>>(V, ldv, n, off, ent, (uint32_t)s1, W1);
+    RQR_LAUNCH_CHECK();
+    return RQR_OK;
+}
+
+// =========================================================================================
+// A2: Gaussian sketch  W = S2 W1, split-K GEMM + fixed-order reduction
+// =========================================================================================
+#define GS_BM 64
+#define GS_BN 64
+#define GS_BK 16
+
+// partial[ks] (s2 x n) = S2[:, k0:k1] * W1[k0:k1, :].  64x64 tile per CTA, 4x4 per thread.
+__global__ void __launch_bounds__(256)
+k_gauss_gemm_splitk(const double* __restrict__ S2, const double* __restrict__ W1, int64_t s1,
+                    int n, int s2, int64_t kchunk, double* __restrict__ part)
+{
+    __shared__ double As[GS_BK][GS_BM + 1];
+    __shared__ double Bs[GS_BK][GS_BN];
+    const int tid = threadIdx.x;
+    const int tx = tid & 15, ty = tid >> 4;       // 16 x 16 threads
+    const int row_base = blockIdx.y * GS_BM, col_base = blockIdx.x * GS_BN;
+    const int64_t k0 = (int64_t)blockIdx.z * kchunk;
+    const int64_t k1 = k0 + kchunk < s1 ? k0 + kchunk : s1;
+    double acc[4][4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j] = 0.0;
+    for (int64_t kk = k0; kk < k1; kk += GS_BK) {
+        // A tile: 64 rows x 16 k  (1024 elements, 4 per thread), k fastest in global
+#pragma unroll
+        for (int t = 0; t < 4; ++t) {
+            int idx = tid + t * 256;
+            int r = idx >> 4, k = idx & 15;
+            int gr = row_base + r; int64_t gk = kk + k;
+            As[k][r] = (gr < s2 && gk < k1) ? S2[(int64_t)gr * s1 + gk] : 0.0;
+        }
+        // B tile: 16 k x 64 cols
+#pragma unroll
+        for (int t = 0; t < 4; ++t) {
+            int idx = tid + t * 256;
+            int k = idx >> 6, c = idx & 63;
+            int gc = col_base + c; int64_t gk = kk + k;
+            Bs[k][c] = (gc < n && gk < k1) ? W1[gk * n + gc] : 0.0;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < GS_BK; ++k) {
+            double a[4], b[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) a[i] = As[k][ty + 16 * i];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) b[j] = Bs[k][tx + 16 * j];
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) acc[i][j] = fma(a[i], b[j], acc[i][j]);
+        }
+        __syncthreads();
+    }
+    double* P = part + (int64_t)blockIdx.z * s2 * n;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        int gr = row_base + ty + 16 * i;
+        if (gr >= s2) continue;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            int gc = col_base + tx + 16 * j;
+            if (gc < n) P[(int64_t)gr * n + gc] = acc[i][j];
+        }
+    }
+}
+
+// out[e] = sum_{p ascending} part[p][e]
+__global__ void k_reduce_partials(const double* __restrict__ part, int nparts, int64_t elems,
+                                  double* __restrict__ out)
+{
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < elems;
+         e += (int64_t)gridDim.x * blockDim.x) {
+        double s = part[e];
+        for (int p = 1; p < nparts; ++p) s += part[(int64_t)p * elems + e];
+        out[e] = s;
+    }
+}
+
+extern "C" const double* rqr_workspace_S2(void* work, int n, int64_t s1)
+{
+    RqrLayout L = rqr_layout(1, n, s1);
+    return (const double*)((char*)work + L.C);
+}
+
+extern "C" int rqr_gauss_sketch(const double* W1, int64_t s1, int n, int s2, uint64_t seed,
+                                double* W, void* work, int flags, void* stream)
+{
+    if (!W1) return -1;
+    if (s1 < 1 || s1 >= ((int64_t)1 << 31)) return -2;
+    if (n < 2 || n > RQR_MAX_N) return -3;
+    if (s2 < 1 || s2 > RQR_MAX_S2 || s2 > s1) return -4;
+    if (!W) return -6;
+    if (!work) return -7;
+    cudaStream_t st = (cudaStream_t)stream;
+    RqrLayout L = rqr_layout(1, n, s1);
+    char* w = (char*)work;
+    double* S2 = (double*)(w + L.C);
+    double* part = (double*)(w + L.D);
+    if (!(flags & RQR_FLAG_PREPARED)) {
+        int rc = launch_prepare_S2(s1, s2, seed, S2, st);
+        if (rc != RQR_OK) return rc;
+    }
+    int tiles_m = (s2 + GS_BM - 1) / GS_BM, tiles_n = (n + GS_BN - 1) / GS_BN;
+    int64_t ks = 296 / (tiles_m * tiles_n);
+    int64_t ks_cap = RQR_GAUSS_PARTIAL_ROWS / s2;
+    if (ks > ks_cap) ks = ks_cap;
+    int64_t kblocks = (s1 + GS_BK - 1) / GS_BK;
+    if (ks > kblocks) ks = kblocks;
+    if (ks < 1) ks = 1;
+    int64_t kchunk = ((kblocks + ks - 1) / ks) * GS_BK;
+    ks = (s1 + kchunk - 1) / kchunk;
+    dim3 grid(tiles_n, tiles_m, (unsigned)ks);
+    k_gauss_gemm_splitk<<<grid, 256, 0, st>>>(S2, W1, s1, n, s2, kchunk, part);
+    RQR_LAUNCH_CHECK();
+    int64_t elems = (int64_t)s2 * n;
+    int rb = (int)((elems + 255) / 256);
+    k_reduce_partials<<<rb, 256, 0, st>>>(part, (int)ks, elems, W);
+    RQR_LAUNCH_CHECK();
+    return RQR_OK;
+}
+
+// =========================================================================================
+// Single dense Gaussian sketch  W = S V,  S (s x m_total) = N(0,1)/sqrt(s) generated on the
+// fly from Philox stream 3.  Comparator only.
+// grid = (P persistent row-chunk walkers, ceil(s/32) sketch-row tiles).
+// =========================================================================================
+#define DG_ROWS 32
+__global__ void __launch_bounds__(256)
+k_dense_gauss_sketch(const double* __restrict__ V, int64_t m, int n, int64_t ldv, int64_t row0,
+                     int64_t m_total, int s, uint64_t seed, double* __restrict__ part)
+{
+    extern __shared__ double sm[];
+    double* St = sm;                         // [32][33]
+    double* Vt = sm + 32 * 33;               // [32][n]
+    const int tid = threadIdx.x;
+    const int r = tid >> 3, cq = tid & 7;
+    const int srow = blockIdx.y * 32 + r;
+    const double d = sqrt((double)s);
+    double acc[RQR_MAX_N / 8];
+#pragma unroll
+    for (int j = 0; j < RQR_MAX_N / 8; ++j) acc[j] = 0.0;
+    const int64_t nchunks = (m + DG_ROWS - 1) / DG_ROWS;
+    for (int64_t ch = blockIdx.x; ch < nchunks; ch += gridDim.x) {
+        const int64_t i0 = ch * DG_ROWS;
+        for (int t = tid; t < 32 * 32; t += 256) {
+            int rr = t >> 5, ii = t & 31;
+            int sr = blockIdx.y * 32 + rr;
+            double val = 0.0;
+            if (sr < s && i0 + ii < m) {
+                uint64_t e = (uint64_t)sr * (uint64_t)m_total + (uint64_t)(row0 + i0 + ii);
+                val = rqr_gauss_entry(seed, e, RQR_PHILOX_STREAM_DENSE) / d;
+            }
+            St[rr * 33 + ii] = val;
+        }
+        for (int t = tid; t < 32 * n; t += 256) {
+            int ii = t / n, c = t - ii * n;
+            Vt[t] = (i0 + ii < m) ? V[(i0 + ii) * ldv + c] : 0.0;
+        }
+        __syncthreads();
+        for (int ii = 0; ii < 32; ++ii) {
+            const double a = St[r * 33 + ii];
+#pragma unroll
+            for (int j = 0; j < RQR_MAX_N / 8; ++j) {
+                int c = cq + 8 * j;
+                if (c < n) acc[j] = fma(a, Vt[ii * n + c], acc[j]);
+            }
+        }
+        __syncthreads();
+    }
+    if (srow < s) {
+        double* P = part + ((int64_t)blockIdx.x * s + srow) * n;
+#pragma unroll
+        for (int j = 0; j < RQR_MAX_N / 8; ++j) {
+            int c = cq + 8 * j;
+            if (c < n) P[c] = acc[j];
+        }
+    }
+}
+
+extern "C" int rqr_dense_gauss_sketch(const double* V, int64_t m, int n, int64_t ldv, int64_t row0,
+                                      int64_t m_total, int s, uint64_t seed, double* W, void* work,
+                                      void* stream)
+{
+    if (!V) return -1;
+    if (m < 1) return -2;
+    if (n < 2 || n > RQR_MAX_N) return -3;
+    if (ldv < n) return -4;
+    if (row0 < 0 || row0 + m > m_total) return -5;
+    if (s < 1 || s > RQR_MAX_S2) return -7;
+    if (!W) return -9;
+    if (!work) return -10;
+    cudaStream_t st = (cudaStream_t)stream;
+    double* part = (double*)((char*)work + 256);      // region A
+    int stiles = (s + 31) / 32;
+    int64_t nchunks = (m + DG_ROWS - 1) / DG_ROWS;
+    int64_t P = (148 * 4) / stiles;
+    int64_t Pcap = ((int64_t)RQR_MAX_GRAM_PARTIALS * n) / s;
+    if (P > Pcap) P = Pcap;
+    if (P > nchunks) P = nchunks;
+    if (P < 1) P = 1;
+    size_t smem = (size_t)(32 * 33 + 32 * n) * sizeof(double);
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaFuncSetAttribute(k_dense_gauss_sketch, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+        attr_set = true;
+    }
+    dim3 grid((unsigned)P, stiles);
+    k_dense_gauss_sketch<<<grid, 256, smem, st>>>(V, m, n, ldv, row0, m_total, s, seed, part);
+    RQR_LAUNCH_CHECK();
+    int64_t elems = (int64_t)s * n;
+    k_reduce_partials<<<(int)((elems + 255) / 256), 256, 0, st>>>(part, (int)P, elems, W);
+    RQR_LAUNCH_CHECK();
+    return RQR_OK;
+}
+
+// =========================================================================================
+// Inspection helpers for the parity tests
+// =========================================================================================
+__global__ void k_debug_hash_sign(uint64_t seed, int64_t row0, int64_t count, uint32_t s1,
+                                  uint32_t* __restrict__ bucket, int8_t* __restrict__ sign)
+{
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < count;
+         i += (int64_t)gridDim.x * blockDim.x) {
+        uint32_t b, neg;
+        rqr_hash_sign(seed, (uint64_t)(row0 + i), s1, b, neg);
+        bucket[i] = b;
+        sign[i] = neg ? (int8_t)-1 : (int8_t)1;
+    }
+}
+
+__global__ void k_debug_gauss(uint64_t seed, uint32_t stream_id, uint64_t first, int64_t count,
+                              double* __restrict__ z)
+{
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < count;
+         i += (int64_t)gridDim.x * blockDim.x)
+        z[i] = rqr_gauss_entry(seed, first + (uint64_t)i, stream_id);
+}
+
+extern "C" int rqr_debug_hash_sign(uint64_t seed, int64_t row0, int64_t count, int64_t s1,
+                                   uint32_t* bucket, int8_t* sign, void* stream)
+{
+    if (count < 1) return -3;
+    if (s1 < 1 || s1 >= ((int64_t)1 << 31)) return -4;
+    if (!bucket) return -5;
+    if (!sign) return -6;
+    int blocks = (int)((count + 255) / 256 < 4096 ? (count + 255) / 256 : 4096);
+    k_debug_hash_sign<<<blocks, 256, 0, (cudaStream_t)stream>>>(seed, row0, count, (uint32_t)s1, bucket, sign);
+    RQR_LAUNCH_CHECK();
+    return RQR_OK;
+}
+
+extern "C" int rqr_debug_gauss(uint64_t seed, uint32_t stream_id, uint64_t first, int64_t count,
+                               double* z, void* stream)
+{
+    if (count < 1) return -4;
+    if (!z) return -5;
+    int blocks = (int)((count + 255) / 256 < 4096 ? (count + 255) / 256 : 4096);
+    k_debug_gauss<<<blocks, 256, 0, (cudaStream_t)stream>>>(seed, stream_id, first, count, z);
+    RQR_LAUNCH_CHECK();
+    return RQR_OK;
+}

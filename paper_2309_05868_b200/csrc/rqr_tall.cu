@@ -1,0 +1,176 @@
+// rqr_tall.cu -- the m-sized passes: A4 fused V R0^-1 + Gram (rqr_trsm_gram) and A6 triangular
+// apply (rqr_apply).  This file holds the GENERIC kernels (any 2 <= n <= 256, any ld); the
+// DMMA fast paths live in rqr_tall_mma.cu and are dispatched from here.
+#include "rqr_common.cuh"
+#include "rqr_tall.cuh"
+
+#define GEN_TR 64      // rows per tile in the generic kernels
+
+// One row of X = V R^-1 by forward substitution (eq. (42)), in place in a
+// shared-memory row.  Explicit fma so that every kernel that calls it rounds identically (H1).
+__device__ __forceinline__ void row_trsm_inplace(double* __restrict__ x, const double* __restrict__ R,
+                                                 int n)
+{
+    for (int j = 0; j < n; ++j) {
+        double acc = x[j];
+        for (int k = 0; k < j; ++k) acc = fma(-x[k], __ldg(R + k * n + j), acc);
+        x[j] = acc / __ldg(R + j * n + j);
+    }
+}
+
+// Generic A4: per 64-row tile: load, optional row-wise substitution, optional store of V1, then
+// this CTA's partial Gram (upper triangle) accumulated in its own slice of `part`.
+__global__ void __launch_bounds__(256)
+k_trsm_gram_generic(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
+                    const double* __restrict__ R0, double* __restrict__ V1, int64_t ldq,
+                    double* __restrict__ part)
+{
+    extern __shared__ double Xs[];                // GEN_TR x (n+1)
+    const int ld = n + 1;
+    const int tid = threadIdx.x;
+    double* P = part + (int64_t)blockIdx.x * n * n;
+    for (int e = tid; e < n * n; e += 256) P[e] = 0.0;
+    const int64_t ntiles = (m + GEN_TR - 1) / GEN_TR;
+    for (int64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        const int64_t i0 = t * GEN_TR;
+        const int rows = (int)((m - i0) < GEN_TR ? (m - i0) : GEN_TR);
+        __syncthreads();
+        for (int e = tid; e < GEN_TR * n; e += 256) {
+            int r = e / n, c = e - r * n;
+            Xs[r * ld + c] = (r < rows) ? V[(i0 + r) * ldv + c] : 0.0;
+        }
+        __syncthreads();
+        if (R0 && tid < rows) row_trsm_inplace(Xs + tid * ld, R0, n);
+        __syncthreads();
+        if (V1) {
+            for (int e = tid; e < rows * n; e += 256) {
+                int r = e / n, c = e - r * n;
+                V1[(i0 + r) * ldq + c] = Xs[r * ld + c];
+            }
+        }
+        for (int e = tid; e < n * n; e += 256) {
+            int a = e / n, b = e - a * n;
+            if (b < a) continue;
+            double s = 0.0;
+            for (int r = 0; r < GEN_TR; ++r) s = fma(Xs[r * ld + a], Xs[r * ld + b], s);
+            P[e] += s;
+        }
+    }
+}
+
+// G[a][b] = G[b][a] = sum_p part[p][a][b] (a <= b), p ascending
+__global__ void k_gram_reduce(const double* __restrict__ part, int nparts, int n,
+                              double* __restrict__ G)
+{
+    for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < n * n; e += gridDim.x * blockDim.x) {
+        int a = e / n, b = e - a * n;
+        if (b < a) continue;
+        double s = part[e];
+        for (int p = 1; p < nparts; ++p) s += part[(int64_t)p * n * n + e];
+        G[a * n + b] = s;
+        G[b * n + a] = s;
+    }
+}
+
+// Generic A6: Q = (V R0^-1) R1^-1 row by row; R0 == NULL: Q = V R1^-1.
+__global__ void __launch_bounds__(256)
+k_apply_generic(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
+                const double* __restrict__ R0, const double* __restrict__ R1,
+                double* __restrict__ Q, int64_t ldq)
+{
+    extern __shared__ double Xs[];
+    const int ld = n + 1;
+    const int tid = threadIdx.x;
+    const int64_t ntiles = (m + GEN_TR - 1) / GEN_TR;
+    for (int64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        const int64_t i0 = t * GEN_TR;
+        const int rows = (int)((m - i0) < GEN_TR ? (m - i0) : GEN_TR);
+        __syncthreads();
+        for (int e = tid; e < rows * n; e += 256) {
+            int r = e / n, c = e - r * n;
+            Xs[r * ld + c] = V[(i0 + r) * ldv + c];
+        }
+        __syncthreads();
+        if (tid < rows) {
+            if (R0) row_trsm_inplace(Xs + tid * ld, R0, n);
+            row_trsm_inplace(Xs + tid * ld, R1, n);
+        }
+        __syncthreads();
+        for (int e = tid; e < rows * n; e += 256) {
+            int r = e / n, c = e - r * n;
+            Q[(i0 + r) * ldq + c] = Xs[r * ld + c];
+        }
+    }
+}
+
+static int generic_grid(int64_t m)
+{
+    int64_t ntiles = (m + GEN_TR - 1) / GEN_TR;
+    int64_t g = ntiles < RQR_MAX_GRAM_PARTIALS ? ntiles : RQR_MAX_GRAM_PARTIALS;
+    return (int)(g < 1 ? 1 : g);
+}
+
+static void generic_attrs()
+{
+    static bool done = false;
+    if (done) return;
+    cudaFuncSetAttribute(k_trsm_gram_generic, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
+    cudaFuncSetAttribute(k_apply_generic, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
+    done = true;
+}
+
+static int g_force_generic = 0;
+extern "C" void rqr_debug_force_generic(int on) { g_force_generic = on; }
+
+extern "C" int rqr_trsm_gram(const double* V, int64_t m, int n, int64_t ldv, const double* R0,
+                             double* G, double* V1, int64_t ldq, void* work, void* stream)
+{
+    if (!V) return -1;
+    if (m < 1 || m >= ((int64_t)1 << 31)) return -2;
+    if (n < 2 || n > RQR_MAX_N) return -3;
+    if (ldv < n) return -4;
+    if (!G) return -6;
+    if (V1 && ldq < n) return -8;
+    if (!work) return -9;
+    cudaStream_t st = (cudaStream_t)stream;
+    double* part = (double*)((char*)work + 256);        // region A
+    int nparts = 0;
+    int rc = g_force_generic ? RQR_TALL_NOT_HANDLED
+                             : rqr_trsm_gram_mma(V, m, n, ldv, R0, V1, ldq, part, &nparts, st);
+    if (rc == RQR_TALL_NOT_HANDLED) {
+        generic_attrs();
+        nparts = generic_grid(m);
+        size_t smem = (size_t)GEN_TR * (n + 1) * sizeof(double);
+        k_trsm_gram_generic<<<nparts, 256, smem, st>>>(V, m, n, ldv, R0, V1, ldq, part);
+        RQR_LAUNCH_CHECK();
+    } else if (rc != RQR_OK) return rc;
+    int rb = (n * n + 255) / 256;
+    k_gram_reduce<<<rb, 256, 0, st>>>(part, nparts, n, G);
+    RQR_LAUNCH_CHECK();
+    return RQR_OK;
+}
+
+extern "C" int rqr_apply(const double* V, int64_t m, int n, int64_t ldv, const double* R0,
+                         const double* R1, double* Q, int64_t ldq, void* work, void* stream)
+{
+    if (!V) return -1;
+    if (m < 1 || m >= ((int64_t)1 << 31)) return -2;
+    if (n < 2 || n > RQR_MAX_N) return -3;
+    if (ldv < n) return -4;
+    if (!R1) return -6;
+    if (!Q) return -7;
+    if (ldq < n) return -8;
+    (void)work;
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = g_force_generic ? RQR_TALL_NOT_HANDLED : rqr_apply_mma(V, m, n, ldv, R0, R1, Q, ldq, st);
+    if (rc == RQR_TALL_NOT_HANDLED) {
+        generic_attrs();
+        size_t smem = (size_t)GEN_TR * (n + 1) * sizeof(double);
+        int64_t ntiles = (m + GEN_TR - 1) / GEN_TR;
+        int grid = (int)(ntiles < 148 * 8 ? ntiles : 148 * 8);
+        k_apply_generic<<<grid, 256, smem, st>>>(V, m, n, ldv, R0, R1, Q, ldq);
+        RQR_LAUNCH_CHECK();
+        return RQR_OK;
+    }
+    return rc;
+}

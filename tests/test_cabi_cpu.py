@@ -1,0 +1,94 @@
+"""CPU-side checks of the C-ABI library: it builds, loads, exports every symbol the headers
+declare, and rejects bad arguments before touching the GPU.  No compute calls here."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2309_05868_b200 import build
+    build.build_lib()
+    from paper_2309_05868_b200 import binding
+    return binding.lib()
+
+
+def declared_symbols():
+    names = set()
+    inc = os.path.join(ROOT, "include")
+    for f in os.listdir(inc):
+        if f.endswith(".h"):
+            src = open(os.path.join(inc, f)).read()
+            src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+            names |= set(re.findall(r"\b(rqr_[a-zA-Z0-9_]+)\s*\(", src))
+    return names
+
+
+def test_every_declared_symbol_is_exported(lib):
+    names = declared_symbols()
+    assert {"rqr_countsketch", "rqr_gauss_sketch", "rqr_small_geqrf", "rqr_trsm_gram", "rqr_chol",
+            "rqr_apply", "rqr_rand_cholqr", "rqr_cholqr2", "rqr_scholqr3"} <= names
+    for n in names:
+        assert hasattr(lib, n), n
+    from paper_2309_05868_b200 import binding
+    assert names == set(binding.SIGNATURES), names ^ set(binding.SIGNATURES)
+
+
+def test_version_and_workspace(lib):
+    assert b"rqr" in lib.rqr_version()
+    b1 = lib.rqr_workspace_bytes(1 << 20, 64, 8192, 128, 0)
+    b2 = lib.rqr_workspace_bytes(1 << 23, 64, 8192, 128, 0)
+    assert 0 < b1 < b2 < (1 << 30)
+    assert b2 - b1 == ((1 << 23) - (1 << 20)) * 4          # only the sorted row list grows with m
+    assert lib.rqr_workspace_bytes(100, 1, 10, 10, 0) == 0   # n < 2
+    assert lib.rqr_workspace_bytes(100, 300, 10, 10, 0) == 0
+
+
+def test_argument_validation_without_gpu(lib):
+    one = ctypes.c_void_p(16)   # non-null dummy, never dereferenced: checks come first
+    z = ctypes.c_void_p(0)
+    assert lib.rqr_countsketch(z, 10, 4, 4, 0, 8, 1, one, one, 0, 0, z) == -1
+    assert lib.rqr_countsketch(one, 10, 1, 4, 0, 8, 1, one, one, 0, 0, z) == -3
+    assert lib.rqr_countsketch(one, 10, 4, 3, 0, 8, 1, one, one, 0, 0, z) == -4     # ldv < n
+    assert lib.rqr_countsketch(one, 10, 4, 4, 0, 8, 1, one, one, 7, 0, z) == -10
+    assert lib.rqr_gauss_sketch(one, 8, 4, 9, 1, one, one, 0, z) == -4              # s2 > s1
+    assert lib.rqr_small_geqrf(one, 3, 4, one, z, z) == -3                          # n > s2
+    assert lib.rqr_trsm_gram(one, 10, 4, 2, z, one, z, 4, one, z) == -4
+    assert lib.rqr_chol(z, 4, 0.0, one, z, z) == -1
+    assert lib.rqr_apply(one, 10, 4, 4, z, z, one, 4, z, z) == -6
+    assert lib.rqr_triu_mul(one, one, 4, one, z) == -4                              # aliasing
+    # eq. (20): 1 < n <= s2 <= s1 <= m
+    assert lib.rqr_rand_cholqr(one, 100, 8, 200, 16, 1, one, one, one, z, 0, 0, z) == -4   # s1 > m
+    assert lib.rqr_rand_cholqr(one, 100, 8, 64, 4, 1, one, one, one, z, 0, 0, z) == -5     # s2 < n
+    assert lib.rqr_rand_cholqr(one, 100, 8, 64, 80, 1, one, one, one, z, 0, 0, z) == -5    # s2 > s1
+    assert lib.rqr_rand_cholqr(one, 4, 8, 4, 8, 1, one, one, one, z, 0, 0, z) == -3        # n > m
+    assert lib.rqr_cholqr2(z, 100, 8, one, one, one, z, z) == -1
+    assert lib.rqr_sketch_prepare(100, 8, 0, 64, 600, 1, 0, one, z) == -5
+    assert lib.rqr_probe_fp64(5, 1, 1, one, z, z) == -1
+
+
+def test_binding_refuses_cpu_tensors(lib):
+    import torch
+    from paper_2309_05868_b200 import binding
+    V = torch.zeros(8, 4, dtype=torch.float64)
+    with pytest.raises(binding.RqrError):
+        binding.countsketch(V, 4, 1, torch.zeros(4, 4, dtype=torch.float64), None)
+
+
+def test_product_does_not_import_oracle():
+    bad = re.compile(r"^\s*(import|from)\s+\S*oracle|#include.*oracle|librqr_oracle|CDLL\(.*oracle")
+    pkg = os.path.join(ROOT, "paper_2309_05868_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                for ln in open(os.path.join(dirpath, f)).read().splitlines():
+                    assert not bad.search(ln), (f, ln)
+    bad2 = re.compile(r"^\s*(import|from)\s+paper_2309_05868_b200|#include\s+\"[^\"]*(rqr\.h|csrc|\.cuh)|CDLL\(.*librqr\.so")
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith(".py") or f.endswith(".c"):
+            for ln in open(os.path.join(ROOT, "oracle", f)).read().splitlines():
+                assert not bad2.search(ln), (f, ln)

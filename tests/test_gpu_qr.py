@@ -1,0 +1,192 @@
+"""GPU parity of the one-shot drivers against the oracle and against what the paper proves.
+Q is not unique entry by entry at large kappa: compare the
+invariants (Thm 5.3), the structure of R, and R norm-wise against the oracle.
+The checks themselves use torch float64 library ops, not the library under test."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2309_05868_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+ORTH_TOL = 1e-12      # BASELINE.json north_star
+RES_TOL = 1e-13
+R_TOL = 1e-9
+
+
+@pytest.fixture(scope="module")
+def rq():
+    from paper_2309_05868_b200 import binding
+    binding.lib()
+    assert torch.cuda.is_available()
+    return binding
+
+
+def orth_err(Q):
+    n = Q.shape[1]
+    return float(torch.linalg.norm(Q.T @ Q - torch.eye(n, dtype=Q.dtype, device=Q.device)))
+
+
+def resid(V, Q, R):
+    return float(torch.linalg.norm(V - Q @ R) / torch.linalg.norm(V))
+
+
+def check_R(R):
+    Rh = R.cpu().numpy()
+    assert np.array_equal(np.tril(Rh, -1), np.zeros_like(Rh))
+    assert (np.diag(Rh) > 0).all()
+
+
+def run_rand(rq, Vd, s1, s2, seed, variant=0, flags=0, prepared=False):
+    m, n = Vd.shape
+    Q = torch.empty_like(Vd)
+    R = torch.empty(n, n, dtype=torch.float64, device="cuda")
+    work = rq.alloc_workspace(m, n, s1, s2, variant)
+    info = rq.new_info()
+    if prepared:
+        rq.sketch_prepare(m, n, s1, s2, seed, work, variant)
+        flags |= rq.FLAG_PREPARED
+    rq.rand_cholqr(Vd, s1, s2, seed, Q, R, work, info, variant, flags)
+    torch.cuda.synchronize()
+    return Q, R, int(info.item())
+
+
+CASES = [("C1", 20000, 16, 1e10), ("n64", 65536, 64, 1e12), ("n70", 100000, 70, 1e8),
+         ("n32", 40000, 32, 1e14), ("n128", 40000, 128, 1e12), ("n256", 140000, 256, 1e14),
+         ("tiny", 600, 8, 1e5), ("ragged", 4099, 24, 1e6)]
+
+
+@pytest.mark.parametrize("name,m,n,kappa", CASES)
+def test_rand_cholqr_matches_oracle(rq, orc, name, m, n, kappa):
+    s1, s2 = inputs.sketch_sizes(n)
+    V = inputs.make_V(m, n, kappa, 1234)
+    Vd = V.cuda()
+    Qo, Ro, io = orc.rand_cholqr(V.numpy(), s1, s2, 42)
+    assert io == 0
+    for variant, flags, prepared in [(0, 0, False), (0, rq.FLAG_RECOMPUTE_V1, True), (1, 0, True)]:
+        Q, R, info = run_rand(rq, Vd, s1, s2, 42, variant, flags, prepared)
+        assert info == 0
+        assert orth_err(Q) <= ORTH_TOL
+        assert resid(Vd, Q, R) <= RES_TOL
+        check_R(R)
+        Rh = R.cpu().numpy()
+        assert np.linalg.norm(Rh - Ro) <= R_TOL * np.linalg.norm(Ro)
+    # the oracle satisfies the same bounds on the same input (both sides, north_star)
+    Qot = torch.from_numpy(Qo)
+    assert orth_err(Qot) <= ORTH_TOL and resid(V, Qot, torch.from_numpy(Ro)) <= RES_TOL
+
+
+def test_rand_cholqr_in_place_and_seeds(rq, orc):
+    m, n = 30000, 32
+    s1, s2 = inputs.sketch_sizes(n)
+    Vd = inputs.make_V(m, n, 1e10, 5).cuda()
+    Rs = []
+    for seed in inputs.SKETCH_SEEDS:
+        Q, R, info = run_rand(rq, Vd, s1, s2, seed)
+        assert info == 0 and orth_err(Q) <= ORTH_TOL and resid(Vd, Q, R) <= RES_TOL
+        Rs.append(R)
+    # QR with positive diagonal is unique: any sketch seed gives the same R norm-wise
+    assert float(torch.linalg.norm(Rs[0] - Rs[1]) / torch.linalg.norm(Rs[0])) <= R_TOL
+    assert float(torch.linalg.norm(Rs[0] - Rs[2]) / torch.linalg.norm(Rs[0])) <= R_TOL
+    X = Vd.clone()
+    R = torch.empty(n, n, dtype=torch.float64, device="cuda")
+    work = rq.alloc_workspace(m, n, s1, s2)
+    info = rq.new_info()
+    rq.rand_cholqr(X, s1, s2, 42, X, R, work, info)          # Q == V
+    assert int(info.item()) == 0 and orth_err(X) <= ORTH_TOL and resid(Vd, X, R) <= RES_TOL
+
+
+def test_rank_deficient_input_reports_singular(rq):
+    V = torch.zeros(2000, 8, dtype=torch.float64, device="cuda")
+    V[:, 0] = 1.0
+    _, _, info = run_rand(rq, V, 128, 16, 42)
+    assert info >= rq.INFO_SINGULAR
+
+
+@pytest.mark.parametrize("n", [32, 64])
+def test_kappa_sweep_vs_comparators(rq, orc, n):
+    """Fig. 4: rand_cholQR O(u) for every kappa; cholQR2 fails past ~1e8;
+    sCholQR3 holds to 1e12."""
+    m = 65536
+    s1, s2 = inputs.sketch_sizes(n)
+    work = rq.alloc_workspace(m, n, s1, s2)
+    info = rq.new_info()
+    R = torch.empty(n, n, dtype=torch.float64, device="cuda")
+    for kappa in (1e0, 1e4, 1e8, 1e12, 1e15):
+        Vd = inputs.make_V(m, n, kappa, 77).cuda()
+        Q = torch.empty_like(Vd)
+        rq.rand_cholqr(Vd, s1, s2, 42, Q, R, work, info)
+        assert int(info.item()) == 0 and orth_err(Q) <= ORTH_TOL and resid(Vd, Q, R) <= RES_TOL
+        rq.cholqr2(Vd, Q, R, work, info)
+        i2 = int(info.item())
+        if kappa <= 1e6:
+            assert i2 == 0 and orth_err(Q) <= ORTH_TOL and resid(Vd, Q, R) <= RES_TOL
+            check_R(R)
+        if kappa >= 1e10:
+            assert i2 >= rq.INFO_NOT_SPD or orth_err(Q) > 1e3 * ORTH_TOL
+        rq.scholqr3(Vd, Q, R, work, info)
+        i3 = int(info.item())
+        if kappa <= 1e12:
+            assert i3 == 0 and orth_err(Q) <= ORTH_TOL and resid(Vd, Q, R) <= RES_TOL
+            check_R(R)
+
+
+def test_comparators_match_oracle(rq, orc):
+    m, n = 30000, 24
+    V = inputs.make_V(m, n, 1e5, 9)
+    Vd = V.cuda()
+    work = rq.alloc_workspace(m, n, 2 * n * n, 2 * n)
+    info = rq.new_info()
+    Q = torch.empty_like(Vd)
+    R = torch.empty(n, n, dtype=torch.float64, device="cuda")
+    rq.cholqr2(Vd, Q, R, work, info)
+    _, Ro, io = orc.cholqr2(V.numpy())
+    assert int(info.item()) == 0 and io == 0
+    assert np.linalg.norm(R.cpu().numpy() - Ro) <= R_TOL * np.linalg.norm(Ro)
+    rq.scholqr3(Vd, Q, R, work, info)
+    _, Ro, io, _ = orc.scholqr3(V.numpy())
+    assert int(info.item()) == 0 and io == 0
+    assert np.linalg.norm(R.cpu().numpy() - Ro) <= R_TOL * np.linalg.norm(Ro)
+    assert orth_err(Q) <= ORTH_TOL
+    rq.gauss_randcholqr(Vd, 2 * n, 42, Q, R, work, info)
+    _, Ro, io = orc.gauss_rand_cholqr(V.numpy(), 2 * n, 42)
+    assert int(info.item()) == 0 and io == 0
+    assert np.linalg.norm(R.cpu().numpy() - Ro) <= R_TOL * np.linalg.norm(Ro)
+    assert orth_err(Q) <= ORTH_TOL and resid(Vd, Q, R) <= RES_TOL
+
+
+def test_stress_inputs(rq):
+    n = 64
+    s1, s2 = inputs.sketch_sizes(n)
+    for V in (inputs.make_graded_V(50000, n, 14, 5), inputs.make_vandermonde_V(50000, n)):
+        Vd = V.cuda()
+        Q, R, info = run_rand(rq, Vd, s1, s2, 42)
+        assert info == 0 and resid(Vd, Q, R) <= RES_TOL
+        check_R(R)
+    Q, R, info = run_rand(rq, inputs.make_graded_V(50000, n, 14, 5).cuda(), s1, s2, 42)
+    assert orth_err(Q) <= ORTH_TOL
+
+
+def test_graph_capture_of_one_shot(rq):
+    """The C ABI promises no synchronisation or allocation: the whole factorization must be
+    capturable in a CUDA graph (bench.py times it that way)."""
+    m, n = 20000, 16
+    s1, s2 = inputs.sketch_sizes(n)
+    Vd = inputs.make_V(m, n, 1e10, 1234).cuda()
+    Q = torch.empty_like(Vd)
+    R = torch.empty(n, n, dtype=torch.float64, device="cuda")
+    work = rq.alloc_workspace(m, n, s1, s2)
+    info = rq.new_info()
+    rq.sketch_prepare(m, n, s1, s2, 42, work)
+    rq.rand_cholqr(Vd, s1, s2, 42, Q, R, work, info, 0, rq.FLAG_PREPARED)   # warm up (func attrs)
+    torch.cuda.synchronize()
+    Q.zero_(); R.zero_()
+    g = torch.cuda.CUDAGraph()
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        with torch.cuda.graph(g, stream=st):
+            rq.rand_cholqr(Vd, s1, s2, 42, Q, R, work, info, 0, rq.FLAG_PREPARED)
+    g.replay()
+    torch.cuda.synchronize()
+    assert int(info.item()) == 0 and orth_err(Q) <= ORTH_TOL and resid(Vd, Q, R) <= RES_TOL

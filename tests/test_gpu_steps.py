@@ -1,0 +1,253 @@
+"""GPU parity, step by step: every C-ABI entry point against the CPU oracle on the same seeded
+inputs (element by element where the result is unique, invariants where it is not).
+Tolerances: integer/index work bit-exact; Gaussian entries 1e-15
+(north_star); sums and triangular solves with well-conditioned factors 1e-13 relative."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2309_05868_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def rq():
+    from paper_2309_05868_b200 import binding
+    binding.lib()
+    assert torch.cuda.is_available()
+    return binding
+
+
+def dev(a):
+    return torch.as_tensor(np.ascontiguousarray(a)).cuda()
+
+
+def host(t):
+    return t.detach().cpu().numpy()
+
+
+@pytest.mark.parametrize("s1,row0,count", [(512, 0, 5000), (8192, 0, 70000), (9940, 123, 4097),
+                                           (8192, (1 << 33) + 5, 300), (131072, 7, 20000)])
+def test_hash_sign_bit_exact(rq, orc, s1, row0, count):
+    b, s = rq.debug_hash_sign(42, row0, count, s1)
+    bo, so = orc.hash_sign(42, row0, count, s1)
+    assert np.array_equal(host(b).astype(np.uint32), bo)
+    assert np.array_equal(host(s), so)
+
+
+def test_gauss_entries_within_1e15(rq, orc):
+    for stream, first, count in [(1, 0, 200001), (3, (1 << 40) + 1, 50001), (1, 12345, 7)]:
+        z = host(rq.debug_gauss(42, stream, first, count))
+        zo = orc.gauss_z(42, stream, first, count)
+        assert np.all(np.abs(z - zo) <= 1e-15 * np.maximum(np.abs(zo), 1.0))
+        assert np.max(np.abs(z - zo) / np.maximum(np.abs(zo), 1e-3)) < 1e-12
+
+
+def test_prepared_S2_matches_oracle(rq, orc):
+    m, n = 4096, 16
+    s1, s2 = 700, 33                      # odd sizes: pairs straddle rows
+    work = rq.alloc_workspace(m, n, s1, s2)
+    rq.sketch_prepare(m, n, s1, s2, 43, work)
+    S2 = host(rq.workspace_S2(work, n, s1, s2))
+    S2o = orc.gauss_matrix(43, s2, s1)
+    assert np.all(np.abs(S2 - S2o) <= 1e-15 * np.maximum(np.abs(S2o), 1.0 / np.sqrt(s2)))
+
+
+@pytest.mark.parametrize("m,n,s1", [(20000, 16, 512), (100000, 70, 9940), (65536, 64, 8192),
+                                    (5000, 33, 64), (3000, 256, 4000), (37, 8, 16), (8192, 2, 8)])
+@pytest.mark.parametrize("variant", [0, 1])
+def test_countsketch_parity(rq, orc, m, n, s1, variant):
+    V = inputs.make_V(m, n, 1e8, 7)
+    Vd = V.cuda()
+    W1 = torch.empty(s1, n, dtype=torch.float64, device="cuda")
+    work = rq.alloc_workspace(m, n, s1, min(2 * n, s1))
+    rq.countsketch(Vd, s1, 42, W1, work, variant=variant)
+    W1o = orc.countsketch(V.numpy(), s1, 42)
+    scale = np.abs(W1o).max()
+    assert np.abs(host(W1) - W1o).max() <= 1e-13 * scale
+    if variant == 0:                      # sorted variant is bit-reproducible
+        W1b = torch.empty_like(W1)
+        rq.countsketch(Vd, s1, 42, W1b, work, variant=0)
+        assert torch.equal(W1, W1b)
+    # integer input: every partial sum exact => bit-exact whatever the order (K4)
+    Vi = inputs.make_integer_V(m, n, 3)
+    rq.countsketch(Vi.cuda(), s1, 42, W1, work, variant=variant)
+    assert np.array_equal(host(W1), orc.countsketch(Vi.numpy(), s1, 42))
+
+
+def test_countsketch_strided_and_row_offset(rq, orc):
+    m, n, s1 = 6000, 24, 300
+    big = inputs.make_integer_V(m, n + 6, 5).cuda()
+    V = big[:, :n]                        # ldv = n + 6
+    W1 = torch.empty(s1, n, dtype=torch.float64, device="cuda")
+    work = rq.alloc_workspace(m, n, s1, 2 * n)
+    for variant in (0, 1):
+        rq.countsketch(V, s1, 9, W1, work, variant=variant, row0=1000)
+        ref = orc.countsketch(host(V), s1, 9, row0=1000)
+        assert np.array_equal(host(W1), ref)
+
+
+@pytest.mark.parametrize("s1,n,s2", [(512, 16, 32), (8192, 64, 128), (9940, 70, 140), (300, 5, 7),
+                                     (4096, 256, 512)])
+def test_gauss_sketch_parity(rq, orc, s1, n, s2):
+    rng = np.random.default_rng(s1 + n)
+    W1 = rng.standard_normal((s1, n))
+    W = torch.empty(s2, n, dtype=torch.float64, device="cuda")
+    work = rq.alloc_workspace(s1, n, s1, s2)
+    rq.gauss_sketch(dev(W1), s2, 42, W, work)
+    Wo = orc.gauss_sketch(W1, s2, 42)
+    assert np.abs(host(W) - Wo).max() <= 1e-13 * np.abs(Wo).max()
+
+
+def test_dense_gauss_sketch_parity(rq, orc):
+    m, n, s = 5000, 20, 40
+    V = inputs.make_V(m, n, 1e3, 2)
+    W = torch.empty(s, n, dtype=torch.float64, device="cuda")
+    work = rq.alloc_workspace(m, n, 2 * n * n, 2 * n)
+    rq.dense_gauss_sketch(V.cuda(), s, 5, W, work)
+    Wo = orc.dense_gauss_sketch(V.numpy(), s, 5)
+    assert np.abs(host(W) - Wo).max() <= 1e-13 * np.abs(Wo).max()
+
+
+@pytest.mark.parametrize("s2,n", [(32, 16), (128, 64), (140, 70), (256, 128), (512, 256), (9, 9),
+                                  (64, 2), (300, 37)])
+def test_small_geqrf_parity(rq, orc, s2, n):
+    rng = np.random.default_rng(s2 * 1000 + n)
+    W = rng.standard_normal((s2, n)) * np.logspace(0, -10, n)
+    R0 = torch.full((n, n), np.nan, dtype=torch.float64, device="cuda")
+    info = rq.new_info()
+    rq.small_geqrf(dev(W), R0, info)
+    Ro, io = orc.hhqr_r(W)
+    R = host(R0)
+    assert int(info.item()) == 0 and io == 0
+    assert np.array_equal(np.tril(R, -1), np.zeros_like(R))
+    assert (np.diag(R) > 0).all()
+    assert np.linalg.norm(R - Ro) <= 1e-13 * np.linalg.norm(Ro)
+    # row-wise too: row j of R is determined to ~u relative to ||W[:, j:]|| scaling
+    assert np.all(np.linalg.norm(R - Ro, axis=1) <= 1e-12 * np.linalg.norm(Ro, axis=1) + 1e-300)
+
+
+def test_small_geqrf_flags_rank_deficiency(rq, orc):
+    W = np.zeros((20, 4)); W[:, 0] = 1; W[:, 2] = 2; W[3, 3] = 1
+    info = rq.new_info()
+    R0 = torch.empty(4, 4, dtype=torch.float64, device="cuda")
+    rq.small_geqrf(dev(W), R0, info)
+    _, io = orc.hhqr_r(W)
+    assert int(info.item()) == rq.INFO_SINGULAR + 2 == io - orc.ORC_SINGULAR + rq.INFO_SINGULAR
+
+
+SHAPES_TALL = [(20000, 16), (4099, 64), (10000, 70), (3000, 32), (2500, 128), (700, 256), (65, 8), (5, 2)]
+
+
+@pytest.mark.parametrize("m,n", SHAPES_TALL)
+@pytest.mark.parametrize("generic", [False, True])
+def test_trsm_gram_parity(rq, orc, m, n, generic):
+    rq.force_generic(generic)
+    try:
+        V = inputs.make_V(m, n, 1e3, 11) if m >= n else inputs.make_graded_V(m, n, 1, 11)
+        R0 = inputs.make_upper(n, 5)                      # well conditioned: X is unique to ~1e-13
+        Vd = V.cuda()
+        G = torch.empty(n, n, dtype=torch.float64, device="cuda")
+        V1 = torch.empty_like(Vd)
+        work = rq.alloc_workspace(m, n, max(n, 2), 2)
+        rq.trsm_gram(Vd, R0.cuda(), G, V1, work)
+        Xo = orc.trsm(V.numpy(), R0.numpy())
+        Go = orc.gram(Xo)
+        assert np.abs(host(V1) - Xo).max() <= 1e-12 * np.abs(Xo).max()
+        assert np.linalg.norm(host(G) - Go) <= 1e-13 * np.linalg.norm(Go)
+        assert torch.equal(G, G.T)
+        # R0 = NULL: plain Gram; V1 = NULL: nothing stored; integer input: exact
+        Vi = inputs.make_integer_V(m, n, 4)
+        rq.trsm_gram(Vi.cuda(), None, G, None, work)
+        assert np.array_equal(host(G), orc.gram(Vi.numpy()))
+        # in place (V1 == V)
+        Vc = Vd.clone()
+        rq.trsm_gram(Vc, R0.cuda(), G, Vc, work)
+        assert torch.equal(Vc, V1)
+    finally:
+        rq.force_generic(False)
+
+
+@pytest.mark.parametrize("m,n", SHAPES_TALL)
+@pytest.mark.parametrize("generic", [False, True])
+def test_apply_parity_and_bit_identical_recompute(rq, orc, m, n, generic):
+    rq.force_generic(generic)
+    try:
+        V = inputs.make_V(m, n, 1e3, 12) if m >= n else inputs.make_graded_V(m, n, 1, 12)
+        R0 = inputs.make_upper(n, 6); R1 = inputs.make_upper(n, 7)
+        Vd = V.cuda()
+        G = torch.empty(n, n, dtype=torch.float64, device="cuda")
+        V1 = torch.empty_like(Vd)
+        work = rq.alloc_workspace(m, n, max(n, 2), 2)
+        rq.trsm_gram(Vd, R0.cuda(), G, V1, work)
+        Qa = torch.empty_like(Vd); Qb = torch.empty_like(Vd)
+        rq.apply(V1, None, R1.cuda(), Qa, work)              # stored V1
+        rq.apply(Vd, R0.cuda(), R1.cuda(), Qb, work)         # V1 re-formed inside
+        assert torch.equal(Qa, Qb)                           # H1: same bits
+        Qo = orc.trsm(orc.trsm(V.numpy(), R0.numpy()), R1.numpy())
+        assert np.abs(host(Qa) - Qo).max() <= 1e-12 * np.abs(Qo).max()
+        Vc = V1.clone()
+        rq.apply(Vc, None, R1.cuda(), Vc, work)              # in place
+        assert torch.equal(Vc, Qa)
+    finally:
+        rq.force_generic(False)
+
+
+def test_trsm_rowwise_backward_error_with_graded_R(rq):
+    # eq. (42): each row solves x (R + dR) = v with |dR| <= c n u |R|.
+    # R0 = R factor of a column-graded matrix (12 decades), as randQR meets at kappa = 1e12.
+    m, n = 3000, 64
+    Rg = torch.linalg.qr(inputs.make_graded_V(500, n, 12, 8), mode="r").R
+    Rg = (Rg * torch.sign(torch.diagonal(Rg))[:, None]).contiguous()
+    X0 = inputs.make_graded_V(m, n, 0, 9)
+    R0 = Rg.cuda()
+    V = (X0 @ Rg).contiguous().cuda()
+    for generic in (False, True):
+        rq.force_generic(generic)
+        try:
+            G = torch.empty(n, n, dtype=torch.float64, device="cuda")
+            V1 = torch.empty_like(V)
+            work = rq.alloc_workspace(m, n, n, 2)
+            rq.trsm_gram(V, R0, G, V1, work)
+            resid = (V1 @ R0 - V).abs()
+            bound = 16 * n * 2.0 ** -53 * (V1.abs() @ R0.abs())
+            assert bool((resid <= bound + 1e-300).all())
+            assert float(torch.linalg.norm(G - V1.T @ V1) / torch.linalg.norm(G)) <= 1e-13
+        finally:
+            rq.force_generic(False)
+
+
+@pytest.mark.parametrize("n", [2, 16, 64, 70, 128, 256])
+def test_chol_parity_and_failure(rq, orc, n):
+    A = inputs.make_V(4 * n + 3, n, 30.0, n).numpy()
+    Gm = A.T @ A
+    R1 = torch.empty(n, n, dtype=torch.float64, device="cuda")
+    info = rq.new_info()
+    rq.chol(dev(Gm), R1, info)
+    Ro, io = orc.chol(Gm)
+    assert int(info.item()) == 0 and io == 0
+    R = host(R1)
+    assert np.array_equal(np.tril(R, -1), np.zeros_like(R)) and (np.diag(R) > 0).all()
+    assert np.linalg.norm(R - Ro) <= 1e-13 * np.linalg.norm(Ro)
+    rq.chol(dev(Gm), R1, info, shift=0.75)
+    Rs, _ = orc.chol(Gm, 0.75)
+    assert np.linalg.norm(host(R1) - Rs) <= 1e-13 * np.linalg.norm(Rs)
+    bad = Gm.copy(); j = n // 2; bad[j, j] = -1.0
+    rq.chol(dev(bad), R1, info)
+    _, io = orc.chol(bad)
+    assert int(info.item()) == rq.INFO_NOT_SPD + j + 1 == io - orc.ORC_NOT_SPD + rq.INFO_NOT_SPD
+    info.zero_()
+    nan = Gm.copy(); nan[0, 0] = np.nan
+    rq.chol(dev(nan), R1, info)
+    assert int(info.item()) == rq.INFO_NOT_SPD + 1
+
+
+@pytest.mark.parametrize("n", [2, 16, 70, 256])
+def test_triu_mul_parity(rq, orc, n):
+    R1 = inputs.make_upper(n, 1); R0 = inputs.make_upper(n, 2, 6)
+    R = torch.empty(n, n, dtype=torch.float64, device="cuda")
+    rq.triu_mul(R1.cuda(), R0.cuda(), R)
+    Ro = orc.triu_mul(R1.numpy(), R0.numpy())
+    assert np.abs(host(R) - Ro).max() <= 1e-15 * n * np.abs(Ro).max()
+    assert np.array_equal(np.tril(host(R), -1), np.zeros((n, n)))
