@@ -2,22 +2,29 @@
 //
 // Design: one persistent CTA per SM, 8 warps, NO block-level
 // synchronisation in the main loop.  Every warp is its own pipeline over 8-row blocks of V:
-//   * a private ring of STAGES shared-memory row-blocks (8 rows x LD doubles, LD = n8 + 4 so
-//     that all three fragment access patterns are bank-conflict free), filled by per-row
-//     cp.async.bulk (TMA bulk copy, SASS UBLKCP) completing on the warp's own mbarriers;
+//   * a private ring of STAGES "landing" row-blocks in shared memory (8 rows x (n8+8) doubles),
+//     filled by per-row cp.async.bulk (TMA bulk copy, SASS UBLKCP) completing on the warp's own
+//     mbarriers; read once (128-bit C-fragment pattern, conflict free at this row stride);
+//   * a private double-buffered 8 x n8 "xs" block with a 16-byte-unit XOR swizzle under which
+//     all three fragment patterns (C 128-bit, A 64-bit, Gram 64-bit) are bank-conflict free;
 //   * blocked forward substitution with 8x8 diagonal blocks (reading S7/H6):
 //       X_J = acc_J T_J,  acc_J' -= X_J R[J,J']  (J' > J),  T_J = inv(R[J,J]) by substitution,
-//     every product an mma.sync.m8n8k4.f64 (SASS DMMA); C->A fragment conversions go through
-//     the warp's own row-block in shared memory (in place);
+//     every product an mma.sync.m8n8k4.f64 (SASS DMMA); C->A fragment conversions go through xs;
+//   * software pipelining inside the warp: the 72 independent Gram DMMAs of row-block i are
+//     interleaved, 9 per substitution step, with the latency-bound chain of row-block i+1;
 //   * the Gram update G += X^T X on the upper block triangle, 36 (n = 64) 8x8 accumulators
 //     held in the warp's registers for the whole kernel; X^T as A and X as B are the SAME
 //     register (lane l holds X[l%4][l/4] of a 4-row slab).
 // The same trsm routine serves rqr_apply, so V1 re-formed there has the same bits (H1).
 #include "rqr_common.cuh"
 #include "rqr_tall.cuh"
+#include <type_traits>
 
-#define MMA_WARPS 8
-#define MMA_STAGES 4
+#define GRAM_WARPS 8      // A4: 240 registers/thread (36 Gram accumulators) => 8 warps per SM
+#define GRAM_STAGES 3
+#define APPLY_WARPS 12    // A6: ~100 registers/thread => 12 warps per SM hide the trsm chain latency
+#define APPLY_STAGES 2
+#define LDL_PAD 8         // landing rows: LD = n8 + 8  (conflict-free 128-bit C-fragment reads)
 
 // ------------------------------------------------------------------------------------------
 // PTX helpers
@@ -116,40 +123,116 @@ __device__ void build_tri_frags(const double* __restrict__ R, int n, double* __r
 }
 
 // ------------------------------------------------------------------------------------------
-// X = X R^-1 on one 8-row block held in shared memory (rb: 8 x LD doubles), in place, by the
-// calling warp.  Optionally stores X to global (gout = row 0 of the block, guarded).
+// xs: per-warp 8 x N8 block, 16-byte units XOR-swizzled by g(r) = 4 (r&1) + (r&2).
+// Element (r, c) lives at r*N8 + (((c>>1) ^ g(r)) << 1) + (c&1).
 // ------------------------------------------------------------------------------------------
-template <int NB, int LD>
-__device__ __forceinline__ void trsm_rowblock(double* __restrict__ rb, const double* __restrict__ Tf,
-                                              const double* __restrict__ nRf, double* __restrict__ gout,
-                                              int64_t ldq, int rows_valid, int n, int lane)
-{
-    const int r = lane >> 2, q = lane & 3;
-    double acc[NB][2];
+__device__ __forceinline__ int xs_swz(int r) { return ((r & 1) << 2) | (r & 2); }
+
+template <int N8>
+struct XsAddr {
+    int c_base;   // C fragment of block J:  c_base + ((8J) ^ c_x)      (double2)
+    int c_x;
+    int a_base;   // A fragment (J, h):      a_base + ((8J + 4h) ^ a_x)
+    int a_x;
+    int g_base[2];// Gram fragment (h, a):   g_base[h] + ((8a) ^ g_x[h])
+    int g_x[2];
+    __device__ __forceinline__ explicit XsAddr(int lane)
+    {
+        const int r = lane >> 2, q = lane & 3;
+        // C: (r, 8J + 2q): unit 4J + q ^ g(r)
+        c_base = r * N8; c_x = ((q ^ xs_swz(r)) << 1);
+        // A: (r, 8J + 4h + q): unit (4J + 2h + (q>>1)) ^ g(r), word q&1
+        a_base = r * N8 + (q & 1); a_x = (((q >> 1) ^ xs_swz(r)) << 1);
 #pragma unroll
-    for (int J = 0; J < NB; ++J) {
-        double2 v = *reinterpret_cast<const double2*>(rb + r * LD + 8 * J + 2 * q);
-        acc[J][0] = v.x; acc[J][1] = v.y;
+        for (int h = 0; h < 2; ++h) {
+            // Gram: (row 4h + q, col 8a + r): unit (4a + (r>>1)) ^ g(row), word r&1
+            const int row = 4 * h + q;
+            g_base[h] = row * N8 + (r & 1); g_x[h] = (((r >> 1) ^ xs_swz(row)) << 1);
+        }
     }
+    __device__ __forceinline__ int c(int J) const { return c_base + ((8 * J) ^ c_x); }
+    __device__ __forceinline__ int a(int J, int h) const { return a_base + ((8 * J + 4 * h) ^ a_x); }
+    __device__ __forceinline__ int g(int h, int a_) const { return g_base[h] + ((8 * a_) ^ g_x[h]); }
+};
+
+// t-th Gram DMMA of a row-block, t in [0, 2*NBLK): slab h = t / NBLK, then (a, b), a <= b, row-major
+template <int NB>
+__device__ __forceinline__ constexpr int gram_a(int t)
+{
+    int rem = t % (NB * (NB + 1) / 2), a = 0;
+    while (rem >= NB - a) { rem -= NB - a; ++a; }
+    return a;
+}
+template <int NB>
+__device__ __forceinline__ constexpr int gram_b(int t)
+{
+    int rem = t % (NB * (NB + 1) / 2), a = 0;
+    while (rem >= NB - a) { rem -= NB - a; ++a; }
+    return a + rem;
+}
+
+template <int I, int N, class F>
+__device__ __forceinline__ void static_for(F&& f)
+{
+    if constexpr (I < N) {
+        f(std::integral_constant<int, I>{});
+        static_for<I + 1, N>(f);
+    }
+}
+
+// Gram DMMAs [T0, T1) of the row-block held in xsp; g = fragment registers carried across calls.
+template <int NB, int N8, int T0, int T1>
+__device__ __forceinline__ void gram_chunk(const double* __restrict__ xsp, const XsAddr<N8>& ad,
+                                           double (&g)[NB], double (&G)[NB * (NB + 1) / 2][2])
+{
+    constexpr int NBLK = NB * (NB + 1) / 2;
+    static_for<T0, T1>([&](auto tc) {
+        constexpr int t = decltype(tc)::value;
+        if constexpr (t % NBLK == 0) {
+            constexpr int h = t / NBLK;
 #pragma unroll
-    for (int J = 0; J < NB; ++J) {
-        // C -> A fragments of acc_J through the row-block (in place)
-        *reinterpret_cast<double2*>(rb + r * LD + 8 * J + 2 * q) = make_double2(acc[J][0], acc[J][1]);
+            for (int a_ = 0; a_ < NB; ++a_) g[a_] = xsp[ad.g(h, a_)];
+        }
+        constexpr int idx = t % NBLK;
+        dmma(G[idx][0], G[idx][1], g[gram_a<NB>(t)], g[gram_b<NB>(t)]);
+    });
+}
+
+// ------------------------------------------------------------------------------------------
+// One 8-row block:  X = A R^-1 by blocked substitution (DMMA), A given as C fragments in acc.
+// X ends up (swizzled) in xsc and, if gout != nullptr, in global memory.  When GRAM is set the
+// Gram DMMAs of the PREVIOUS row-block (held in xsp) are interleaved, NB+1 per step.
+// The arithmetic on (acc, Tf, nRf) is the same instruction sequence for every caller (H1).
+// ------------------------------------------------------------------------------------------
+template <int NB, bool GRAM>
+__device__ __forceinline__ void trsm_rowblock(double (&acc)[NB][2], double* __restrict__ xsc,
+                                              const double* __restrict__ xsp,
+                                              const XsAddr<8 * NB>& ad, const double* __restrict__ Tf,
+                                              const double* __restrict__ nRf, double* __restrict__ gout,
+                                              int64_t ldq, int rows_valid, int n, int lane,
+                                              double (&g)[NB], double (&G)[NB * (NB + 1) / 2][2])
+{
+    constexpr int N8 = 8 * NB;
+    const int r = lane >> 2, q = lane & 3;
+    static_for<0, NB>([&](auto Jc) {
+        constexpr int J = decltype(Jc)::value;
+        // C -> A fragments of acc_J through xs
+        *reinterpret_cast<double2*>(xsc + ad.c(J)) = make_double2(acc[J][0], acc[J][1]);
         __syncwarp();
-        double a0 = rb[r * LD + 8 * J + q], a1 = rb[r * LD + 8 * J + 4 + q];
-        __syncwarp();
+        double a0 = xsc[ad.a(J, 0)], a1 = xsc[ad.a(J, 1)];
         double x0 = 0.0, x1 = 0.0;
         dmma(x0, x1, a0, Tf[J * 64 + lane]);
         dmma(x0, x1, a1, Tf[J * 64 + 32 + lane]);
-        *reinterpret_cast<double2*>(rb + r * LD + 8 * J + 2 * q) = make_double2(x0, x1);
+        __syncwarp();
+        *reinterpret_cast<double2*>(xsc + ad.c(J)) = make_double2(x0, x1);
         if (gout != nullptr && r < rows_valid) {
             const int c = 8 * J + 2 * q;
             if (c + 1 < n) *reinterpret_cast<double2*>(gout + (int64_t)r * ldq + c) = make_double2(x0, x1);
             else if (c < n) gout[(int64_t)r * ldq + c] = x0;
         }
-        if (J + 1 < NB) {
+        if constexpr (J + 1 < NB) {
             __syncwarp();
-            a0 = rb[r * LD + 8 * J + q]; a1 = rb[r * LD + 8 * J + 4 + q];
+            a0 = xsc[ad.a(J, 0)]; a1 = xsc[ad.a(J, 1)];
 #pragma unroll
             for (int Jp = J + 1; Jp < NB; ++Jp) {
                 const int p = TriFrags<NB>::pair(J, Jp);
@@ -157,15 +240,16 @@ __device__ __forceinline__ void trsm_rowblock(double* __restrict__ rb, const dou
                 dmma(acc[Jp][0], acc[Jp][1], a1, nRf[p * 64 + 32 + lane]);
             }
         }
-    }
+        if constexpr (GRAM) gram_chunk<NB, N8, J * (NB + 1), (J + 1) * (NB + 1)>(xsp, ad, g, G);
+    });
     __syncwarp();
 }
 
-// Per-warp ring of row-blocks fed by bulk async copies.
+// Per-warp ring of landing row-blocks fed by bulk async copies.
 template <int LD>
 struct WarpRing {
-    double* buf;          // MMA_STAGES x 8 x LD doubles (this warp's)
-    uint64_t* bar;        // MMA_STAGES mbarriers (this warp's)
+    double* buf;          // STAGES x 8 x LD doubles (this warp's)
+    uint64_t* bar;        // STAGES mbarriers (this warp's)
     const double* V;
     int64_t ldv, m;
     int n;
@@ -182,37 +266,51 @@ struct WarpRing {
 };
 
 template <int NB> struct TallCfg {
-    static constexpr int LD = 8 * NB + 4;
+    static constexpr int N8 = 8 * NB;
+    static constexpr int LDL = 8 * NB + LDL_PAD;
     static constexpr int NBLK = NB * (NB + 1) / 2;
     static constexpr int FRAG_DOUBLES = TriFrags<NB>::DOUBLES;         // Tf + nRf
 };
 
-// shared-memory carve-up (doubles): [frag sets][scratch NB*64][bars as u64][ring]
-template <int NB, int WARPS, int STAGES, int NSETS>
+// shared-memory carve-up (doubles): [frag sets][scratch NB*64][bars][xs: WARPS x 2 x 8 x N8][ring]
+template <int NB, int WARPS, int STAGES, int NSETS, int XSBUF>
 struct SmemPlan {
-    static constexpr int LD = TallCfg<NB>::LD;
-    static constexpr size_t frag = (size_t)NSETS * TallCfg<NB>::FRAG_DOUBLES;
-    static constexpr size_t scratch = frag;
+    static constexpr int LDL = TallCfg<NB>::LDL;
+    static constexpr int N8 = TallCfg<NB>::N8;
+    static constexpr size_t scratch = (size_t)NSETS * TallCfg<NB>::FRAG_DOUBLES;
     static constexpr size_t bars = scratch + NB * 64;
-    static constexpr size_t ring = bars + WARPS * STAGES;
-    static constexpr size_t ring_doubles = (size_t)WARPS * STAGES * 8 * LD;
+    static constexpr size_t xs = bars + ((WARPS * STAGES + 1) & ~1);
+    static constexpr size_t ring = xs + (size_t)WARPS * XSBUF * 8 * N8;
+    static constexpr size_t ring_doubles = (size_t)WARPS * STAGES * 8 * LDL;
     static constexpr size_t red_doubles = (size_t)WARPS * TallCfg<NB>::NBLK * 64;
     static constexpr size_t total_doubles =
         (ring + ring_doubles) > red_doubles ? (ring + ring_doubles) : red_doubles;
     static constexpr size_t bytes = total_doubles * sizeof(double);
 };
 
+// load the C fragments of a landing row-block (row stride LDL)
+template <int NB, int LDL>
+__device__ __forceinline__ void load_acc(double (&acc)[NB][2], const double* __restrict__ rb, int lane)
+{
+    const int r = lane >> 2, q = lane & 3;
+#pragma unroll
+    for (int J = 0; J < NB; ++J) {
+        double2 v = *reinterpret_cast<const double2*>(rb + r * LDL + 8 * J + 2 * q);
+        acc[J][0] = v.x; acc[J][1] = v.y;
+    }
+}
+
 // ------------------------------------------------------------------------------------------
 // A4: V1 = V R0^-1 (optional), store V1 (optional), partial Gram per CTA.
 // ------------------------------------------------------------------------------------------
 template <int NB, bool HAS_R>
-__global__ void __launch_bounds__(MMA_WARPS * 32, 1)
+__global__ void __launch_bounds__(GRAM_WARPS * 32, 1)
 k_trsm_gram_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
                 const double* __restrict__ R0, double* __restrict__ V1, int64_t ldq,
                 double* __restrict__ part)
 {
-    using Plan = SmemPlan<NB, MMA_WARPS, MMA_STAGES, 1>;
-    constexpr int LD = Plan::LD;
+    using Plan = SmemPlan<NB, GRAM_WARPS, GRAM_STAGES, 1, 2>;
+    constexpr int LDL = Plan::LDL, N8 = Plan::N8;
     constexpr int NBLK = TallCfg<NB>::NBLK;
     extern __shared__ __align__(16) double smem[];
     double* Tf = smem;
@@ -221,60 +319,68 @@ k_trsm_gram_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + Plan::bars);
     double* ring = smem + Plan::ring;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int r = lane >> 2, q = lane & 3;
+    double* xs = smem + Plan::xs + (size_t)warp * 2 * 8 * N8;
 
     for (int i = threadIdx.x; i < (int)Plan::ring_doubles; i += blockDim.x) ring[i] = 0.0;
-    if (threadIdx.x < MMA_WARPS * MMA_STAGES) mbar_init(bars + threadIdx.x, 1);
+    if (threadIdx.x < GRAM_WARPS * GRAM_STAGES) mbar_init(bars + threadIdx.x, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     fence_proxy_async();
     __syncthreads();
     if (HAS_R) build_tri_frags<NB>(R0, n, Tf, nRf, scratch);
 
-    WarpRing<LD> wr{ring + (size_t)warp * MMA_STAGES * 8 * LD, bars + warp * MMA_STAGES, V, ldv, m, n};
+    WarpRing<LDL> wr{ring + (size_t)warp * GRAM_STAGES * 8 * LDL, bars + warp * GRAM_STAGES, V, ldv, m, n};
+    const XsAddr<N8> ad(lane);
     const int64_t nrb = (m + 7) / 8;
-    const int64_t gw = (int64_t)blockIdx.x * MMA_WARPS + warp;
-    const int64_t stride = (int64_t)gridDim.x * MMA_WARPS;
+    const int64_t gw = (int64_t)blockIdx.x * GRAM_WARPS + warp;
+    const int64_t stride = (int64_t)gridDim.x * GRAM_WARPS;
 #pragma unroll
-    for (int s = 0; s < MMA_STAGES; ++s)
+    for (int s = 0; s < GRAM_STAGES; ++s)
         if (gw + s * stride < nrb) wr.issue(s, gw + s * stride, lane);
 
     double G[NBLK][2];
 #pragma unroll
     for (int b = 0; b < NBLK; ++b) { G[b][0] = 0.0; G[b][1] = 0.0; }
+    double g[NB];
+    double acc[NB][2];
 
     int it = 0;
     for (int64_t rblk = gw; rblk < nrb; rblk += stride, ++it) {
-        const int stage = it % MMA_STAGES;
-        mbar_wait(wr.bar + stage, (uint32_t)((it / MMA_STAGES) & 1));
-        double* rb = wr.buf + stage * 8 * LD;
+        const int stage = it % GRAM_STAGES;
+        mbar_wait(wr.bar + stage, (uint32_t)((it / GRAM_STAGES) & 1));
+        double* rb = wr.buf + stage * 8 * LDL;
         const int valid = (int)((m - rblk * 8) < 8 ? (m - rblk * 8) : 8);
         if (valid < 8) {
-            for (int e = lane; e < (8 - valid) * LD; e += 32) rb[valid * LD + e] = 0.0;
+            for (int e = lane; e < (8 - valid) * LDL; e += 32) rb[valid * LDL + e] = 0.0;
             __syncwarp();
         }
-        if (HAS_R)
-            trsm_rowblock<NB, LD>(rb, Tf, nRf, V1 ? V1 + rblk * 8 * ldq : nullptr, ldq, valid, n, lane);
-        // Gram: two 4-row slabs; lane holds X[4h + q][8a + r] = A fragment of X^T = B fragment of X
+        load_acc<NB, LDL>(acc, rb, lane);
+        double* xsc = xs + (it & 1) * 8 * N8;
+        const double* xsp = xs + ((it & 1) ^ 1) * 8 * N8;
+        if (HAS_R) {
+            double* gout = V1 ? V1 + rblk * 8 * ldq : nullptr;
+            if (it > 0) trsm_rowblock<NB, true>(acc, xsc, xsp, ad, Tf, nRf, gout, ldq, valid, n, lane, g, G);
+            else        trsm_rowblock<NB, false>(acc, xsc, xsp, ad, Tf, nRf, gout, ldq, valid, n, lane, g, G);
+        } else {
+            // plain Gram of V: move the row-block into xs, Gram of the previous one meanwhile
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            double g[NB];
-#pragma unroll
-            for (int a = 0; a < NB; ++a) g[a] = rb[(4 * h + q) * LD + 8 * a + r];
-            int idx = 0;
-#pragma unroll
-            for (int a = 0; a < NB; ++a)
-#pragma unroll
-                for (int b = a; b < NB; ++b) { dmma(G[idx][0], G[idx][1], g[a], g[b]); ++idx; }
+            for (int J = 0; J < NB; ++J)
+                *reinterpret_cast<double2*>(xsc + ad.c(J)) = make_double2(acc[J][0], acc[J][1]);
+            if (it > 0) gram_chunk<NB, N8, 0, 2 * NBLK>(xsp, ad, g, G);
+            __syncwarp();
         }
-        __syncwarp();
-        const int64_t next = rblk + (int64_t)MMA_STAGES * stride;
+        // the landing block was consumed by load_acc: refill it
+        const int64_t next = rblk + (int64_t)GRAM_STAGES * stride;
         if (next < nrb) {
             fence_proxy_async();
             __syncwarp();
             wr.issue(stage, next, lane);
         }
     }
-    // fixed-order reduction of the 8 warps' accumulators, then this CTA's partial (upper blocks)
+    if (it > 0) {
+        __syncwarp();
+        gram_chunk<NB, N8, 0, 2 * NBLK>(xs + ((it - 1) & 1) * 8 * N8, ad, g, G);
+    }
+    // fixed-order reduction of the warps' accumulators, then this CTA's partial (upper blocks)
     __syncthreads();
     double* red = smem;
 #pragma unroll
@@ -288,8 +394,7 @@ k_trsm_gram_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
         const int b = e >> 6, l = (e >> 1) & 31, k = e & 1;
         double s = red[(size_t)b * 64 + 2 * l + k];
 #pragma unroll
-        for (int w = 1; w < MMA_WARPS; ++w) s += red[((size_t)w * NBLK + b) * 64 + 2 * l + k];
-        // block b -> (a, bb)
+        for (int w = 1; w < GRAM_WARPS; ++w) s += red[((size_t)w * NBLK + b) * 64 + 2 * l + k];
         int a = 0, rem = b;
         while (rem >= NB - a) { rem -= NB - a; ++a; }
         const int bb = a + rem;
@@ -302,14 +407,15 @@ k_trsm_gram_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
 // A6: Q = (V R0^-1) R1^-1  (TWO) or Q = V R1^-1.
 // ------------------------------------------------------------------------------------------
 template <int NB, bool TWO>
-__global__ void __launch_bounds__(MMA_WARPS * 32, 1)
+__global__ void __launch_bounds__(APPLY_WARPS * 32, 1)
 k_apply_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
             const double* __restrict__ R0, const double* __restrict__ R1,
             double* __restrict__ Q, int64_t ldq)
 {
-    using Plan = SmemPlan<NB, MMA_WARPS, MMA_STAGES, 2>;
-    constexpr int LD = Plan::LD;
+    using Plan = SmemPlan<NB, APPLY_WARPS, APPLY_STAGES, 2, 1>;
+    constexpr int LDL = Plan::LDL, N8 = Plan::N8;
     constexpr int FD = TallCfg<NB>::FRAG_DOUBLES;
+    constexpr int NBLK = TallCfg<NB>::NBLK;
     extern __shared__ __align__(16) double smem[];
     double* Tf1 = smem;
     double* nRf1 = smem + NB * 64;
@@ -319,35 +425,49 @@ k_apply_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + Plan::bars);
     double* ring = smem + Plan::ring;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double* xs = smem + Plan::xs + (size_t)warp * 8 * N8;
 
     for (int i = threadIdx.x; i < (int)Plan::ring_doubles; i += blockDim.x) ring[i] = 0.0;
-    if (threadIdx.x < MMA_WARPS * MMA_STAGES) mbar_init(bars + threadIdx.x, 1);
+    if (threadIdx.x < APPLY_WARPS * APPLY_STAGES) mbar_init(bars + threadIdx.x, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     fence_proxy_async();
     __syncthreads();
     build_tri_frags<NB>(R1, n, Tf1, nRf1, scratch);
     if (TWO) build_tri_frags<NB>(R0, n, Tf0, nRf0, scratch);
 
-    WarpRing<LD> wr{ring + (size_t)warp * MMA_STAGES * 8 * LD, bars + warp * MMA_STAGES, V, ldv, m, n};
+    WarpRing<LDL> wr{ring + (size_t)warp * APPLY_STAGES * 8 * LDL, bars + warp * APPLY_STAGES, V, ldv, m, n};
+    const XsAddr<N8> ad(lane);
     const int64_t nrb = (m + 7) / 8;
-    const int64_t gw = (int64_t)blockIdx.x * MMA_WARPS + warp;
-    const int64_t stride = (int64_t)gridDim.x * MMA_WARPS;
+    const int64_t gw = (int64_t)blockIdx.x * APPLY_WARPS + warp;
+    const int64_t stride = (int64_t)gridDim.x * APPLY_WARPS;
 #pragma unroll
-    for (int s = 0; s < MMA_STAGES; ++s)
+    for (int s = 0; s < APPLY_STAGES; ++s)
         if (gw + s * stride < nrb) wr.issue(s, gw + s * stride, lane);
+    double acc[NB][2];
+    double g[NB];
+    double G[NBLK][2];      // unused (GRAM = false): optimised away
     int it = 0;
     for (int64_t rblk = gw; rblk < nrb; rblk += stride, ++it) {
-        const int stage = it % MMA_STAGES;
-        mbar_wait(wr.bar + stage, (uint32_t)((it / MMA_STAGES) & 1));
-        double* rb = wr.buf + stage * 8 * LD;
+        const int stage = it % APPLY_STAGES;
+        mbar_wait(wr.bar + stage, (uint32_t)((it / APPLY_STAGES) & 1));
+        double* rb = wr.buf + stage * 8 * LDL;
         const int valid = (int)((m - rblk * 8) < 8 ? (m - rblk * 8) : 8);
         if (valid < 8) {
-            for (int e = lane; e < (8 - valid) * LD; e += 32) rb[valid * LD + e] = 0.0;
+            for (int e = lane; e < (8 - valid) * LDL; e += 32) rb[valid * LDL + e] = 0.0;
             __syncwarp();
         }
-        if (TWO) trsm_rowblock<NB, LD>(rb, Tf0, nRf0, nullptr, ldq, valid, n, lane);
-        trsm_rowblock<NB, LD>(rb, Tf1, nRf1, Q + rblk * 8 * ldq, ldq, valid, n, lane);
-        const int64_t next = rblk + (int64_t)MMA_STAGES * stride;
+        load_acc<NB, LDL>(acc, rb, lane);
+        if (TWO) {
+            trsm_rowblock<NB, false>(acc, xs, xs, ad, Tf0, nRf0, nullptr, ldq, valid, n, lane, g, G);
+#pragma unroll
+            for (int J = 0; J < NB; ++J) {
+                double2 v = *reinterpret_cast<const double2*>(xs + ad.c(J));
+                acc[J][0] = v.x; acc[J][1] = v.y;
+            }
+            __syncwarp();
+        }
+        trsm_rowblock<NB, false>(acc, xs, xs, ad, Tf1, nRf1, Q + rblk * 8 * ldq, ldq, valid, n, lane, g, G);
+        const int64_t next = rblk + (int64_t)APPLY_STAGES * stride;
         if (next < nrb) {
             fence_proxy_async();
             __syncwarp();
@@ -367,10 +487,10 @@ static bool fast_ok(const void* V, int n, int64_t ldv, const void* Q, int64_t ld
     return true;
 }
 
-static int grid_for(int64_t m)
+static int grid_for(int64_t m, int warps)
 {
     int64_t nrb = (m + 7) / 8;
-    int64_t g = (nrb + MMA_WARPS - 1) / MMA_WARPS;
+    int64_t g = (nrb + warps - 1) / warps;
     return (int)(g < 148 ? (g < 1 ? 1 : g) : 148);
 }
 
@@ -378,17 +498,18 @@ template <int NB>
 static int launch_trsm_gram(const double* V, int64_t m, int n, int64_t ldv, const double* R0, double* V1,
                             int64_t ldq, double* part, int* nparts, cudaStream_t st)
 {
-    using Plan = SmemPlan<NB, MMA_WARPS, MMA_STAGES, 1>;
+    using Plan = SmemPlan<NB, GRAM_WARPS, GRAM_STAGES, 1, 2>;
+    static_assert(Plan::bytes <= 227 * 1024, "A4 shared memory plan too large");
     static bool attr = false;
     if (!attr) {
         cudaFuncSetAttribute(k_trsm_gram_mma<NB, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
         cudaFuncSetAttribute(k_trsm_gram_mma<NB, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
         attr = true;
     }
-    const int grid = grid_for(m);
+    const int grid = grid_for(m, GRAM_WARPS);
     *nparts = grid;
-    if (R0) k_trsm_gram_mma<NB, true><<<grid, MMA_WARPS * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, V1, ldq, part);
-    else    k_trsm_gram_mma<NB, false><<<grid, MMA_WARPS * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, nullptr, ldq, part);
+    if (R0) k_trsm_gram_mma<NB, true><<<grid, GRAM_WARPS * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, V1, ldq, part);
+    else    k_trsm_gram_mma<NB, false><<<grid, GRAM_WARPS * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, nullptr, ldq, part);
     RQR_LAUNCH_CHECK();
     return RQR_OK;
 }
@@ -407,16 +528,17 @@ template <int NB>
 static int launch_apply(const double* V, int64_t m, int n, int64_t ldv, const double* R0, const double* R1,
                         double* Q, int64_t ldq, cudaStream_t st)
 {
-    using Plan = SmemPlan<NB, MMA_WARPS, MMA_STAGES, 2>;
+    using Plan = SmemPlan<NB, APPLY_WARPS, APPLY_STAGES, 2, 1>;
+    static_assert(Plan::bytes <= 227 * 1024, "A6 shared memory plan too large");
     static bool attr = false;
     if (!attr) {
         cudaFuncSetAttribute(k_apply_mma<NB, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
         cudaFuncSetAttribute(k_apply_mma<NB, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
         attr = true;
     }
-    const int grid = grid_for(m);
-    if (R0) k_apply_mma<NB, true><<<grid, MMA_WARPS * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, R1, Q, ldq);
-    else    k_apply_mma<NB, false><<<grid, MMA_WARPS * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, R1, Q, ldq);
+    const int grid = grid_for(m, APPLY_WARPS);
+    if (R0) k_apply_mma<NB, true><<<grid, APPLY_WARPS * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, R1, Q, ldq);
+    else    k_apply_mma<NB, false><<<grid, APPLY_WARPS * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, R1, Q, ldq);
     RQR_LAUNCH_CHECK();
     return RQR_OK;
 }
