@@ -5,13 +5,18 @@
 //   * a private ring of STAGES "landing" row-blocks in shared memory (8 rows x (n8+8) doubles),
 //     filled by per-row cp.async.bulk (TMA bulk copy, SASS UBLKCP) completing on the warp's own
 //     mbarriers; read once (128-bit C-fragment pattern, conflict free at this row stride);
-//   * a private double-buffered 8 x n8 "xs" block with a 16-byte-unit XOR swizzle under which
-//     all three fragment patterns (C 128-bit, A 64-bit, Gram 64-bit) are bank-conflict free;
 //   * blocked forward substitution with 8x8 diagonal blocks (reading S7/H6):
 //       X_J = acc_J T_J,  acc_J' -= X_J R[J,J']  (J' > J),  T_J = inv(R[J,J]) by substitution,
-//     every product an mma.sync.m8n8k4.f64 (SASS DMMA); C->A fragment conversions go through xs;
+//     every product an mma.sync.m8n8k4.f64 (SASS DMMA).  The chain never leaves the register
+//     file: an 8x8 product is two k=4 DMMAs, and the contraction index is PERMUTED so that
+//     piece s in {0,1} contracts over columns {2k+s}: lane (r,k) of the A operand then needs
+//     X[r][2k+s], which is exactly element s of the C fragment the same lane already holds.  The
+//     B fragments (T_J, -R[J,J']) are built once per CTA with the matching row permutation;
+//   * a private double-buffered 8 x n8 "xs" block (A4 only) through which X reaches the Gram
+//     fragment layout (a transpose across lanes), 16-byte-unit XOR swizzle, conflict free;
 //   * software pipelining inside the warp: the 72 independent Gram DMMAs of row-block i are
-//     interleaved, 9 per substitution step, with the latency-bound chain of row-block i+1;
+//     interleaved, 9 per substitution step, into the dependent-issue gaps of the chain of
+//     row-block i+1;
 //   * the Gram update G += X^T X on the upper block triangle, 36 (n = 64) 8x8 accumulators
 //     held in the warp's registers for the whole kernel; X^T as A and X as B are the SAME
 //     register (lane l holds X[l%4][l/4] of a 4-row slab).
@@ -20,10 +25,18 @@
 #include "rqr_tall.cuh"
 #include <type_traits>
 
-#define GRAM_WARPS 8      // A4: 240 registers/thread (36 Gram accumulators) => 8 warps per SM
+#ifndef GRAM_WARPS
+#define GRAM_WARPS 8      // A4: 248 registers/thread (36 Gram accumulators) => 8 warps per SM
+#endif
+#ifndef GRAM_STAGES
 #define GRAM_STAGES 3
-#define APPLY_WARPS 12    // A6: ~100 registers/thread => 12 warps per SM hide the trsm chain latency
+#endif
+#ifndef APPLY_WARPS
+#define APPLY_WARPS 12    // A6: ~90 registers/thread
+#endif
+#ifndef APPLY_STAGES
 #define APPLY_STAGES 2
+#endif
 #define LDL_PAD 8         // landing rows: LD = n8 + 8  (conflict-free 128-bit C-fragment reads)
 
 // ------------------------------------------------------------------------------------------
@@ -71,8 +84,8 @@ __device__ __forceinline__ void fence_proxy_async()
 
 // ------------------------------------------------------------------------------------------
 // Triangular-factor fragments in shared memory, built by every CTA in its prologue:
-//   Tf [J][h][lane]      = T_J[4h + lane%4][lane/4],     T_J = inv(R[J,J])   (B fragments)
-//   nRf[p(J,J')][h][lane] = -R[8J + 4h + lane%4][8J' + lane/4],  J < J'
+//   Tf [J][s][lane]      = T_J[2(lane%4) + s][lane/4],     T_J = inv(R[J,J])   (B fragments)
+//   nRf[p(J,J')][s][lane] = -R[8J + 2(lane%4) + s][8J' + lane/4],  J < J'
 // R is n x n; columns/rows >= n are padded with the identity.
 // ------------------------------------------------------------------------------------------
 template <int NB>
@@ -109,7 +122,7 @@ __device__ void build_tri_frags(const double* __restrict__ R, int n, double* __r
     __syncthreads();
     for (int t = tid; t < NB * 64; t += blockDim.x) {
         const int J = t >> 6, h = (t >> 5) & 1, lane = t & 31;
-        Tf[t] = scratch[J * 64 + (4 * h + (lane & 3)) * 8 + (lane >> 2)];
+        Tf[t] = scratch[J * 64 + (2 * (lane & 3) + h) * 8 + (lane >> 2)];
     }
     for (int t = tid; t < TriFrags<NB>::NPAIR * 64; t += blockDim.x) {
         const int p = t >> 6, h = (t >> 5) & 1, lane = t & 31;
@@ -117,7 +130,7 @@ __device__ void build_tri_frags(const double* __restrict__ R, int n, double* __r
         int J = 0, rem = p;
         while (rem >= NB - 1 - J) { rem -= NB - 1 - J; ++J; }
         const int Jp = J + 1 + rem;
-        nRf[t] = -r_padded(R, n, 8 * J + 4 * h + (lane & 3), 8 * Jp + (lane >> 2));
+        nRf[t] = -r_padded(R, n, 8 * J + 2 * (lane & 3) + h, 8 * Jp + (lane >> 2));
     }
     __syncthreads();
 }
@@ -199,12 +212,14 @@ __device__ __forceinline__ void gram_chunk(const double* __restrict__ xsp, const
 }
 
 // ------------------------------------------------------------------------------------------
-// One 8-row block:  X = A R^-1 by blocked substitution (DMMA), A given as C fragments in acc.
-// X ends up (swizzled) in xsc and, if gout != nullptr, in global memory.  When GRAM is set the
-// Gram DMMAs of the PREVIOUS row-block (held in xsp) are interleaved, NB+1 per step.
+// One 8-row block:  X = A R^-1 by blocked substitution (DMMA), A given as C fragments in acc; on
+// return acc holds X (C fragments).  X is also written (swizzled) to xsc if XS, and to global
+// memory if gout != nullptr.  When GRAM is set the NB+1 Gram DMMAs per step of the PREVIOUS
+// row-block (held in xsp) are issued in four groups placed in the dependent-issue gaps of the
+// chain  T(s=0) -> T(s=1) -> U(J+1, s=0) -> U(J+1, s=1) -> next step.
 // The arithmetic on (acc, Tf, nRf) is the same instruction sequence for every caller (H1).
 // ------------------------------------------------------------------------------------------
-template <int NB, bool GRAM>
+template <int NB, bool GRAM, bool XS>
 __device__ __forceinline__ void trsm_rowblock(double (&acc)[NB][2], double* __restrict__ xsc,
                                               const double* __restrict__ xsp,
                                               const XsAddr<8 * NB>& ad, const double* __restrict__ Tf,
@@ -213,36 +228,33 @@ __device__ __forceinline__ void trsm_rowblock(double (&acc)[NB][2], double* __re
                                               double (&g)[NB], double (&G)[NB * (NB + 1) / 2][2])
 {
     constexpr int N8 = 8 * NB;
+    constexpr int GP = NB + 1;                       // Gram DMMAs per step
+    constexpr int E1 = GP / 4, E2 = GP / 2, E3 = (3 * GP) / 4;
     const int r = lane >> 2, q = lane & 3;
     static_for<0, NB>([&](auto Jc) {
         constexpr int J = decltype(Jc)::value;
-        // C -> A fragments of acc_J through xs
-        *reinterpret_cast<double2*>(xsc + ad.c(J)) = make_double2(acc[J][0], acc[J][1]);
-        __syncwarp();
-        double a0 = xsc[ad.a(J, 0)], a1 = xsc[ad.a(J, 1)];
         double x0 = 0.0, x1 = 0.0;
-        dmma(x0, x1, a0, Tf[J * 64 + lane]);
-        dmma(x0, x1, a1, Tf[J * 64 + 32 + lane]);
-        __syncwarp();
-        *reinterpret_cast<double2*>(xsc + ad.c(J)) = make_double2(x0, x1);
+        dmma(x0, x1, acc[J][0], Tf[J * 64 + lane]);
+        if constexpr (GRAM) gram_chunk<NB, N8, J * GP, J * GP + E1>(xsp, ad, g, G);
+        dmma(x0, x1, acc[J][1], Tf[J * 64 + 32 + lane]);
+        if constexpr (GRAM) gram_chunk<NB, N8, J * GP + E1, J * GP + E2>(xsp, ad, g, G);
+#pragma unroll
+        for (int Jp = J + 1; Jp < NB; ++Jp)
+            dmma(acc[Jp][0], acc[Jp][1], x0, nRf[TriFrags<NB>::pair(J, Jp) * 64 + lane]);
+        if constexpr (GRAM) gram_chunk<NB, N8, J * GP + E2, J * GP + E3>(xsp, ad, g, G);
+#pragma unroll
+        for (int Jp = J + 1; Jp < NB; ++Jp)
+            dmma(acc[Jp][0], acc[Jp][1], x1, nRf[TriFrags<NB>::pair(J, Jp) * 64 + 32 + lane]);
+        acc[J][0] = x0; acc[J][1] = x1;
+        if constexpr (XS) *reinterpret_cast<double2*>(xsc + ad.c(J)) = make_double2(x0, x1);
         if (gout != nullptr && r < rows_valid) {
             const int c = 8 * J + 2 * q;
             if (c + 1 < n) *reinterpret_cast<double2*>(gout + (int64_t)r * ldq + c) = make_double2(x0, x1);
             else if (c < n) gout[(int64_t)r * ldq + c] = x0;
         }
-        if constexpr (J + 1 < NB) {
-            __syncwarp();
-            a0 = xsc[ad.a(J, 0)]; a1 = xsc[ad.a(J, 1)];
-#pragma unroll
-            for (int Jp = J + 1; Jp < NB; ++Jp) {
-                const int p = TriFrags<NB>::pair(J, Jp);
-                dmma(acc[Jp][0], acc[Jp][1], a0, nRf[p * 64 + lane]);
-                dmma(acc[Jp][0], acc[Jp][1], a1, nRf[p * 64 + 32 + lane]);
-            }
-        }
-        if constexpr (GRAM) gram_chunk<NB, N8, J * (NB + 1), (J + 1) * (NB + 1)>(xsp, ad, g, G);
+        if constexpr (GRAM) gram_chunk<NB, N8, J * GP + E3, (J + 1) * GP>(xsp, ad, g, G);
     });
-    __syncwarp();
+    if constexpr (XS) __syncwarp();
 }
 
 // Per-warp ring of landing row-blocks fed by bulk async copies.
@@ -282,7 +294,7 @@ struct SmemPlan {
     static constexpr size_t xs = bars + ((WARPS * STAGES + 1) & ~1);
     static constexpr size_t ring = xs + (size_t)WARPS * XSBUF * 8 * N8;
     static constexpr size_t ring_doubles = (size_t)WARPS * STAGES * 8 * LDL;
-    static constexpr size_t red_doubles = (size_t)WARPS * TallCfg<NB>::NBLK * 64;
+    static constexpr size_t red_doubles = XSBUF ? (size_t)WARPS * TallCfg<NB>::NBLK * 64 : 0;   // A4 only
     static constexpr size_t total_doubles =
         (ring + ring_doubles) > red_doubles ? (ring + ring_doubles) : red_doubles;
     static constexpr size_t bytes = total_doubles * sizeof(double);
@@ -358,8 +370,8 @@ k_trsm_gram_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
         const double* xsp = xs + ((it & 1) ^ 1) * 8 * N8;
         if (HAS_R) {
             double* gout = V1 ? V1 + rblk * 8 * ldq : nullptr;
-            if (it > 0) trsm_rowblock<NB, true>(acc, xsc, xsp, ad, Tf, nRf, gout, ldq, valid, n, lane, g, G);
-            else        trsm_rowblock<NB, false>(acc, xsc, xsp, ad, Tf, nRf, gout, ldq, valid, n, lane, g, G);
+            if (it > 0) trsm_rowblock<NB, true, true>(acc, xsc, xsp, ad, Tf, nRf, gout, ldq, valid, n, lane, g, G);
+            else        trsm_rowblock<NB, false, true>(acc, xsc, xsp, ad, Tf, nRf, gout, ldq, valid, n, lane, g, G);
         } else {
             // plain Gram of V: move the row-block into xs, Gram of the previous one meanwhile
 #pragma unroll
@@ -412,7 +424,7 @@ k_apply_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
             const double* __restrict__ R0, const double* __restrict__ R1,
             double* __restrict__ Q, int64_t ldq)
 {
-    using Plan = SmemPlan<NB, APPLY_WARPS, APPLY_STAGES, 2, 1>;
+    using Plan = SmemPlan<NB, APPLY_WARPS, APPLY_STAGES, 2, 0>;
     constexpr int LDL = Plan::LDL, N8 = Plan::N8;
     constexpr int FD = TallCfg<NB>::FRAG_DOUBLES;
     constexpr int NBLK = TallCfg<NB>::NBLK;
@@ -425,7 +437,6 @@ k_apply_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + Plan::bars);
     double* ring = smem + Plan::ring;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    double* xs = smem + Plan::xs + (size_t)warp * 8 * N8;
 
     for (int i = threadIdx.x; i < (int)Plan::ring_doubles; i += blockDim.x) ring[i] = 0.0;
     if (threadIdx.x < APPLY_WARPS * APPLY_STAGES) mbar_init(bars + threadIdx.x, 1);
@@ -457,16 +468,8 @@ k_apply_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
             __syncwarp();
         }
         load_acc<NB, LDL>(acc, rb, lane);
-        if (TWO) {
-            trsm_rowblock<NB, false>(acc, xs, xs, ad, Tf0, nRf0, nullptr, ldq, valid, n, lane, g, G);
-#pragma unroll
-            for (int J = 0; J < NB; ++J) {
-                double2 v = *reinterpret_cast<const double2*>(xs + ad.c(J));
-                acc[J][0] = v.x; acc[J][1] = v.y;
-            }
-            __syncwarp();
-        }
-        trsm_rowblock<NB, false>(acc, xs, xs, ad, Tf1, nRf1, Q + rblk * 8 * ldq, ldq, valid, n, lane, g, G);
+        if (TWO) trsm_rowblock<NB, false, false>(acc, nullptr, nullptr, ad, Tf0, nRf0, nullptr, ldq, valid, n, lane, g, G);
+        trsm_rowblock<NB, false, false>(acc, nullptr, nullptr, ad, Tf1, nRf1, Q + rblk * 8 * ldq, ldq, valid, n, lane, g, G);
         const int64_t next = rblk + (int64_t)APPLY_STAGES * stride;
         if (next < nrb) {
             fence_proxy_async();
@@ -528,7 +531,7 @@ template <int NB>
 static int launch_apply(const double* V, int64_t m, int n, int64_t ldv, const double* R0, const double* R1,
                         double* Q, int64_t ldq, cudaStream_t st)
 {
-    using Plan = SmemPlan<NB, APPLY_WARPS, APPLY_STAGES, 2, 1>;
+    using Plan = SmemPlan<NB, APPLY_WARPS, APPLY_STAGES, 2, 0>;
     static_assert(Plan::bytes <= 227 * 1024, "A6 shared memory plan too large");
     static bool attr = false;
     if (!attr) {
