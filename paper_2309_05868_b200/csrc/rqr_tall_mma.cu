@@ -219,18 +219,36 @@ __device__ __forceinline__ void gram_chunk(const double* __restrict__ xsp, const
 // chain  T(s=0) -> T(s=1) -> U(J+1, s=0) -> U(J+1, s=1) -> next step.
 // The arithmetic on (acc, Tf, nRf) is the same instruction sequence for every caller (H1).
 // ------------------------------------------------------------------------------------------
-template <int NB, bool GRAM, bool XS>
+// Per-lane output state of a row-block: gp = address of (row r, column 2q) in the output or
+// nullptr when this lane's row is not stored; colmask bit 2J = "columns 8J+2q and 8J+2q+1 both
+// exist", bit 2J+1 = "column 8J+2q exists" (computed once per kernel by col_mask()).
+template <int NB>
+__device__ __forceinline__ uint32_t col_mask(int n, int lane)
+{
+    uint32_t msk = 0;
+#pragma unroll
+    for (int J = 0; J < NB; ++J) {
+        const int c = 8 * J + 2 * (lane & 3);
+        msk |= (uint32_t)(c + 1 < n) << (2 * J);
+        msk |= (uint32_t)(c < n) << (2 * J + 1);
+    }
+    return msk;
+}
+
+// `after_first` runs once after step 0 has issued its updates: every acc register loaded from the
+// landing block has been consumed by a DMMA by then, so the hook may refill that block.
+template <int NB, bool GRAM, bool XS, bool FULL, class Hook>
 __device__ __forceinline__ void trsm_rowblock(double (&acc)[NB][2], double* __restrict__ xsc,
                                               const double* __restrict__ xsp,
                                               const XsAddr<8 * NB>& ad, const double* __restrict__ Tf,
-                                              const double* __restrict__ nRf, double* __restrict__ gout,
-                                              int64_t ldq, int rows_valid, int n, int lane,
-                                              double (&g)[NB], double (&G)[NB * (NB + 1) / 2][2])
+                                              const double* __restrict__ nRf, double* __restrict__ gp,
+                                              uint32_t colmask, int lane,
+                                              double (&g)[NB], double (&G)[NB * (NB + 1) / 2][2],
+                                              Hook&& after_first)
 {
     constexpr int N8 = 8 * NB;
     constexpr int GP = NB + 1;                       // Gram DMMAs per step
     constexpr int E1 = GP / 4, E2 = GP / 2, E3 = (3 * GP) / 4;
-    const int r = lane >> 2, q = lane & 3;
     static_for<0, NB>([&](auto Jc) {
         constexpr int J = decltype(Jc)::value;
         double x0 = 0.0, x1 = 0.0;
@@ -246,13 +264,14 @@ __device__ __forceinline__ void trsm_rowblock(double (&acc)[NB][2], double* __re
         for (int Jp = J + 1; Jp < NB; ++Jp)
             dmma(acc[Jp][0], acc[Jp][1], x1, nRf[TriFrags<NB>::pair(J, Jp) * 64 + 32 + lane]);
         acc[J][0] = x0; acc[J][1] = x1;
-        if constexpr (XS) *reinterpret_cast<double2*>(xsc + ad.c(J)) = make_double2(x0, x1);
-        if (gout != nullptr && r < rows_valid) {
-            const int c = 8 * J + 2 * q;
-            if (c + 1 < n) *reinterpret_cast<double2*>(gout + (int64_t)r * ldq + c) = make_double2(x0, x1);
-            else if (c < n) gout[(int64_t)r * ldq + c] = x0;
-        }
+        if constexpr (J == 0) after_first();
         if constexpr (GRAM) gram_chunk<NB, N8, J * GP + E3, (J + 1) * GP>(xsp, ad, g, G);
+        // stores last: x has long been produced, the warp does not stall on the DMMA result
+        if constexpr (XS) *reinterpret_cast<double2*>(xsc + ad.c(J)) = make_double2(x0, x1);
+        if (gp != nullptr) {
+            if (FULL || ((colmask >> (2 * J)) & 1u)) *reinterpret_cast<double2*>(gp + 8 * J) = make_double2(x0, x1);
+            else if ((colmask >> (2 * J + 1)) & 1u) gp[8 * J] = x0;
+        }
     });
     if constexpr (XS) __syncwarp();
 }
@@ -315,7 +334,7 @@ __device__ __forceinline__ void load_acc(double (&acc)[NB][2], const double* __r
 // ------------------------------------------------------------------------------------------
 // A4: V1 = V R0^-1 (optional), store V1 (optional), partial Gram per CTA.
 // ------------------------------------------------------------------------------------------
-template <int NB, bool HAS_R>
+template <int NB, bool HAS_R, bool FULL>
 __global__ void __launch_bounds__(GRAM_WARPS * 32, 1)
 k_trsm_gram_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
                 const double* __restrict__ R0, double* __restrict__ V1, int64_t ldq,
@@ -354,11 +373,13 @@ k_trsm_gram_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
     for (int b = 0; b < NBLK; ++b) { G[b][0] = 0.0; G[b][1] = 0.0; }
     double g[NB];
     double acc[NB][2];
+    const uint32_t colmask = col_mask<NB>(n, lane);
+    const int64_t lane_off = (int64_t)(lane >> 2) * ldq + 2 * (lane & 3);
 
-    int it = 0;
+    int it = 0, stage = 0;
+    uint32_t phase = 0;
     for (int64_t rblk = gw; rblk < nrb; rblk += stride, ++it) {
-        const int stage = it % GRAM_STAGES;
-        mbar_wait(wr.bar + stage, (uint32_t)((it / GRAM_STAGES) & 1));
+        mbar_wait(wr.bar + stage, phase);
         double* rb = wr.buf + stage * 8 * LDL;
         const int valid = (int)((m - rblk * 8) < 8 ? (m - rblk * 8) : 8);
         if (valid < 8) {
@@ -366,27 +387,31 @@ k_trsm_gram_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
             __syncwarp();
         }
         load_acc<NB, LDL>(acc, rb, lane);
+        // refill of the landing block once its values have been consumed (registers -> DMMA / xs)
+        auto refill = [&]() {
+            const int64_t next = rblk + (int64_t)GRAM_STAGES * stride;
+            if (next < nrb) {
+                fence_proxy_async();
+                __syncwarp();
+                wr.issue(stage, next, lane);
+            }
+        };
         double* xsc = xs + (it & 1) * 8 * N8;
         const double* xsp = xs + ((it & 1) ^ 1) * 8 * N8;
         if (HAS_R) {
-            double* gout = V1 ? V1 + rblk * 8 * ldq : nullptr;
-            if (it > 0) trsm_rowblock<NB, true, true>(acc, xsc, xsp, ad, Tf, nRf, gout, ldq, valid, n, lane, g, G);
-            else        trsm_rowblock<NB, false, true>(acc, xsc, xsp, ad, Tf, nRf, gout, ldq, valid, n, lane, g, G);
+            double* gp = (V1 && (lane >> 2) < valid) ? V1 + rblk * 8 * ldq + lane_off : nullptr;
+            if (it > 0) trsm_rowblock<NB, true, true, FULL>(acc, xsc, xsp, ad, Tf, nRf, gp, colmask, lane, g, G, refill);
+            else        trsm_rowblock<NB, false, true, FULL>(acc, xsc, xsp, ad, Tf, nRf, gp, colmask, lane, g, G, refill);
         } else {
             // plain Gram of V: move the row-block into xs, Gram of the previous one meanwhile
 #pragma unroll
             for (int J = 0; J < NB; ++J)
                 *reinterpret_cast<double2*>(xsc + ad.c(J)) = make_double2(acc[J][0], acc[J][1]);
+            refill();
             if (it > 0) gram_chunk<NB, N8, 0, 2 * NBLK>(xsp, ad, g, G);
             __syncwarp();
         }
-        // the landing block was consumed by load_acc: refill it
-        const int64_t next = rblk + (int64_t)GRAM_STAGES * stride;
-        if (next < nrb) {
-            fence_proxy_async();
-            __syncwarp();
-            wr.issue(stage, next, lane);
-        }
+        if (++stage == GRAM_STAGES) { stage = 0; phase ^= 1u; }
     }
     if (it > 0) {
         __syncwarp();
@@ -418,7 +443,7 @@ k_trsm_gram_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
 // ------------------------------------------------------------------------------------------
 // A6: Q = (V R0^-1) R1^-1  (TWO) or Q = V R1^-1.
 // ------------------------------------------------------------------------------------------
-template <int NB, bool TWO>
+template <int NB, bool TWO, bool FULL>
 __global__ void __launch_bounds__(APPLY_WARPS * 32, 1)
 k_apply_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
             const double* __restrict__ R0, const double* __restrict__ R1,
@@ -457,10 +482,12 @@ k_apply_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
     double acc[NB][2];
     double g[NB];
     double G[NBLK][2];      // unused (GRAM = false): optimised away
-    int it = 0;
-    for (int64_t rblk = gw; rblk < nrb; rblk += stride, ++it) {
-        const int stage = it % APPLY_STAGES;
-        mbar_wait(wr.bar + stage, (uint32_t)((it / APPLY_STAGES) & 1));
+    const uint32_t colmask = col_mask<NB>(n, lane);
+    const int64_t lane_off = (int64_t)(lane >> 2) * ldq + 2 * (lane & 3);
+    int stage = 0;
+    uint32_t phase = 0;
+    for (int64_t rblk = gw; rblk < nrb; rblk += stride) {
+        mbar_wait(wr.bar + stage, phase);
         double* rb = wr.buf + stage * 8 * LDL;
         const int valid = (int)((m - rblk * 8) < 8 ? (m - rblk * 8) : 8);
         if (valid < 8) {
@@ -468,14 +495,23 @@ k_apply_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
             __syncwarp();
         }
         load_acc<NB, LDL>(acc, rb, lane);
-        if (TWO) trsm_rowblock<NB, false, false>(acc, nullptr, nullptr, ad, Tf0, nRf0, nullptr, ldq, valid, n, lane, g, G);
-        trsm_rowblock<NB, false, false>(acc, nullptr, nullptr, ad, Tf1, nRf1, Q + rblk * 8 * ldq, ldq, valid, n, lane, g, G);
-        const int64_t next = rblk + (int64_t)APPLY_STAGES * stride;
-        if (next < nrb) {
-            fence_proxy_async();
-            __syncwarp();
-            wr.issue(stage, next, lane);
+        auto refill = [&]() {
+            const int64_t next = rblk + (int64_t)APPLY_STAGES * stride;
+            if (next < nrb) {
+                fence_proxy_async();
+                __syncwarp();
+                wr.issue(stage, next, lane);
+            }
+        };
+        auto nohook = []() {};
+        double* gp = ((lane >> 2) < valid) ? Q + rblk * 8 * ldq + lane_off : nullptr;
+        if (TWO) {
+            trsm_rowblock<NB, false, false, FULL>(acc, nullptr, nullptr, ad, Tf0, nRf0, nullptr, colmask, lane, g, G, refill);
+            trsm_rowblock<NB, false, false, FULL>(acc, nullptr, nullptr, ad, Tf1, nRf1, gp, colmask, lane, g, G, nohook);
+        } else {
+            trsm_rowblock<NB, false, false, FULL>(acc, nullptr, nullptr, ad, Tf1, nRf1, gp, colmask, lane, g, G, refill);
         }
+        if (++stage == APPLY_STAGES) { stage = 0; phase ^= 1u; }
     }
 }
 
@@ -505,14 +541,16 @@ static int launch_trsm_gram(const double* V, int64_t m, int n, int64_t ldv, cons
     static_assert(Plan::bytes <= 227 * 1024, "A4 shared memory plan too large");
     static bool attr = false;
     if (!attr) {
-        cudaFuncSetAttribute(k_trsm_gram_mma<NB, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
-        cudaFuncSetAttribute(k_trsm_gram_mma<NB, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
+        cudaFuncSetAttribute(k_trsm_gram_mma<NB, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
+        cudaFuncSetAttribute(k_trsm_gram_mma<NB, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
+        cudaFuncSetAttribute(k_trsm_gram_mma<NB, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
         attr = true;
     }
     const int grid = grid_for(m, GRAM_WARPS);
     *nparts = grid;
-    if (R0) k_trsm_gram_mma<NB, true><<<grid, GRAM_WARPS * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, V1, ldq, part);
-    else    k_trsm_gram_mma<NB, false><<<grid, GRAM_WARPS * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, nullptr, ldq, part);
+    if (R0 && n == 8 * NB) k_trsm_gram_mma<NB, true, true><<<grid, GRAM_WARPS * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, V1, ldq, part);
+    else if (R0)           k_trsm_gram_mma<NB, true, false><<<grid, GRAM_WARPS * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, V1, ldq, part);
+    else                   k_trsm_gram_mma<NB, false, false><<<grid, GRAM_WARPS * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, nullptr, ldq, part);
     RQR_LAUNCH_CHECK();
     return RQR_OK;
 }
@@ -535,13 +573,18 @@ static int launch_apply(const double* V, int64_t m, int n, int64_t ldv, const do
     static_assert(Plan::bytes <= 227 * 1024, "A6 shared memory plan too large");
     static bool attr = false;
     if (!attr) {
-        cudaFuncSetAttribute(k_apply_mma<NB, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
-        cudaFuncSetAttribute(k_apply_mma<NB, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
+        cudaFuncSetAttribute(k_apply_mma<NB, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
+        cudaFuncSetAttribute(k_apply_mma<NB, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
+        cudaFuncSetAttribute(k_apply_mma<NB, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
+        cudaFuncSetAttribute(k_apply_mma<NB, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
         attr = true;
     }
     const int grid = grid_for(m, APPLY_WARPS);
-    if (R0) k_apply_mma<NB, true><<<grid, APPLY_WARPS * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, R1, Q, ldq);
-    else    k_apply_mma<NB, false><<<grid, APPLY_WARPS * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, R1, Q, ldq);
+    const bool full = (n == 8 * NB);
+    if (R0 && full)  k_apply_mma<NB, true, true><<<grid, APPLY_WARPS * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, R1, Q, ldq);
+    else if (R0)     k_apply_mma<NB, true, false><<<grid, APPLY_WARPS * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, R1, Q, ldq);
+    else if (full)   k_apply_mma<NB, false, true><<<grid, APPLY_WARPS * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, R1, Q, ldq);
+    else             k_apply_mma<NB, false, false><<<grid, APPLY_WARPS * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, R1, Q, ldq);
     RQR_LAUNCH_CHECK();
     return RQR_OK;
 }
