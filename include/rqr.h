@@ -60,7 +60,8 @@ extern "C" {
                                  what it needs first, on the same stream.                   */
 #define RQR_FLAG_RECOMPUTE_V1 2 /* one-shot drivers: do not store V1 = V R0^-1; re-form it in
                                  the apply pass with bit-identical arithmetic (32mn bytes of
-                                 traffic instead of 40mn, 4mn^2 flops instead of 3mn^2)      */
+                                 traffic instead of 40mn, 4mn^2 flops instead of 3mn^2).
+                                 Honoured for n <= 64; for n > 64 V1 is always stored.       */
 
 /* Size in bytes of the workspace every call below accepts for this problem shape. */
 size_t rqr_workspace_bytes(int64_t m, int n, int64_t s1, int s2, int variant);
@@ -90,7 +91,10 @@ int rqr_small_geqrf(double* W, int s2, int n, double* R0, int* d_info, void* str
  * PAPER.md:449-453) and Gram matrix G = V1^T V1 (Alg. 2 step 1), split over
  * row tiles with a fixed-order reduction.  R0 == NULL means identity (plain Gram of V).
  * G (n x n) is written full symmetric.  V1 != NULL: V1 (m x n, ld ldq) is also stored;
- * V1 == V is allowed.                                                                        */
+ * V1 == V is allowed.  For n > 64 with R0 != NULL the tensor-core path needs V1 (returns -7
+ * otherwise): the substitution and the Gram are two kernels there, and a V1 re-formed by other
+ * arithmetic would not be the matrix rqr_apply transforms (orthogonality would drop to
+ * u kappa(V)).                                                                                */
 int rqr_trsm_gram(const double* V, int64_t m, int n, int64_t ldv, const double* R0, double* G,
                   double* V1, int64_t ldq, void* work, void* stream);
 

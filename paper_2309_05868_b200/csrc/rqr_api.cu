@@ -41,7 +41,7 @@ static int check_common(const double* V, int64_t m, int n, double* Q, double* R,
 static int tail_cholqr(const double* V, int64_t m, int n, const double* R0, double* Q, double* R1,
                        double* G, void* work, int* d_info, int recompute, cudaStream_t st)
 {
-    if (recompute && R0) {
+    if (recompute && R0 && n <= 64) {     // n > 64: A4 is FP64-bound either way and V1 is always stored
         RQR_TRY(rqr_trsm_gram(V, m, n, n, R0, G, nullptr, n, work, st));
         RQR_TRY(rqr_chol_dev(G, n, 0.0, nullptr, R1, d_info, st));
         RQR_TRY(rqr_apply(V, m, n, n, R0, R1, Q, n, work, st));

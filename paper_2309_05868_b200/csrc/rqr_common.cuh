@@ -10,6 +10,7 @@
 #define RQR_MAX_S2 512
 #define RQR_MAX_GRAM_PARTIALS 304        // >= 2 CTAs per SM on 148 SMs
 #define RQR_GAUSS_PARTIAL_ROWS 16384     // ksplit * s2 <= this
+#define RQR_PANEL_FRAG_BYTES (2 * 10 * 4096 * sizeof(double))   // rqr_tall_panel.cu
 
 #define RQR_PHILOX_STREAM_COUNT 0u
 #define RQR_PHILOX_STREAM_S2 1u
@@ -26,7 +27,8 @@ static inline size_t rqr_align256(size_t x) { return (x + 255) & ~(size_t)255; }
 // Workspace layout.  Offsets of a region depend only on
 // arguments every user of that region has.
 //   [0,256)            header: counters / flags used inside single calls
-//   A  tall scratch    f(n)      Gram partials, small matrices of the one-shot drivers
+//   A  tall scratch    f(n)      Gram partials, small matrices of the one-shot drivers, panel
+//                                fragment slots of the n > 64 kernels (2 sets x 10 x 32 KB)
 //   B  bucket offsets  f(s1)     (s1+1) u32 offsets, s1 u32 cursors
 //   C  S2 slot         f(s1)     sized for s2 = RQR_MAX_S2
 //   D  gauss partials  f(n)
@@ -34,7 +36,7 @@ static inline size_t rqr_align256(size_t x) { return (x + 255) & ~(size_t)255; }
 //   F  one-shot        W1 (s1 x n), W (s2max x n)
 // ---------------------------------------------------------------------------------------
 struct RqrLayout {
-    size_t hdr, A, A_small, B_off, B_cur, C, D, E, F_W1, F_W, total;
+    size_t hdr, A, A_small, A_frags, B_off, B_cur, C, D, E, F_W1, F_W, total;
 };
 
 static inline RqrLayout rqr_layout(int64_t m, int n, int64_t s1)
@@ -44,7 +46,8 @@ static inline RqrLayout rqr_layout(int64_t m, int n, int64_t s1)
     L.hdr = 0;
     L.A = 256;
     L.A_small = L.A + rqr_align256((size_t)RQR_MAX_GRAM_PARTIALS * nn);
-    L.B_off = L.A_small + rqr_align256(16 * nn);
+    L.A_frags = L.A_small + rqr_align256(16 * nn);
+    L.B_off = L.A_frags + RQR_PANEL_FRAG_BYTES;
     L.B_cur = L.B_off + rqr_align256((size_t)(s1 + 1) * 4);
     L.C = L.B_cur + rqr_align256((size_t)s1 * 4);
     L.D = L.C + rqr_align256((size_t)RQR_MAX_S2 * (size_t)s1 * sizeof(double));

@@ -135,8 +135,11 @@ extern "C" int rqr_trsm_gram(const double* V, int64_t m, int n, int64_t ldv, con
     cudaStream_t st = (cudaStream_t)stream;
     double* part = (double*)((char*)work + 256);        // region A
     int nparts = 0;
+    double* frags = (double*)((char*)work + rqr_layout(1, n, 1).A_frags);
     int rc = g_force_generic ? RQR_TALL_NOT_HANDLED
                              : rqr_trsm_gram_mma(V, m, n, ldv, R0, V1, ldq, part, &nparts, st);
+    if (rc == RQR_TALL_NOT_HANDLED && !g_force_generic)
+        rc = rqr_trsm_gram_panel(V, m, n, ldv, R0, V1, ldq, part, &nparts, frags, st);
     if (rc == RQR_TALL_NOT_HANDLED) {
         generic_attrs();
         nparts = generic_grid(m);
@@ -160,9 +163,13 @@ extern "C" int rqr_apply(const double* V, int64_t m, int n, int64_t ldv, const d
     if (!R1) return -6;
     if (!Q) return -7;
     if (ldq < n) return -8;
-    (void)work;
     cudaStream_t st = (cudaStream_t)stream;
     int rc = g_force_generic ? RQR_TALL_NOT_HANDLED : rqr_apply_mma(V, m, n, ldv, R0, R1, Q, ldq, st);
+    if (rc == RQR_TALL_NOT_HANDLED && !g_force_generic && n > 64) {
+        if (!work) return -9;
+        rc = rqr_apply_panel(V, m, n, ldv, R0, R1, Q, ldq,
+                             (double*)((char*)work + rqr_layout(1, n, 1).A_frags), st);
+    }
     if (rc == RQR_TALL_NOT_HANDLED) {
         generic_attrs();
         size_t smem = (size_t)GEN_TR * (n + 1) * sizeof(double);

@@ -1,0 +1,430 @@
+// rqr_tall_panel.cu -- FP64 DMMA paths of A4 (rqr_trsm_gram) and A6 (rqr_apply) for 64 < n <= 256.
+//
+// For n >= 128 both halves of A4 are FP64-bound on B200 (n/8 and n/4 flop/byte against a ridge of
+// 5.7), so fusing them saves nothing; and the Gram accumulator (n^2/2 doubles) no longer fits next
+// to the substitution state in one SM's register file.  A4 is therefore two kernels:
+//   k_trsm_panel  X = V R^-1 (row-wise blocked substitution, eq. (42)), stores X
+//   k_syrk_fold   G = X^T X partials (Alg. 2 step 1)
+// and A6 is k_trsm_panel in place.  ("large n".)
+//
+// k_trsm_panel: columns in panels of 64.  A warp owns an 8-row block; the whole block (NP panels
+// x 8 C fragments) lives in registers.  For panel P:  x_P -= x_P' R[P',P] (P' < P; 128 independent
+// DMMAs per pair), then the in-panel chain with R[P,P] (trsm_rowblock<8>, the routine of the
+// n <= 64 kernels).  The B fragments of one (P',P) step are a 32 KB slot, prebuilt in global memory
+// by k_build_panel_frags and streamed through a CTA-wide double buffer by a producer warp with
+// bulk async copies (full/empty mbarriers); the 8 consumer warps use each slot once per row-block.
+//
+// k_syrk_fold: the upper block triangle of G (NB x NB blocks of 8 x 8, NB even) is folded into NB/2
+// rows of NB+1 blocks -- fold f = {(f, b): b >= f} + {(NB-1-f, b): b >= NB-1-f} -- one fold per warp,
+// perfectly balanced; all its operands are the column-block fragments f..NB-1 of a 4-row slab, loaded
+// once per slab.  Accumulators stay in registers for the whole kernel.  NB = 32 needs two CTAs
+// (blockIdx.y) to hold all folds: they walk the same row tiles, the second read hits L2.
+#include "rqr_mma.cuh"
+
+#define PANEL_WARPS 8        // consumer warps; warp PANEL_WARPS is the producer
+#define PANEL_SLOT 4096      // doubles per fragment slot (32 KB)
+#define PANEL_DIAG 2304      // doubles used by a diagonal slot: Tf (8*64) + nRf (28*64)
+#define SYRK_TR 32           // rows per tile of k_syrk_fold
+
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(smem_u32(bar)) : "memory");
+}
+
+// slot order: for P = 0..NP-1: off(0,P), ..., off(P-1,P), diag(P)
+__host__ __device__ __forceinline__ void panel_slot_decode(int s, int& Pp, int& P)
+{
+    P = 0;
+    while (s > P) { s -= P + 1; ++P; }
+    Pp = s;                                  // Pp == P: diagonal slot
+}
+
+// One CTA per slot.  off(P',P)[((J'*8+J)*2+s)*32+lane] = -R[64P'+8J'+2(lane%4)+s][64P+8J+lane/4];
+// diag(P) = the Tf / nRf arrays of build_tri_frags for the 64x64 block R[P,P].  Padded with identity.
+__global__ void __launch_bounds__(256)
+k_build_panel_frags(const double* __restrict__ R, int n, double* __restrict__ frags)
+{
+    __shared__ double scratch[8 * 64];
+    int Pp, P;
+    panel_slot_decode(blockIdx.x, Pp, P);
+    double* out = frags + (size_t)blockIdx.x * PANEL_SLOT;
+    if (Pp == P) {
+        build_tri_frags<8>(R, n, out, out + 512, scratch, 64 * P);
+    } else {
+        for (int t = threadIdx.x; t < PANEL_SLOT; t += blockDim.x) {
+            const int jj = t >> 6, h = (t >> 5) & 1, lane = t & 31;
+            const int Jp = jj >> 3, J = jj & 7;
+            out[t] = -r_padded(R, n, 64 * Pp + 8 * Jp + 2 * (lane & 3) + h, 64 * P + 8 * J + (lane >> 2));
+        }
+    }
+}
+
+template <int NP>
+struct PanelPlan {
+    static constexpr int N8 = 64 * NP;
+    static constexpr int LDL = N8 + LDL_PAD;
+    static constexpr int STEPS = NP * (NP + 1) / 2;
+    static constexpr int LSTAGES = (NP <= 2) ? 2 : 1;
+    static constexpr int NBARS = 4 + PANEL_WARPS * LSTAGES;       // full[2], empty[2], landing
+    static constexpr size_t bars = 2 * PANEL_SLOT;                // doubles
+    static constexpr size_t ring = bars + ((NBARS + 1) & ~1);
+    static constexpr size_t ring_doubles = (size_t)PANEL_WARPS * LSTAGES * 8 * LDL;
+    static constexpr size_t bytes = (ring + ring_doubles) * sizeof(double);
+};
+
+// X = V R^-1 (npass = 1) or (V Ra^-1) Rb^-1 (npass = 2; fragment sets Ra then Rb), X -> Q.
+template <int NP, bool FULL>
+__global__ void __launch_bounds__((PANEL_WARPS + 1) * 32, 1)
+k_trsm_panel(const double* V, int64_t m, int n, int64_t ldv, const double* __restrict__ frags,
+             int npass, double* Q, int64_t ldq)
+{
+    using Plan = PanelPlan<NP>;
+    constexpr int LDL = Plan::LDL, STEPS = Plan::STEPS, LST = Plan::LSTAGES;
+    extern __shared__ __align__(16) double smem[];
+    double* Bbuf = smem;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + Plan::bars);
+    uint64_t* full = bars;
+    uint64_t* empty = bars + 2;
+    uint64_t* land = bars + 4;
+    double* ring = smem + Plan::ring;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+
+    for (int i = threadIdx.x; i < (int)Plan::ring_doubles; i += blockDim.x) ring[i] = 0.0;
+    if (threadIdx.x < 2) mbar_init(full + threadIdx.x, 1);
+    else if (threadIdx.x < 4) mbar_init(empty + (threadIdx.x - 2), PANEL_WARPS);
+    else if (threadIdx.x < Plan::NBARS) mbar_init(bars + threadIdx.x, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    fence_proxy_async();
+    __syncthreads();
+
+    const int64_t nrb = (m + 7) / 8;
+    const int64_t ntiles = (nrb + PANEL_WARPS - 1) / PANEL_WARPS;
+
+    if (warp == PANEL_WARPS) {
+        // producer: streams the fragment slots, in consumption order, for every tile of this CTA
+        if (lane == 0) {
+            int buf = 0;
+            uint32_t ph = 0;
+            for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x)
+                for (int pass = 0; pass < npass; ++pass)
+                    for (int s = 0; s < STEPS; ++s) {
+                        int Pp, P;
+                        panel_slot_decode(s, Pp, P);
+                        const uint32_t bytes = (uint32_t)((Pp == P ? PANEL_DIAG : PANEL_SLOT) * sizeof(double));
+                        mbar_wait(empty + buf, ph ^ 1u);
+                        mbar_expect_tx(full + buf, bytes);
+                        bulk_g2s(Bbuf + (size_t)buf * PANEL_SLOT,
+                                 frags + ((size_t)pass * STEPS + s) * PANEL_SLOT, bytes, full + buf);
+                        if (++buf == 2) { buf = 0; ph ^= 1u; }
+                    }
+        }
+        return;
+    }
+
+    WarpRing<LDL> wr{ring + (size_t)warp * LST * 8 * LDL, land + warp * LST, V, ldv, m, n};
+    const XsAddr<64> ad(lane);
+    const int r = lane >> 2, q = lane & 3;
+    const int64_t lane_off = (int64_t)r * ldq + 2 * q;
+    uint32_t colmask[NP];
+#pragma unroll
+    for (int P = 0; P < NP; ++P) colmask[P] = col_mask<8>(n - 64 * P, lane);
+#pragma unroll
+    for (int s = 0; s < LST; ++s) {
+        const int64_t t = blockIdx.x + (int64_t)s * gridDim.x;
+        if (t < ntiles && t * PANEL_WARPS + warp < nrb) wr.issue(s, t * PANEL_WARPS + warp, lane);
+    }
+
+    double x[NP][8][2];
+    double g[8];
+    double G[36][2];        // unused by trsm_rowblock<.., GRAM = false>: optimised away
+    int lstage = 0, buf = 0;
+    uint32_t lphase = 0, fph = 0;
+    auto nohook = []() {};
+    for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const int64_t rblk = tile * PANEL_WARPS + warp;
+        const bool active = rblk < nrb;
+        int valid = 0;
+        if (active) {
+            mbar_wait(wr.bar + lstage, lphase);
+            double* rb = wr.buf + lstage * 8 * LDL;
+            valid = (int)((m - rblk * 8) < 8 ? (m - rblk * 8) : 8);
+            if (valid < 8) {
+                for (int e = lane; e < (8 - valid) * LDL; e += 32) rb[valid * LDL + e] = 0.0;
+                __syncwarp();
+            }
+#pragma unroll
+            for (int P = 0; P < NP; ++P)
+#pragma unroll
+                for (int J = 0; J < 8; ++J) {
+                    double2 v = *reinterpret_cast<const double2*>(rb + r * LDL + 64 * P + 8 * J + 2 * q);
+                    x[P][J][0] = v.x; x[P][J][1] = v.y;
+                }
+            // the whole row-block is in registers: refill the stage for the tile LST rounds ahead
+            const int64_t nt = tile + (int64_t)LST * gridDim.x;
+            if (nt < ntiles && nt * PANEL_WARPS + warp < nrb) {
+                fence_proxy_async();
+                __syncwarp();
+                wr.issue(lstage, nt * PANEL_WARPS + warp, lane);
+            }
+        } else {
+#pragma unroll
+            for (int P = 0; P < NP; ++P)
+#pragma unroll
+                for (int J = 0; J < 8; ++J) { x[P][J][0] = 0.0; x[P][J][1] = 0.0; }
+        }
+        if (++lstage == LST) { lstage = 0; lphase ^= 1u; }
+        double* gp = (active && r < valid) ? Q + rblk * 8 * ldq + lane_off : nullptr;
+        for (int pass = 0; pass < npass; ++pass) {
+            double* gpp = (pass == npass - 1) ? gp : nullptr;
+            static_for<0, NP>([&](auto Pc) {
+                constexpr int P = decltype(Pc)::value;
+                static_for<0, P>([&](auto Ppc) {
+                    constexpr int Pp = decltype(Ppc)::value;
+                    mbar_wait(full + buf, fph);
+                    const double* B = Bbuf + (size_t)buf * PANEL_SLOT + lane;
+#pragma unroll
+                    for (int Jp = 0; Jp < 8; ++Jp) {
+#pragma unroll
+                        for (int J = 0; J < 8; ++J)
+                            dmma(x[P][J][0], x[P][J][1], x[Pp][Jp][0], B[((Jp * 8 + J) * 2 + 0) * 32]);
+#pragma unroll
+                        for (int J = 0; J < 8; ++J)
+                            dmma(x[P][J][0], x[P][J][1], x[Pp][Jp][1], B[((Jp * 8 + J) * 2 + 1) * 32]);
+                    }
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(empty + buf);
+                    if (++buf == 2) { buf = 0; fph ^= 1u; }
+                });
+                mbar_wait(full + buf, fph);
+                const double* B = Bbuf + (size_t)buf * PANEL_SLOT;
+                trsm_rowblock<8, false, false, FULL>(x[P], nullptr, nullptr, ad, B, B + 512,
+                                                     gpp ? gpp + 64 * P : nullptr, colmask[P], lane, g, G, nohook);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(empty + buf);
+                if (++buf == 2) { buf = 0; fph ^= 1u; }
+            });
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// k_syrk_fold
+// ------------------------------------------------------------------------------------------
+template <int NB>
+struct SyrkPlan {
+    static constexpr int N8 = 8 * NB;
+    static constexpr int LDS = N8 + 4;          // row stride = 8 words mod 32: Gram-fragment reads conflict free
+    static constexpr int STAGES = (NB <= 16) ? 5 : (NB <= 24 ? 4 : 3);
+    static constexpr size_t stage_doubles = (size_t)SYRK_TR * LDS;
+    static constexpr size_t bars = STAGES * stage_doubles;
+    static constexpr size_t bytes = (bars + 2 * STAGES) * sizeof(double);
+};
+
+// consumer warp owning fold F (compile time): walks the CTA's tiles, then writes its NB+1 blocks
+template <int NB, int F>
+__device__ __forceinline__ void syrk_fold_warp(const double* __restrict__ stages, uint64_t* full, uint64_t* empty,
+                                               int64_t m, int64_t ntiles, int n, int lane,
+                                               double* __restrict__ P)
+{
+    using Plan = SyrkPlan<NB>;
+    constexpr int LDS = Plan::LDS, NF = NB - F, A2 = NB - 1 - 2 * F;
+    const int r = lane >> 2, q = lane & 3;
+    double G[NB + 1][2];
+#pragma unroll
+    for (int b = 0; b <= NB; ++b) { G[b][0] = 0.0; G[b][1] = 0.0; }
+    int stage = 0;
+    uint32_t ph = 0;
+    for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const int64_t left = m - tile * SYRK_TR;
+        const int valid = (int)(left < SYRK_TR ? left : SYRK_TR);
+        mbar_wait(full + stage, ph);
+        const double* base = stages + (size_t)stage * Plan::stage_doubles + q * LDS + r + 8 * F;
+        const int nslab = (valid + 3) >> 2;
+#pragma unroll 1
+        for (int h = 0; h < nslab; ++h) {
+            const bool ok = 4 * h + q < valid;       // rows past the end of V hold stale data
+            double fr[NF];
+#pragma unroll
+            for (int j = 0; j < NF; ++j) fr[j] = ok ? base[(size_t)h * 4 * LDS + 8 * j] : 0.0;
+#pragma unroll
+            for (int j = 0; j < NF; ++j) dmma(G[j][0], G[j][1], fr[0], fr[j]);
+#pragma unroll
+            for (int k = 0; k <= F; ++k) dmma(G[NF + k][0], G[NF + k][1], fr[A2], fr[A2 + k]);
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(empty + stage);
+        if (++stage == Plan::STAGES) { stage = 0; ph ^= 1u; }
+    }
+#pragma unroll
+    for (int b = 0; b <= NB; ++b) {
+        const int a_blk = b < NF ? F : NB - 1 - F;
+        const int b_blk = b < NF ? F + b : NB - 1 - F + (b - NF);
+        const int row = 8 * a_blk + r, col = 8 * b_blk + 2 * q;
+        if (row < n && col < n) P[(size_t)row * n + col] = G[b][0];
+        if (row < n && col + 1 < n) P[(size_t)row * n + col + 1] = G[b][1];
+    }
+}
+
+template <int NB, int F>
+__device__ __forceinline__ void syrk_dispatch(int f, const double* stages, uint64_t* full, uint64_t* empty,
+                                              int64_t m, int64_t ntiles, int n, int lane, double* P)
+{
+    if constexpr (F < NB / 2) {
+        if (f == F) syrk_fold_warp<NB, F>(stages, full, empty, m, ntiles, n, lane, P);
+        else syrk_dispatch<NB, F + 1>(f, stages, full, empty, m, ntiles, n, lane, P);
+    }
+}
+
+// grid = (row walkers, ceil(NB/2 / 8)); part[blockIdx.x] receives this walker's partial (upper blocks)
+template <int NB>
+__global__ void __launch_bounds__((PANEL_WARPS + 1) * 32, 1)
+k_syrk_fold(const double* __restrict__ X, int64_t m, int n, int64_t ldx, double* __restrict__ part)
+{
+    using Plan = SyrkPlan<NB>;
+    extern __shared__ __align__(16) double smem[];
+    double* stages = smem;
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem + Plan::bars);
+    uint64_t* empty = full + Plan::STAGES;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int i = threadIdx.x; i < (int)Plan::bars; i += blockDim.x) stages[i] = 0.0;
+    if (threadIdx.x < Plan::STAGES) mbar_init(full + threadIdx.x, 1);
+    else if (threadIdx.x < 2 * Plan::STAGES) mbar_init(empty + (threadIdx.x - Plan::STAGES), PANEL_WARPS);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    fence_proxy_async();
+    __syncthreads();
+    const int64_t ntiles = (m + SYRK_TR - 1) / SYRK_TR;
+
+    if (warp == PANEL_WARPS) {
+        int stage = 0;
+        uint32_t ph = 0;
+        for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+            const int64_t row0 = tile * SYRK_TR;
+            const int valid = (int)((m - row0) < SYRK_TR ? (m - row0) : SYRK_TR);
+            mbar_wait(empty + stage, ph ^ 1u);
+            if (lane == 0) mbar_expect_tx(full + stage, (uint32_t)(valid * n * 8));
+            __syncwarp();
+            if (lane < valid)
+                bulk_g2s(stages + (size_t)stage * Plan::stage_doubles + (size_t)lane * Plan::LDS,
+                         X + (row0 + lane) * ldx, (uint32_t)(n * 8), full + stage);
+            if (++stage == Plan::STAGES) { stage = 0; ph ^= 1u; }
+        }
+        return;
+    }
+    const int f = blockIdx.y * PANEL_WARPS + warp;
+    double* P = part + (size_t)blockIdx.x * n * n;
+    if (f < NB / 2) {
+        syrk_dispatch<NB, 0>(f, stages, full, empty, m, ntiles, n, lane, P);
+    } else {
+        // no fold for this warp (NB/2 not a multiple of 8): keep the empty-barrier protocol alive
+        int stage = 0;
+        uint32_t ph = 0;
+        for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+            mbar_wait(full + stage, ph);
+            if (lane == 0) mbar_arrive(empty + stage);
+            if (++stage == Plan::STAGES) { stage = 0; ph ^= 1u; }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// host dispatch
+// ------------------------------------------------------------------------------------------
+static bool panel_ok(const void* V, int n, int64_t ldv, const void* Q, int64_t ldq)
+{
+    if (n <= 64 || n > 256 || (n & 1) || (ldv & 1)) return false;
+    if (((uintptr_t)V & 15) != 0) return false;
+    if (Q && (((uintptr_t)Q & 15) != 0 || (ldq & 1))) return false;
+    return true;
+}
+
+template <int NP>
+static int launch_panel(const double* V, int64_t m, int n, int64_t ldv, const double* frags, int npass,
+                        double* Q, int64_t ldq, cudaStream_t st)
+{
+    using Plan = PanelPlan<NP>;
+    static_assert(Plan::bytes <= 227 * 1024, "k_trsm_panel shared memory plan too large");
+    static bool attr = false;
+    if (!attr) {
+        cudaFuncSetAttribute(k_trsm_panel<NP, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
+        cudaFuncSetAttribute(k_trsm_panel<NP, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
+        attr = true;
+    }
+    const int64_t ntiles = ((m + 7) / 8 + PANEL_WARPS - 1) / PANEL_WARPS;
+    const int grid = (int)(ntiles < 148 ? ntiles : 148);
+    const int threads = (PANEL_WARPS + 1) * 32;
+    if (n == 64 * NP) k_trsm_panel<NP, true><<<grid, threads, Plan::bytes, st>>>(V, m, n, ldv, frags, npass, Q, ldq);
+    else              k_trsm_panel<NP, false><<<grid, threads, Plan::bytes, st>>>(V, m, n, ldv, frags, npass, Q, ldq);
+    RQR_LAUNCH_CHECK();
+    return RQR_OK;
+}
+
+template <int NB>
+static int launch_syrk(const double* X, int64_t m, int n, int64_t ldx, double* part, int* nparts, cudaStream_t st)
+{
+    using Plan = SyrkPlan<NB>;
+    static_assert(Plan::bytes <= 227 * 1024, "k_syrk_fold shared memory plan too large");
+    static bool attr = false;
+    if (!attr) {
+        cudaFuncSetAttribute(k_syrk_fold<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
+        attr = true;
+    }
+    constexpr int PARTS = (NB / 2 + PANEL_WARPS - 1) / PANEL_WARPS;
+    const int64_t ntiles = (m + SYRK_TR - 1) / SYRK_TR;
+    int walkers = 148 / PARTS;
+    if (ntiles < walkers) walkers = (int)ntiles;
+    *nparts = walkers;
+    dim3 grid(walkers, PARTS);
+    k_syrk_fold<NB><<<grid, (PANEL_WARPS + 1) * 32, Plan::bytes, st>>>(X, m, n, ldx, part);
+    RQR_LAUNCH_CHECK();
+    return RQR_OK;
+}
+
+static int build_frags(const double* R, int n, int NP, double* frags, cudaStream_t st)
+{
+    k_build_panel_frags<<<NP * (NP + 1) / 2, 256, 0, st>>>(R, n, frags);
+    RQR_LAUNCH_CHECK();
+    return RQR_OK;
+}
+
+int rqr_trsm_gram_panel(const double* V, int64_t m, int n, int64_t ldv, const double* R0, double* V1,
+                        int64_t ldq, double* part, int* nparts, double* frags, cudaStream_t st)
+{
+    if (!panel_ok(V, n, ldv, V1, ldq)) return RQR_TALL_NOT_HANDLED;
+    if (R0 && !V1) return -7;                       // n > 64: V1 must be stored (see include/rqr.h, hazard H1)
+    if (!R0 && V1) return RQR_TALL_NOT_HANDLED;     // plain copy + Gram: generic kernel
+    const int NP = (n + 63) / 64;
+    const double* X = V;
+    int64_t ldx = ldv;
+    if (R0) {
+        int rc = build_frags(R0, n, NP, frags, st);
+        if (rc != RQR_OK) return rc;
+        rc = NP == 2 ? launch_panel<2>(V, m, n, ldv, frags, 1, V1, ldq, st)
+           : NP == 3 ? launch_panel<3>(V, m, n, ldv, frags, 1, V1, ldq, st)
+                     : launch_panel<4>(V, m, n, ldv, frags, 1, V1, ldq, st);
+        if (rc != RQR_OK) return rc;
+        X = V1;
+        ldx = ldq;
+    }
+    return NP == 2 ? launch_syrk<16>(X, m, n, ldx, part, nparts, st)
+         : NP == 3 ? launch_syrk<24>(X, m, n, ldx, part, nparts, st)
+                   : launch_syrk<32>(X, m, n, ldx, part, nparts, st);
+}
+
+int rqr_apply_panel(const double* V, int64_t m, int n, int64_t ldv, const double* R0, const double* R1,
+                    double* Q, int64_t ldq, double* frags, cudaStream_t st)
+{
+    if (!panel_ok(V, n, ldv, Q, ldq)) return RQR_TALL_NOT_HANDLED;
+    const int NP = (n + 63) / 64;
+    const int steps = NP * (NP + 1) / 2;
+    int npass = 1, rc;
+    if (R0) {
+        rc = build_frags(R0, n, NP, frags, st);
+        if (rc != RQR_OK) return rc;
+        npass = 2;
+    }
+    rc = build_frags(R1, n, NP, frags + (size_t)(npass - 1) * steps * PANEL_SLOT, st);
+    if (rc != RQR_OK) return rc;
+    return NP == 2 ? launch_panel<2>(V, m, n, ldv, frags, npass, Q, ldq, st)
+         : NP == 3 ? launch_panel<3>(V, m, n, ldv, frags, npass, Q, ldq, st)
+                   : launch_panel<4>(V, m, n, ldv, frags, npass, Q, ldq, st);
+}

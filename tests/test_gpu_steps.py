@@ -137,7 +137,8 @@ def test_small_geqrf_flags_rank_deficiency(rq, orc):
     assert int(info.item()) == rq.INFO_SINGULAR + 2 == io - orc.ORC_SINGULAR + rq.INFO_SINGULAR
 
 
-SHAPES_TALL = [(20000, 16), (4099, 64), (10000, 70), (3000, 32), (2500, 128), (700, 256), (65, 8), (5, 2)]
+SHAPES_TALL = [(20000, 16), (4099, 64), (10000, 70), (3000, 32), (2500, 128), (700, 256), (65, 8), (5, 2),
+               (40003, 128), (30011, 200), (20000, 256), (9001, 66)]
 
 
 @pytest.mark.parametrize("m,n", SHAPES_TALL)
