@@ -388,15 +388,32 @@ k_gauss_gemm_splitk(const double* __restrict__ S2, const double* __restrict__ W1
     }
 }
 
-// out[e] = sum_{p ascending} part[p][e]
-__global__ void k_reduce_partials(const double* __restrict__ part, int nparts, int64_t elems,
-                                  double* __restrict__ out)
+// out[e] = sum_p part[p][e].  Fixed order: 4 interleaved groups of partials (p = g, g+4, ...; 8
+// loads in flight per thread), then the groups in order 0..3 through shared memory.
+__global__ void __launch_bounds__(256)
+k_reduce_partials(const double* __restrict__ part, int nparts, int64_t elems, double* __restrict__ out)
 {
-    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < elems;
-         e += (int64_t)gridDim.x * blockDim.x) {
-        double s = part[e];
-        for (int p = 1; p < nparts; ++p) s += part[(int64_t)p * elems + e];
-        out[e] = s;
+    __shared__ double sg[4][64];
+    const int64_t e = (int64_t)blockIdx.x * 64 + (threadIdx.x & 63);
+    const int g = threadIdx.x >> 6;
+    double s = 0.0;
+    if (e < elems) {
+        const double* src = part + e;
+        int p = g;
+        for (; p + 28 < nparts; p += 32) {
+            double x[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) x[u] = __ldcg(src + (int64_t)(p + 4 * u) * elems);
+#pragma unroll
+            for (int u = 0; u < 8; ++u) s += x[u];
+        }
+        for (; p < nparts; p += 4) s += __ldcg(src + (int64_t)p * elems);
+    }
+    sg[g][threadIdx.x & 63] = s;
+    __syncthreads();
+    if (g == 0 && e < elems) {
+        const int l = threadIdx.x;
+        out[e] = ((sg[0][l] + sg[1][l]) + sg[2][l]) + sg[3][l];
     }
 }
 
@@ -437,8 +454,7 @@ extern "C" int rqr_gauss_sketch(const double* W1, int64_t s1, int n, int s2, uin
     k_gauss_gemm_splitk<<<grid, 256, 0, st>>>(S2, W1, s1, n, s2, kchunk, part);
     RQR_LAUNCH_CHECK();
     int64_t elems = (int64_t)s2 * n;
-    int rb = (int)((elems + 255) / 256);
-    k_reduce_partials<<<rb, 256, 0, st>>>(part, (int)ks, elems, W);
+    k_reduce_partials<<<(int)((elems + 63) / 64), 256, 0, st>>>(part, (int)ks, elems, W);
     RQR_LAUNCH_CHECK();
     return RQR_OK;
 }
@@ -532,7 +548,7 @@ extern "C" int rqr_dense_gauss_sketch(const double* V, int64_t m, int n, int64_t
     k_dense_gauss_sketch<<<grid, 256, smem, st>>>(V, m, n, ldv, row0, m_total, s, seed, part);
     RQR_LAUNCH_CHECK();
     int64_t elems = (int64_t)s * n;
-    k_reduce_partials<<<(int)((elems + 255) / 256), 256, 0, st>>>(part, (int)P, elems, W);
+    k_reduce_partials<<<(int)((elems + 63) / 64), 256, 0, st>>>(part, (int)P, elems, W);
     RQR_LAUNCH_CHECK();
     return RQR_OK;
 }

@@ -109,6 +109,120 @@ k_geqrf_reg(const double* __restrict__ W, int s2, int n, double* __restrict__ R0
         }
 }
 
+// Small-shape version (s2 <= 128, n <= 64: the n = 64 configs).  A Householder step is a chain of
+// dependent latencies executed by ONE warp, so the kernel is written for few instructions per step
+// (measured on B200: DFMA 8.7 cycles dependent, double shuffle-add round 41, sqrt 95, 1/x 77):
+//   * 8 warps; lane = 8 g + t: column c = 8 w + 4 qq + g (qq = 0, 1), rows i = t + 8 p (p < 16): a dot
+//     product is 16 local fma and a 3-round shuffle reduction inside the 8-lane group;
+//   * finished entries LEAVE the register tile: after step j row j (final R0[j][j+1:]) is written to
+//     global memory and zeroed, the pivot column is zeroed.  The tile then only holds rows > j of
+//     columns > j, so norms, dot products and updates need no row or column predicates;
+//   * beta = 2 / v^T v = 1 / (nrm |v_j|) is formed by every thread in the shadow of its dot product.
+__device__ __forceinline__ double group8_sum(double x)
+{
+#pragma unroll
+    for (int o = 1; o < 8; o <<= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+    return x;
+}
+
+#define RQR_SWITCH16(P_, STMT)                                                                     \
+    switch (P_) {                                                                                  \
+        case 0: { constexpr int P = 0; STMT } break;   case 1: { constexpr int P = 1; STMT } break;   \
+        case 2: { constexpr int P = 2; STMT } break;   case 3: { constexpr int P = 3; STMT } break;   \
+        case 4: { constexpr int P = 4; STMT } break;   case 5: { constexpr int P = 5; STMT } break;   \
+        case 6: { constexpr int P = 6; STMT } break;   case 7: { constexpr int P = 7; STMT } break;   \
+        case 8: { constexpr int P = 8; STMT } break;   case 9: { constexpr int P = 9; STMT } break;   \
+        case 10: { constexpr int P = 10; STMT } break; case 11: { constexpr int P = 11; STMT } break; \
+        case 12: { constexpr int P = 12; STMT } break; case 13: { constexpr int P = 13; STMT } break; \
+        case 14: { constexpr int P = 14; STMT } break; default: { constexpr int P = 15; STMT } break; \
+    }
+
+__global__ void __launch_bounds__(256, 1)
+k_geqrf_g8(const double* __restrict__ W, int s2, int n, double* __restrict__ R0, int* d_info)
+{
+    __shared__ double vbuf[2][128];
+    __shared__ double den_s[2], sgn_s[2];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int g = lane >> 3, t = lane & 7;
+    double a[2][16];
+#pragma unroll
+    for (int qq = 0; qq < 2; ++qq)
+#pragma unroll
+        for (int p = 0; p < 16; ++p) {
+            const int c = 8 * w + 4 * qq + g, i = t + 8 * p;
+            a[qq][p] = (c < n && i < s2) ? W[(int64_t)i * n + c] : 0.0;
+        }
+    for (int e = threadIdx.x; e < n * n; e += 256) {      // exact zeros below the diagonal
+        const int i = e / n, c = e - i * n;
+        if (c < i) R0[e] = 0.0;
+    }
+    for (int j = 0; j < n; ++j) {
+        const int pj = j >> 3, tj = j & 7;
+        if (w == pj) {                                     // warp-uniform: the warp that owns column j
+            auto reflect = [&](double (&col)[16]) {
+                double s0 = 0.0, s1 = 0.0, xe = 0.0;
+#pragma unroll
+                for (int p = 0; p < 16; p += 2) { s0 = fma(col[p], col[p], s0); s1 = fma(col[p + 1], col[p + 1], s1); }
+                RQR_SWITCH16(pj, xe = col[P];)
+                const double ss = group8_sum(s0 + s1);                              // ||a[j:, j]||^2
+                const double x1 = __shfl_sync(0xffffffffu, xe, (lane & 24) | tj);   // a[j][j]
+                const double nrm = sqrt(ss);
+                const double sgn = (x1 < 0.0) ? -1.0 : 1.0;
+                const double vj = x1 + sgn * nrm;
+                if (g == (j & 3)) {
+#pragma unroll
+                    for (int p = 0; p < 16; ++p) vbuf[j & 1][t + 8 * p] = col[p];    // rows < j are zero
+                    if (t == tj) vbuf[j & 1][j] = vj;
+                    if (t == 0) {
+                        den_s[j & 1] = nrm * fabs(vj);                               // v^T v / 2
+                        sgn_s[j & 1] = sgn;
+                        R0[(int64_t)j * n + j] = nrm;           // -sgn*nrm, row negated when sgn > 0 (S4)
+                        if (!(nrm > 0.0) || !(nrm < 1.0e308)) rqr_set_info(d_info, RQR_INFO_SINGULAR + j + 1);
+                    }
+#pragma unroll
+                    for (int p = 0; p < 16; ++p) col[p] = 0.0;                       // column j is done
+                }
+            };
+            if ((j >> 2) & 1) reflect(a[1]); else reflect(a[0]);
+        }
+        __syncthreads();
+        double v[16];
+#pragma unroll
+        for (int p = 0; p < 16; ++p) v[p] = vbuf[j & 1][t + 8 * p];
+        const double den = den_s[j & 1], sg = sgn_s[j & 1];
+        const double beta = (den > 0.0) ? 1.0 / den : 0.0;
+        double dot[2];
+#pragma unroll
+        for (int qq = 0; qq < 2; ++qq) {
+            double s0 = 0.0, s1 = 0.0;
+#pragma unroll
+            for (int p = 0; p < 16; p += 2) { s0 = fma(v[p], a[qq][p], s0); s1 = fma(v[p + 1], a[qq][p + 1], s1); }
+            dot[qq] = s0 + s1;
+        }
+#pragma unroll
+        for (int o = 1; o < 8; o <<= 1) {
+            dot[0] += __shfl_xor_sync(0xffffffffu, dot[0], o);
+            dot[1] += __shfl_xor_sync(0xffffffffu, dot[1], o);
+        }
+#pragma unroll
+        for (int qq = 0; qq < 2; ++qq) {
+            const double ws = beta * dot[qq];            // finished and padding columns are all zero: ws = 0
+#pragma unroll
+            for (int p = 0; p < 16; ++p) a[qq][p] = fma(-ws, v[p], a[qq][p]);
+        }
+        if (t == tj) {                                   // row j is final: move it out of the tile
+            RQR_SWITCH16(pj,
+                _Pragma("unroll")
+                for (int qq = 0; qq < 2; ++qq) {
+                    const int c = 8 * w + 4 * qq + g;
+                    const double val = a[qq][P];
+                    a[qq][P] = 0.0;
+                    if (c > j && c < n) R0[(int64_t)j * n + c] = (sg > 0.0) ? -val : val;
+                })
+        }
+    }
+}
+
 // Generic fallback, any 2 <= n <= 256, s2 <= 512: W stays in global memory (L2-resident) and is
 // destroyed.  1024 threads = 4 row groups x 256 columns.
 __global__ void __launch_bounds__(1024, 1)
@@ -166,6 +280,141 @@ k_geqrf_gmem(double* __restrict__ W, int s2, int n, double* __restrict__ R0, int
     }
 }
 
+
+// ---- thread-block-cluster helpers (CTAs of a cluster run on SMs of one GPC; barrier.cluster costs
+// ~380 cycles; release/acquire at cluster scope orders global-memory traffic between the CTAs) ----
+__device__ __forceinline__ unsigned cluster_rank()
+{
+    unsigned r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r;
+}
+__device__ __forceinline__ unsigned cluster_size()
+{
+    unsigned r; asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r)); return r;
+}
+__device__ __forceinline__ void cluster_sync_all()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+
+// Cluster version of k_geqrf_reg for shapes whose register tile does not fit one CTA (n > 64):
+// W is spread over the CTAs of one cluster, column c -> CTA c % ncta, warp (c / ncta) % 16,
+// slot (c / ncta) / 16; lane l owns rows l + 32 p.  512 threads per CTA.  After the load W's own
+// storage is scratch: the reflector v (double-buffered), beta and the sign flags travel through
+// it (L2) with ONE cluster barrier per Householder step.
+template <int RPL>
+__global__ void __launch_bounds__(512, 1)
+k_geqrf_cluster(double* W, int s2, int n, double* __restrict__ R0, int* d_info)
+{
+    constexpr int CPW = 2;
+    const int ncta = (int)cluster_size(), rank = (int)cluster_rank();
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    double a[CPW][RPL];
+#pragma unroll
+    for (int q = 0; q < CPW; ++q)
+#pragma unroll
+        for (int p = 0; p < RPL; ++p) {
+            const int c = (w + 16 * q) * ncta + rank, i = lane + 32 * p;
+            a[q][p] = (c < n && i < s2) ? W[(int64_t)i * n + c] : 0.0;
+        }
+    cluster_sync_all();                      // everyone holds its columns: W is scratch from here on
+    double* gv = W;                          // [2][32 * RPL]
+    double* gbeta = W + 2 * 32 * RPL;        // [2]
+    double* gflip = gbeta + 2;               // [n]
+    for (int j = 0; j < n; ++j) {
+        const int o = j % ncta, jj = j / ncta, wo = jj & 15, qo = jj >> 4, lj = j & 31;
+        double* vj_buf = gv + (j & 1) * 32 * RPL;
+        if (rank == o && w == wo) {
+            double tail2 = 0.0, x1 = 0.0;
+#pragma unroll
+            for (int q = 0; q < CPW; ++q) if (q == qo) {
+#pragma unroll
+                for (int p = 0; p < RPL; ++p) {
+                    const int i = lane + 32 * p;
+                    if (i > j) tail2 += a[q][p] * a[q][p];
+                    if (i == j) x1 = a[q][p];
+                }
+            }
+            tail2 = warp_sum(tail2);
+            x1 = __shfl_sync(0xffffffffu, x1, lj);
+            const double nrm = sqrt(tail2 + x1 * x1);
+            const double sgn = (x1 < 0.0) ? -1.0 : 1.0;
+            const double vj = x1 + sgn * nrm;
+            const double vtv = tail2 + vj * vj;
+            const double beta = (vtv > 0.0) ? 2.0 / vtv : 0.0;
+            if (lane == 0) {
+                gbeta[j & 1] = beta;
+                gflip[j] = (sgn > 0.0) ? 1.0 : 0.0;       // diagonal becomes -sgn*nrm
+                if (!(nrm > 0.0) || !(nrm < 1.0e308)) rqr_set_info(d_info, RQR_INFO_SINGULAR + j + 1);
+            }
+#pragma unroll
+            for (int q = 0; q < CPW; ++q) if (q == qo) {
+#pragma unroll
+                for (int p = 0; p < RPL; ++p) {
+                    const int i = lane + 32 * p;
+                    vj_buf[i] = (i > j) ? a[q][p] : ((i == j) ? vj : 0.0);
+                    if (i == j) a[q][p] = -sgn * nrm;
+                    else if (i > j) a[q][p] = 0.0;
+                }
+            }
+        }
+        cluster_sync_all();
+        double v[RPL];
+#pragma unroll
+        for (int p = 0; p < RPL; ++p) v[p] = __ldcg(vj_buf + lane + 32 * p);
+        const double beta = __ldcg(gbeta + (j & 1));
+        double dot[CPW];
+#pragma unroll
+        for (int q = 0; q < CPW; ++q) {
+            double sacc = 0.0;
+#pragma unroll
+            for (int p = 0; p < RPL; ++p) sacc = fma(v[p], a[q][p], sacc);
+            dot[q] = sacc;
+        }
+#pragma unroll
+        for (int q = 0; q < CPW; ++q) dot[q] = warp_sum(dot[q]);
+#pragma unroll
+        for (int q = 0; q < CPW; ++q) {
+            const int c = (w + 16 * q) * ncta + rank;
+            if (c > j && c < n) {
+                const double ws = beta * dot[q];
+#pragma unroll
+                for (int p = 0; p < RPL; ++p) a[q][p] = fma(-ws, v[p], a[q][p]);
+            }
+        }
+    }
+    cluster_sync_all();
+#pragma unroll
+    for (int q = 0; q < CPW; ++q)
+#pragma unroll
+        for (int p = 0; p < RPL; ++p) {
+            const int c = (w + 16 * q) * ncta + rank, i = lane + 32 * p;
+            if (c < n && i < n) {
+                double rv = (c >= i) ? a[q][p] : 0.0;
+                if (c >= i && __ldcg(gflip + i) != 0.0) rv = -rv;
+                R0[(int64_t)i * n + c] = rv;
+            }
+        }
+}
+
+template <class K, class... Args>
+static int launch_cluster(K kernel, int ncta, int threads, cudaStream_t st, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(ncta);
+    cfg.blockDim = dim3(threads);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = ncta;
+    at[0].val.clusterDim.y = 1;
+    at[0].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    if (cudaLaunchKernelEx(&cfg, kernel, args...) != cudaSuccess) return RQR_ERR_LAUNCH;
+    return RQR_OK;
+}
+
 extern "C" int rqr_small_geqrf(double* W, int s2, int n, double* R0, int* d_info, void* stream)
 {
     if (!W) return -1;
@@ -174,15 +423,26 @@ extern "C" int rqr_small_geqrf(double* W, int s2, int n, double* R0, int* d_info
     if (!R0) return -4;
     cudaStream_t st = (cudaStream_t)stream;
     const int rpl = (s2 + 31) / 32, cpw = (n + 31) / 32;
+    if (s2 <= 128 && n <= 64) {
+        k_geqrf_g8<<<1, 256, 0, st>>>(W, s2, n, R0, d_info);
+        RQR_LAUNCH_CHECK();
+        return RQR_OK;
+    }
 #define GEQRF_CASE(R, C)                                                              \
     if (rpl <= R && cpw <= C) {                                                       \
         k_geqrf_reg<R, C><<<1, 1024, 0, st>>>(W, s2, n, R0, d_info);                   \
         RQR_LAUNCH_CHECK();                                                           \
         return RQR_OK;                                                                \
     }
-    GEQRF_CASE(1, 1) GEQRF_CASE(2, 1) GEQRF_CASE(4, 1) GEQRF_CASE(4, 2) GEQRF_CASE(8, 2)
-    GEQRF_CASE(16, 1)
+    GEQRF_CASE(8, 1) GEQRF_CASE(8, 2) GEQRF_CASE(16, 1)
 #undef GEQRF_CASE
+    // n > 64: the register tile is spread over a cluster of 4 or 8 CTAs.  W's storage doubles as
+    // the exchange buffer (2 * 32 * RPL + 2 + n doubles), which it always has room for here.
+    if ((int64_t)s2 * n >= 2 * 512 + 2 + n) {
+        const int ncta = n <= 128 ? 4 : 8;
+        if (rpl <= 8) return launch_cluster(k_geqrf_cluster<8>, ncta, 512, st, W, s2, n, R0, d_info);
+        return launch_cluster(k_geqrf_cluster<16>, ncta, 512, st, W, s2, n, R0, d_info);
+    }
     k_geqrf_gmem<<<1, 1024, 0, st>>>(W, s2, n, R0, d_info);
     RQR_LAUNCH_CHECK();
     return RQR_OK;
@@ -190,56 +450,169 @@ extern "C" int rqr_small_geqrf(double* W, int s2, int n, double* R0, int* d_info
 
 // =========================================================================================
 // A5: upper Cholesky factor  G + shift I = R1^T R1   (Alg. 2 step 2)
-// Right-looking, one CTA.  `A` is the working n x n array: shared memory when it fits
-// (n <= 160), else the output buffer R1 in global memory.
 // =========================================================================================
-template <bool SMEM>
-__global__ void __launch_bounds__(1024, 1)
-k_chol(const double* __restrict__ G, int n, double shift_h, const double* __restrict__ d_shift,
-       double* __restrict__ R1, int* d_info)
+// Column-distributed right-looking Cholesky, ONE barrier per step.  Column c -> CTA c % ncta,
+// warp (c / ncta) % NW, slot (c / ncta) / NW; lane l owns rows l + 32 p (rows <= c are used).
+// Step j: every column's warp publishes its row-j entry A[j][c] into a double-buffered row buffer;
+// the lane that owns the pivot A[j][j] also publishes d = A[j][j], r = sqrt(d) and 1/r.  After the
+// barrier every thread forms the entries R[j][a] = A[j][a] (1/r) it needs (same inputs, same
+// operations: identical in every thread) and updates A[a][c] -= R[j][a] R[j][c], j < a <= c.
+// Few warps on purpose: the step is latency-bound and FP64 issue is half rate, so redundant
+// scalar work in 32 warps costs more than the parallelism gains.
+// CL = false: one CTA, row buffer in shared memory; CL = true: a cluster, row buffer in the (not
+// yet written) output R1, cluster barrier.
+#define CHOL_ROW_LD (RQR_MAX_N + 4)      // row entries, then d, r, 1/r
+
+// Single-CTA version (n <= 128), written like k_geqrf_g8 for few instructions per step: row j of R
+// goes straight to global memory when it is formed (no select keeps it in the tile), and
+// r = d rsqrt(d), 1/r = rsqrt(d) come from one MUFU-based sequence on the critical path.
+template <int RPL, int CPW, int NW>
+__global__ void __launch_bounds__(NW * 32, 1)
+k_chol_small(const double* __restrict__ G, int n, double shift_h, const double* __restrict__ d_shift,
+             double* __restrict__ R1, int* d_info)
 {
+    __shared__ double srow[2][CHOL_ROW_LD];
     const double shift = shift_h + (d_shift ? *d_shift : 0.0);
-    extern __shared__ double sA[];
-    __shared__ double dinv_s;
-    __shared__ int fail_s;
-    double* A = SMEM ? sA : R1;
-    const int tid = threadIdx.x;
-    for (int e = tid; e < n * n; e += 1024) {
-        int i = e / n, c = e - i * n;
-        A[e] = G[e] + ((i == c) ? shift : 0.0);
-    }
-    if (tid == 0) fail_s = 0;
-    __syncthreads();
-    for (int j = 0; j < n; ++j) {
-        if (tid == 0) {
-            const double d = A[j * n + j];
-            if (!(d > 0.0) || !(d < 1.0e308)) { fail_s = j + 1; dinv_s = 0.0; }
-            else { const double r = sqrt(d); A[j * n + j] = r; dinv_s = r; }
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    double a[CPW][RPL];
+#pragma unroll
+    for (int q = 0; q < CPW; ++q)
+#pragma unroll
+        for (int p = 0; p < RPL; ++p) {
+            const int c = w + NW * q, i = lane + 32 * p;
+            a[q][p] = (c < n && i <= c) ? G[(int64_t)i * n + c] + ((i == c) ? shift : 0.0) : 0.0;
         }
-        __syncthreads();
-        if (fail_s) break;
-        const double rjj = dinv_s;
-        for (int c = j + 1 + tid; c < n; c += 1024) A[j * n + c] = A[j * n + c] / rjj;
-        __syncthreads();
-        // trailing update of the upper triangle: A[a][b] -= R[j][a] R[j][b], j < a <= b
-        const int t = n - j - 1;
-        for (int e = tid; e < t * t; e += 1024) {
-            int a = e / t, b = e - a * t;
-            if (b >= a) {
-                a += j + 1; b += j + 1;
-                A[a * n + b] = fma(-A[j * n + a], A[j * n + b], A[a * n + b]);
+    for (int e = threadIdx.x; e < 2 * CHOL_ROW_LD; e += NW * 32) (&srow[0][0])[e] = 0.0;
+    for (int e = threadIdx.x; e < n * n; e += NW * 32) {          // exact zeros below the diagonal
+        const int i = e / n, c = e - i * n;
+        if (c < i) R1[e] = 0.0;
+    }
+    __syncthreads();
+    int fail = 0;
+    for (int j = 0; j < n; ++j) {
+        const int lj = j & 31, pj = j >> 5;
+        double* rb = srow[j & 1];
+        if (lane == lj) {                                  // publish row j of the trailing matrix
+#pragma unroll
+            for (int p = 0; p < RPL; ++p) if (p == pj) {   // warp-uniform
+#pragma unroll
+                for (int q = 0; q < CPW; ++q) rb[w + NW * q] = a[q][p];
+            }
+            if (w == j % NW) {                             // this lane holds the pivot A[j][j]
+                const int qj = j / NW;
+                double d = 0.0;
+#pragma unroll
+                for (int q = 0; q < CPW; ++q)
+#pragma unroll
+                    for (int p = 0; p < RPL; ++p) d = (q == qj && p == pj) ? a[q][p] : d;
+                const double ri = rsqrt(d);
+                rb[RQR_MAX_N] = d;
+                rb[RQR_MAX_N + 1] = d * ri;
+                rb[RQR_MAX_N + 2] = ri;
             }
         }
         __syncthreads();
+        const double d = rb[RQR_MAX_N], rjj = rb[RQR_MAX_N + 1], rinv = rb[RQR_MAX_N + 2];
+        if (!(d > 0.0) || !(d < 1.0e308)) { fail = j + 1; break; }      // uniform: same d everywhere
+        double rja[RPL];                                   // R[j][a] for this lane's rows; 0 for a <= j
+#pragma unroll
+        for (int p = 0; p < RPL; ++p) {
+            const int i = lane + 32 * p;
+            rja[p] = (i > j) ? rb[i] * rinv : 0.0;
+        }
+#pragma unroll
+        for (int q = 0; q < CPW; ++q) {
+            const int c = w + NW * q;
+            const double rjc = (c > j) ? rb[c] * rinv : 0.0;            // 0 freezes finished columns
+            if (lane == lj && c >= j && c < n) R1[(int64_t)j * n + c] = (c == j) ? rjj : rjc;
+#pragma unroll
+            for (int p = 0; p < RPL; ++p) a[q][p] = fma(-rja[p], rjc, a[q][p]);   // rows > c: never read
+        }
     }
-    if (fail_s) {
-        if (tid == 0) rqr_set_info(d_info, RQR_INFO_NOT_SPD + fail_s);
+    if (fail && threadIdx.x == 0) rqr_set_info(d_info, RQR_INFO_NOT_SPD + fail);
+}
+
+template <int RPL, int CPW, int NW, bool CL>
+__global__ void __launch_bounds__(NW * 32, 1)
+k_chol_cols(const double* __restrict__ G, int n, double shift_h, const double* __restrict__ d_shift,
+            double* R1, int* d_info)
+{
+    __shared__ double srow[2][CHOL_ROW_LD];
+    const double shift = shift_h + (d_shift ? *d_shift : 0.0);
+    const int ncta = CL ? (int)cluster_size() : 1, rank = CL ? (int)cluster_rank() : 0;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    double* rowbuf = CL ? R1 : &srow[0][0];
+    double a[CPW][RPL];
+#pragma unroll
+    for (int q = 0; q < CPW; ++q)
+#pragma unroll
+        for (int p = 0; p < RPL; ++p) {
+            const int c = (w + NW * q) * ncta + rank, i = lane + 32 * p;
+            a[q][p] = (c < n && i <= c) ? G[(int64_t)i * n + c] + ((i == c) ? shift : 0.0) : 0.0;
+        }
+    int fail = 0;
+    // column ids of this thread's slots (c >= n: a padding column, never stored)
+    int col[CPW];
+#pragma unroll
+    for (int q = 0; q < CPW; ++q) col[q] = (w + NW * q) * ncta + rank;
+    for (int j = 0; j < n; ++j) {
+        const int lj = j & 31, pj = j >> 5;
+        double* rb = rowbuf + (j & 1) * CHOL_ROW_LD;
+        // publish row j (branch-free selects; finished columns publish a value nobody reads)
+        double val[CPW];
+#pragma unroll
+        for (int q = 0; q < CPW; ++q) {
+            val[q] = a[q][0];
+#pragma unroll
+            for (int p = 1; p < RPL; ++p) val[q] = (p == pj) ? a[q][p] : val[q];
+        }
+        if (lane == lj) {
+#pragma unroll
+            for (int q = 0; q < CPW; ++q) {
+                if (col[q] < RQR_MAX_N) rb[col[q]] = val[q];
+                if (col[q] == j) {
+                    const double rjj = sqrt(val[q]);
+                    rb[RQR_MAX_N] = val[q];
+                    rb[RQR_MAX_N + 1] = rjj;
+                    rb[RQR_MAX_N + 2] = 1.0 / rjj;
+                }
+            }
+        }
+        if (CL) cluster_sync_all(); else __syncthreads();
+        const double d = CL ? __ldcg(rb + RQR_MAX_N) : rb[RQR_MAX_N];
+        const double rjj = CL ? __ldcg(rb + RQR_MAX_N + 1) : rb[RQR_MAX_N + 1];
+        const double rinv = CL ? __ldcg(rb + RQR_MAX_N + 2) : rb[RQR_MAX_N + 2];
+        double rja[RPL];                                  // R[j][a] for this lane's rows; 0 for a <= j
+#pragma unroll
+        for (int p = 0; p < RPL; ++p) {
+            const int i = lane + 32 * p;
+            const double x = CL ? __ldcg(rb + (i < RQR_MAX_N ? i : 0)) : rb[i < RQR_MAX_N ? i : 0];
+            rja[p] = (i > j && i < n) ? x * rinv : 0.0;
+        }
+        if (!(d > 0.0) || !(d < 1.0e308)) { fail = j + 1; break; }      // uniform: same d everywhere
+#pragma unroll
+        for (int q = 0; q < CPW; ++q) {
+            const int c = col[q];
+            const double x = CL ? __ldcg(rb + (c < RQR_MAX_N ? c : 0)) : rb[c < RQR_MAX_N ? c : 0];
+            // R[j][c]; 0 for finished (c < j) and padding columns so that their entries stay frozen
+            const double rjc = (c == j) ? rjj : ((c > j && c < n) ? x * rinv : 0.0);
+#pragma unroll
+            for (int p = 0; p < RPL; ++p) {
+                const int i = lane + 32 * p;
+                const double upd = fma(-rja[p], rjc, a[q][p]);       // entries with i > c are never read
+                a[q][p] = (i == j && c >= j) ? rjc : upd;
+            }
+        }
     }
-    __syncthreads();
-    for (int e = tid; e < n * n; e += 1024) {
-        int i = e / n, c = e - i * n;
-        R1[e] = (c >= i) ? A[e] : 0.0;
-    }
+    if (fail && threadIdx.x == 0 && rank == 0) rqr_set_info(d_info, RQR_INFO_NOT_SPD + fail);
+    if (CL) cluster_sync_all();            // the row buffer lives in R1: all reads done before it is overwritten
+#pragma unroll
+    for (int q = 0; q < CPW; ++q)
+#pragma unroll
+        for (int p = 0; p < RPL; ++p) {
+            const int c = (w + NW * q) * ncta + rank, i = lane + 32 * p;
+            if (c < n && i < n) R1[(int64_t)i * n + c] = (i <= c) ? a[q][p] : 0.0;
+        }
 }
 
 int rqr_chol_dev(const double* G, int n, double shift, const double* d_shift, double* R1,
@@ -274,17 +647,9 @@ int rqr_chol_dev(const double* G, int n, double shift, const double* d_shift, do
     if (n < 2 || n > RQR_MAX_N) return -2;
     if (!R1) return -4;
     if (G == R1) return -4;
-    size_t bytes = (size_t)n * n * sizeof(double);
-    if (bytes <= 200 * 1024) {
-        static bool attr_set = false;
-        if (!attr_set) {
-            cudaFuncSetAttribute(k_chol<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-            attr_set = true;
-        }
-        k_chol<true><<<1, 1024, bytes, st>>>(G, n, shift, d_shift, R1, d_info);
-    } else {
-        k_chol<false><<<1, 1024, 0, st>>>(G, n, shift, d_shift, R1, d_info);
-    }
+    if (n <= 64)       k_chol_small<2, 8, 8><<<1, 256, 0, st>>>(G, n, shift, d_shift, R1, d_info);
+    else if (n <= 128) k_chol_small<4, 8, 16><<<1, 512, 0, st>>>(G, n, shift, d_shift, R1, d_info);
+    else return launch_cluster(k_chol_cols<8, 4, 8, true>, 8, 256, st, G, n, shift, d_shift, R1, d_info);
     RQR_LAUNCH_CHECK();
     return RQR_OK;
 }

@@ -58,17 +58,35 @@ k_trsm_gram_generic(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
     }
 }
 
-// G[a][b] = G[b][a] = sum_p part[p][a][b] (a <= b), p ascending
-__global__ void k_gram_reduce(const double* __restrict__ part, int nparts, int n,
-                              double* __restrict__ G)
+// G[a][b] = G[b][a] = sum_p part[p][a][b] (a <= b).  Fixed order: 4 interleaved groups of partials
+// (p = g, g+4, ...; 8 loads in flight per thread), then the groups in order 0..3 through shared
+// memory.  One CTA per 64 consecutive entries of a row: latency-bound, so wide and shallow.
+__global__ void __launch_bounds__(256)
+k_gram_reduce(const double* __restrict__ part, int nparts, int n, double* __restrict__ G)
 {
-    for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < n * n; e += gridDim.x * blockDim.x) {
-        int a = e / n, b = e - a * n;
-        if (b < a) continue;
-        double s = part[e];
-        for (int p = 1; p < nparts; ++p) s += part[(int64_t)p * n * n + e];
-        G[a * n + b] = s;
-        G[b * n + a] = s;
+    __shared__ double sg[4][64];
+    const int a = blockIdx.y, b = blockIdx.x * 64 + (threadIdx.x & 63), g = threadIdx.x >> 6;
+    double s = 0.0;
+    if (b < n && b >= a) {
+        const double* src = part + (int64_t)a * n + b;
+        const int64_t nn = (int64_t)n * n;
+        int p = g;
+        for (; p + 28 < nparts; p += 32) {
+            double x[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) x[u] = __ldcg(src + (int64_t)(p + 4 * u) * nn);
+#pragma unroll
+            for (int u = 0; u < 8; ++u) s += x[u];
+        }
+        for (; p < nparts; p += 4) s += __ldcg(src + (int64_t)p * nn);
+    }
+    sg[g][threadIdx.x & 63] = s;
+    __syncthreads();
+    if (g == 0 && b < n && b >= a) {
+        const int l = threadIdx.x;
+        const double t = ((sg[0][l] + sg[1][l]) + sg[2][l]) + sg[3][l];
+        G[(int64_t)a * n + b] = t;
+        G[(int64_t)b * n + a] = t;
     }
 }
 
@@ -147,8 +165,8 @@ extern "C" int rqr_trsm_gram(const double* V, int64_t m, int n, int64_t ldv, con
         k_trsm_gram_generic<<<nparts, 256, smem, st>>>(V, m, n, ldv, R0, V1, ldq, part);
         RQR_LAUNCH_CHECK();
     } else if (rc != RQR_OK) return rc;
-    int rb = (n * n + 255) / 256;
-    k_gram_reduce<<<rb, 256, 0, st>>>(part, nparts, n, G);
+    dim3 rgrid((n + 63) / 64, n);
+    k_gram_reduce<<<rgrid, 256, 0, st>>>(part, nparts, n, G);
     RQR_LAUNCH_CHECK();
     return RQR_OK;
 }
