@@ -26,13 +26,18 @@
 // ------------------------------------------------------------------------------------------
 // A4: V1 = V R0^-1 (optional), store V1 (optional), partial Gram per CTA.
 // ------------------------------------------------------------------------------------------
+// warps per CTA of A4: bounded by registers (NB = 8: 248 per thread => 8 warps); the narrower
+// shapes have small Gram tiles and little work per row-block, so they run more warps to hide the
+// per-row-block latencies (mbarrier wait, chain start).  Measured at 2^22 x 32: 0.48 -> 0.37 ms.
+template <int NB> struct GramWarps { static constexpr int value = NB >= 8 ? 8 : (NB >= 4 ? 16 : 24); };
+
 template <int NB, bool HAS_R, bool FULL>
-__global__ void __launch_bounds__(GRAM_WARPS * 32, 1)
+__global__ void __launch_bounds__(GramWarps<NB>::value * 32, 1)
 k_trsm_gram_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
                 const double* __restrict__ R0, double* __restrict__ V1, int64_t ldq,
                 double* __restrict__ part)
 {
-    using Plan = SmemPlan<NB, GRAM_WARPS, GRAM_STAGES, 1, 2>;
+    using Plan = SmemPlan<NB, GramWarps<NB>::value, GRAM_STAGES, 1, 2>;
     constexpr int LDL = Plan::LDL, N8 = Plan::N8;
     constexpr int NBLK = TallCfg<NB>::NBLK;
     extern __shared__ __align__(16) double smem[];
@@ -45,7 +50,7 @@ k_trsm_gram_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
     double* xs = smem + Plan::xs + (size_t)warp * 2 * 8 * N8;
 
     for (int i = threadIdx.x; i < (int)Plan::ring_doubles; i += blockDim.x) ring[i] = 0.0;
-    if (threadIdx.x < GRAM_WARPS * GRAM_STAGES) mbar_init(bars + threadIdx.x, 1);
+    if (threadIdx.x < GramWarps<NB>::value * GRAM_STAGES) mbar_init(bars + threadIdx.x, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     fence_proxy_async();
     __syncthreads();
@@ -54,8 +59,8 @@ k_trsm_gram_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
     WarpRing<LDL> wr{ring + (size_t)warp * GRAM_STAGES * 8 * LDL, bars + warp * GRAM_STAGES, V, ldv, m, n};
     const XsAddr<N8> ad(lane);
     const int64_t nrb = (m + 7) / 8;
-    const int64_t gw = (int64_t)blockIdx.x * GRAM_WARPS + warp;
-    const int64_t stride = (int64_t)gridDim.x * GRAM_WARPS;
+    const int64_t gw = (int64_t)blockIdx.x * GramWarps<NB>::value + warp;
+    const int64_t stride = (int64_t)gridDim.x * GramWarps<NB>::value;
 #pragma unroll
     for (int s = 0; s < GRAM_STAGES; ++s)
         if (gw + s * stride < nrb) wr.issue(s, gw + s * stride, lane);
@@ -123,7 +128,7 @@ k_trsm_gram_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
         const int b = e >> 6, l = (e >> 1) & 31, k = e & 1;
         double s = red[(size_t)b * 64 + 2 * l + k];
 #pragma unroll
-        for (int w = 1; w < GRAM_WARPS; ++w) s += red[((size_t)w * NBLK + b) * 64 + 2 * l + k];
+        for (int w = 1; w < GramWarps<NB>::value; ++w) s += red[((size_t)w * NBLK + b) * 64 + 2 * l + k];
         int a = 0, rem = b;
         while (rem >= NB - a) { rem -= NB - a; ++a; }
         const int bb = a + rem;
@@ -229,7 +234,7 @@ template <int NB>
 static int launch_trsm_gram(const double* V, int64_t m, int n, int64_t ldv, const double* R0, double* V1,
                             int64_t ldq, double* part, int* nparts, cudaStream_t st)
 {
-    using Plan = SmemPlan<NB, GRAM_WARPS, GRAM_STAGES, 1, 2>;
+    using Plan = SmemPlan<NB, GramWarps<NB>::value, GRAM_STAGES, 1, 2>;
     static_assert(Plan::bytes <= 227 * 1024, "A4 shared memory plan too large");
     static bool attr = false;
     if (!attr) {
@@ -238,11 +243,11 @@ static int launch_trsm_gram(const double* V, int64_t m, int n, int64_t ldv, cons
         cudaFuncSetAttribute(k_trsm_gram_mma<NB, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
         attr = true;
     }
-    const int grid = grid_for(m, GRAM_WARPS);
+    const int grid = grid_for(m, GramWarps<NB>::value);
     *nparts = grid;
-    if (R0 && n == 8 * NB) k_trsm_gram_mma<NB, true, true><<<grid, GRAM_WARPS * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, V1, ldq, part);
-    else if (R0)           k_trsm_gram_mma<NB, true, false><<<grid, GRAM_WARPS * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, V1, ldq, part);
-    else                   k_trsm_gram_mma<NB, false, false><<<grid, GRAM_WARPS * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, nullptr, ldq, part);
+    if (R0 && n == 8 * NB) k_trsm_gram_mma<NB, true, true><<<grid, GramWarps<NB>::value * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, V1, ldq, part);
+    else if (R0)           k_trsm_gram_mma<NB, true, false><<<grid, GramWarps<NB>::value * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, V1, ldq, part);
+    else                   k_trsm_gram_mma<NB, false, false><<<grid, GramWarps<NB>::value * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, nullptr, ldq, part);
     RQR_LAUNCH_CHECK();
     return RQR_OK;
 }

@@ -104,3 +104,25 @@ def make_upper(n: int, seed: int, cond_decades: float = 0.0, device="cpu") -> to
     d = (1.0 + torch.rand(n, generator=gen, dtype=torch.float64, device=device)) * torch.pow(
         torch.tensor(10.0, dtype=torch.float64, device=device), -j * cond_decades / max(n - 1, 1))
     return (r + torch.diag(d)).contiguous()
+
+
+def make_V_reflectors(m: int, n: int, kappa: float, seed: int, device="cpu", k: int = 4) -> torch.Tensor:
+    """Same recipe with a cheaper orthonormal U for the largest sweep points (2^24, 2^25 rows), where a
+    library QR of an m x n Gaussian needs more workspace than the matrix: U = H_1 ... H_k [I_n; 0] with k
+    random Householder reflectors (Gaussian vectors), orthonormal to rounding by construction
+    ("Haar-like"); W Haar as in make_V.  O(k m n) work, in place."""
+    gen = torch.Generator(device=device)
+    gen.manual_seed(int(seed))
+    U = torch.zeros(m, n, dtype=torch.float64, device=device)
+    U[:n] = torch.eye(n, dtype=torch.float64, device=device)
+    for _ in range(k):
+        v = torch.randn(m, generator=gen, dtype=torch.float64, device=device)
+        v /= torch.linalg.norm(v)
+        w = v @ U                                   # n
+        U.addr_(v, w, alpha=-2.0)                   # U -= 2 v (v^T U)
+    W = _haar(n, n, gen, device)
+    sig = singular_values(n, kappa, device)
+    U *= sig
+    V = U @ W.T
+    del U
+    return V.contiguous()
