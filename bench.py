@@ -96,6 +96,19 @@ class ClockSampler(threading.Thread):
         return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons)}
 
 
+def launches_per_step(n):
+    """Kernels of ours launched by one rqr_rand_cholqr with a prepared sketch (sorted variant, stored V1):
+    countsketch 1, Gaussian GEMM + reduce 2, Householder 1, A4 2 (n <= 64: fused kernel + partial reduce) or
+    4 (n > 64: fragment build, panel substitution, syrk, reduce), Cholesky 1, A6 1 (n > 64: + fragment build),
+    triangular product 1."""
+    return 9 if n <= 64 else 12
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+# ncu --set full captures (profiles/): workload -> bytes
+NCU_TRAFFIC = {"C2": 536.9e6 + 493.3e6}
+
+
 def measured_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -106,6 +119,9 @@ def measured_peaks():
 
 
 # ------------------------------------------------------------------------------------------
+ORACLE_SAMPLE_ROWS = 1 << 22      # bounds the CPU leg: ~2 s of oracle work per call at n = 64 on 16 cores
+
+
 def oracle_sample(V_host, n, seed, threads_hint=None):
     """Times the CPU oracle, as it stands, on a bounded sample (the first rows) of the workload."""
     from oracle import rqr_oracle as orc
@@ -118,8 +134,8 @@ def oracle_sample(V_host, n, seed, threads_hint=None):
     dt = time.perf_counter() - t0
     fl = flops.rand_cholqr_flops(ms, n, s1, s2)
     return {"value": fl / dt / 1e9, "unit": "GFLOP/s", "cores": orc.num_threads(), "kind": "oracle",
-            "sample": "first %d of the workload's rows x %d cols, s1=%d s2=%d, %.2f s wall, info=%d"
-                      % (ms, n, s1, s2, dt, info)}, dt
+            "sample": "one whole factorization of the first %d rows of the workload (x %d cols, s1=%d s2=%d), "
+                      "%.2f s wall, info=%d" % (ms, n, s1, s2, dt, info)}, dt
 
 
 def run_reference(args):
@@ -130,7 +146,7 @@ def run_reference(args):
     from paper_2309_05868_b200 import inputs
     c = inputs.config(args.workload)
     n = c["n"]
-    ms = min(c["m"], 1 << 17)
+    ms = min(c["m"], ORACLE_SAMPLE_ROWS)
     V = inputs.make_V(ms, n, c["kappa"], c["seed"]).numpy()
     for _ in range(args.warmup if args.warmup < 2 else 1):
         oracle_sample(V, n, args.seed)
@@ -261,7 +277,7 @@ def run_config(torch, rq, name, args, peaks, p64, want_e2e=True, want_breakdown=
         out["e2e"] = {"value": F / ms_e / 1e6, "unit": "GFLOP/s", "ms_per_step": ms_e,
                       "h2d_bytes_per_step": int(8 * m * n), "d2h_bytes_per_step": int(8 * m * n + 8 * n * n)}
         del Vh, Qh, Vin
-    out["_V_host_sample"] = Vd[: min(m, 1 << 17)].cpu().numpy() if not args.no_cpu_baseline else None
+    out["_V_host_sample"] = Vd[: min(m, ORACLE_SAMPLE_ROWS)].cpu().numpy() if not args.no_cpu_baseline else None
     del Vd, Q, bufs
     torch.cuda.empty_cache()
     return out, F
@@ -311,7 +327,10 @@ def main():
     if dom == "trsm_gram" and flops.trsm_gram_flops(m, n) / (p64 * 1e12) > sb[dom] / (peaks["hbm_gbs"] * 1e9):
         ach = flops.trsm_gram_flops(m, n) / (bd[dom] * 1e-3) / 1e12
         roof = {"kernel": "rqr_trsm_gram", "bound": "tensor", "achieved": ach, "peak": p64, "unit": "TFLOP/s",
-                "frac": ach / p64, "traffic": None,
+                "frac": ach / p64, "traffic": NCU_TRAFFIC.get(args.workload),
+                "traffic_source": "profiles/r1_baseline_summary.md (ncu --set full, per launch)",
+                "algorithmic": "2 m n^2 flops per launch (n^2 substitution + n^2 symmetric Gram per row); "
+                               "16 m n bytes (read V, write V1)",
                 "peak_source": "FP64 probe measured live in this run (max of DFMA %.1f / DMMA %.1f TFLOP/s); "
                                "MEASURED_PEAKS.json has no FP64 figure; bf16 x nominal ratio would give %.1f"
                                % (p64s["dfma"], p64s["dmma"], ratio_peak)}
@@ -337,7 +356,7 @@ def main():
             "cholqr2_ms": main_out["cholqr2_ms"], "cholqr2_info": main_out["cholqr2_info"],
             "sketch_gen_ms": main_out["sketch_gen_ms"], "breakdown_ms": bd,
             "fp64_peak_tflops": p64s, "e2e": main_out.get("e2e"),
-            "gpu_launches": 9 * args.steps, "roofline": roof, "cpu_baseline": cpu,
+            "gpu_launches": launches_per_step(n) * args.steps, "roofline": roof, "cpu_baseline": cpu,
             "clocks": sampler.summary(), "extra": extra}
     print(json.dumps(line))
 
@@ -378,7 +397,7 @@ def run_sharded(torch, rq, args, world, rank):
                 "config": {"workload": args.workload, "m_per_gpu": m, "m_total": m_total, "n": n, "s1": s1, "s2": s2,
                            "parallelism": "row-sharded, 2 all-reduces (W, G) per step",
                            "l2": "inputs_exceed_L2"},
-                "gpu_launches": 9 * args.steps, "info": int(bufs["info"].item())}
+                "gpu_launches": launches_per_step(n) * args.steps, "info": int(bufs["info"].item())}
         print(json.dumps(line))
 
 
