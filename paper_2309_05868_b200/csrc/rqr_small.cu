@@ -125,17 +125,93 @@ __device__ __forceinline__ double group8_sum(double x)
     return x;
 }
 
-#define RQR_SWITCH16(P_, STMT)                                                                     \
-    switch (P_) {                                                                                  \
-        case 0: { constexpr int P = 0; STMT } break;   case 1: { constexpr int P = 1; STMT } break;   \
-        case 2: { constexpr int P = 2; STMT } break;   case 3: { constexpr int P = 3; STMT } break;   \
-        case 4: { constexpr int P = 4; STMT } break;   case 5: { constexpr int P = 5; STMT } break;   \
-        case 6: { constexpr int P = 6; STMT } break;   case 7: { constexpr int P = 7; STMT } break;   \
-        case 8: { constexpr int P = 8; STMT } break;   case 9: { constexpr int P = 9; STMT } break;   \
-        case 10: { constexpr int P = 10; STMT } break; case 11: { constexpr int P = 11; STMT } break; \
-        case 12: { constexpr int P = 12; STMT } break; case 13: { constexpr int P = 13; STMT } break; \
-        case 14: { constexpr int P = 14; STMT } break; default: { constexpr int P = 15; STMT } break; \
+// One Householder step of k_geqrf_g8 with the row-slot index of the pivot, P = j / 8, known at
+// compile time: slots p < P hold finished (zeroed) rows and are skipped, the pivot element is
+// col[P] of lane t == j % 8 without a select, and the owner warp is w == P.
+template <int P>
+__device__ __forceinline__ void geqrf_g8_step(double (&a)[2][16], int j, int n, int w, int lane,
+                                              double (*vbuf)[128], double* den_s, double* sgn_s,
+                                              double* __restrict__ R0, int* d_info)
+{
+    const int g = lane >> 3, t = lane & 7, tj = j & 7;
+    if (w == P) {                                          // warp-uniform: the warp that owns column j
+        auto reflect = [&](double (&col)[16]) {
+            double s0 = 0.0, s1 = 0.0;
+#pragma unroll
+            for (int p = P; p < 16; p += 2) {
+                s0 = fma(col[p], col[p], s0);
+                if (p + 1 < 16) s1 = fma(col[p + 1], col[p + 1], s1);
+            }
+            const double ss = group8_sum(s0 + s1);                                   // ||a[j:, j]||^2
+            const double x1 = __shfl_sync(0xffffffffu, col[P], (lane & 24) | tj);    // a[j][j]
+            const double nrm = sqrt(ss);
+            const double sgn = (x1 < 0.0) ? -1.0 : 1.0;
+            const double vj = x1 + sgn * nrm;
+            if (g == (j & 3)) {
+#pragma unroll
+                for (int p = P; p < 16; ++p) vbuf[j & 1][t + 8 * p] = col[p];        // rows < j are zero
+                if (t == tj) vbuf[j & 1][j] = vj;
+                if (t == 0) {
+                    den_s[j & 1] = nrm * fabs(vj);                                   // v^T v / 2
+                    sgn_s[j & 1] = sgn;
+                    R0[(int64_t)j * n + j] = nrm;               // -sgn*nrm, row negated when sgn > 0 (S4)
+                    if (!(nrm > 0.0) || !(nrm < 1.0e308)) rqr_set_info(d_info, RQR_INFO_SINGULAR + j + 1);
+                }
+#pragma unroll
+                for (int p = P; p < 16; ++p) col[p] = 0.0;                           // column j is done
+            }
+        };
+        if ((j >> 2) & 1) reflect(a[1]); else reflect(a[0]);
     }
+    __syncthreads();
+    double v[16];
+#pragma unroll
+    for (int p = P; p < 16; ++p) v[p] = vbuf[j & 1][t + 8 * p];
+    const double den = den_s[j & 1], sg = sgn_s[j & 1];
+    const double beta = (den > 0.0) ? 1.0 / den : 0.0;
+    double dot[2];
+#pragma unroll
+    for (int qq = 0; qq < 2; ++qq) {
+        double s0 = 0.0, s1 = 0.0;
+#pragma unroll
+        for (int p = P; p < 16; p += 2) {
+            s0 = fma(v[p], a[qq][p], s0);
+            if (p + 1 < 16) s1 = fma(v[p + 1], a[qq][p + 1], s1);
+        }
+        dot[qq] = s0 + s1;
+    }
+#pragma unroll
+    for (int o = 1; o < 8; o <<= 1) {
+        dot[0] += __shfl_xor_sync(0xffffffffu, dot[0], o);
+        dot[1] += __shfl_xor_sync(0xffffffffu, dot[1], o);
+    }
+#pragma unroll
+    for (int qq = 0; qq < 2; ++qq) {
+        const double ws = beta * dot[qq];            // finished and padding columns are all zero: ws = 0
+#pragma unroll
+        for (int p = P; p < 16; ++p) a[qq][p] = fma(-ws, v[p], a[qq][p]);
+    }
+    if (t == tj) {                                   // row j is final: move it out of the tile
+#pragma unroll
+        for (int qq = 0; qq < 2; ++qq) {
+            const int c = 8 * w + 4 * qq + g;
+            const double val = a[qq][P];
+            a[qq][P] = 0.0;
+            if (c > j && c < n) R0[(int64_t)j * n + c] = (sg > 0.0) ? -val : val;
+        }
+    }
+}
+
+template <int P>
+__device__ __forceinline__ void geqrf_g8_steps(double (&a)[2][16], int n, int w, int lane, double (*vbuf)[128],
+                                               double* den_s, double* sgn_s, double* __restrict__ R0, int* d_info)
+{
+    if constexpr (P < 8) {
+        const int jend = (8 * P + 8 < n) ? 8 * P + 8 : n;
+        for (int j = 8 * P; j < jend; ++j) geqrf_g8_step<P>(a, j, n, w, lane, vbuf, den_s, sgn_s, R0, d_info);
+        if (8 * P + 8 < n) geqrf_g8_steps<P + 1>(a, n, w, lane, vbuf, den_s, sgn_s, R0, d_info);
+    }
+}
 
 __global__ void __launch_bounds__(256, 1)
 k_geqrf_g8(const double* __restrict__ W, int s2, int n, double* __restrict__ R0, int* d_info)
@@ -156,71 +232,7 @@ k_geqrf_g8(const double* __restrict__ W, int s2, int n, double* __restrict__ R0,
         const int i = e / n, c = e - i * n;
         if (c < i) R0[e] = 0.0;
     }
-    for (int j = 0; j < n; ++j) {
-        const int pj = j >> 3, tj = j & 7;
-        if (w == pj) {                                     // warp-uniform: the warp that owns column j
-            auto reflect = [&](double (&col)[16]) {
-                double s0 = 0.0, s1 = 0.0, xe = 0.0;
-#pragma unroll
-                for (int p = 0; p < 16; p += 2) { s0 = fma(col[p], col[p], s0); s1 = fma(col[p + 1], col[p + 1], s1); }
-                RQR_SWITCH16(pj, xe = col[P];)
-                const double ss = group8_sum(s0 + s1);                              // ||a[j:, j]||^2
-                const double x1 = __shfl_sync(0xffffffffu, xe, (lane & 24) | tj);   // a[j][j]
-                const double nrm = sqrt(ss);
-                const double sgn = (x1 < 0.0) ? -1.0 : 1.0;
-                const double vj = x1 + sgn * nrm;
-                if (g == (j & 3)) {
-#pragma unroll
-                    for (int p = 0; p < 16; ++p) vbuf[j & 1][t + 8 * p] = col[p];    // rows < j are zero
-                    if (t == tj) vbuf[j & 1][j] = vj;
-                    if (t == 0) {
-                        den_s[j & 1] = nrm * fabs(vj);                               // v^T v / 2
-                        sgn_s[j & 1] = sgn;
-                        R0[(int64_t)j * n + j] = nrm;           // -sgn*nrm, row negated when sgn > 0 (S4)
-                        if (!(nrm > 0.0) || !(nrm < 1.0e308)) rqr_set_info(d_info, RQR_INFO_SINGULAR + j + 1);
-                    }
-#pragma unroll
-                    for (int p = 0; p < 16; ++p) col[p] = 0.0;                       // column j is done
-                }
-            };
-            if ((j >> 2) & 1) reflect(a[1]); else reflect(a[0]);
-        }
-        __syncthreads();
-        double v[16];
-#pragma unroll
-        for (int p = 0; p < 16; ++p) v[p] = vbuf[j & 1][t + 8 * p];
-        const double den = den_s[j & 1], sg = sgn_s[j & 1];
-        const double beta = (den > 0.0) ? 1.0 / den : 0.0;
-        double dot[2];
-#pragma unroll
-        for (int qq = 0; qq < 2; ++qq) {
-            double s0 = 0.0, s1 = 0.0;
-#pragma unroll
-            for (int p = 0; p < 16; p += 2) { s0 = fma(v[p], a[qq][p], s0); s1 = fma(v[p + 1], a[qq][p + 1], s1); }
-            dot[qq] = s0 + s1;
-        }
-#pragma unroll
-        for (int o = 1; o < 8; o <<= 1) {
-            dot[0] += __shfl_xor_sync(0xffffffffu, dot[0], o);
-            dot[1] += __shfl_xor_sync(0xffffffffu, dot[1], o);
-        }
-#pragma unroll
-        for (int qq = 0; qq < 2; ++qq) {
-            const double ws = beta * dot[qq];            // finished and padding columns are all zero: ws = 0
-#pragma unroll
-            for (int p = 0; p < 16; ++p) a[qq][p] = fma(-ws, v[p], a[qq][p]);
-        }
-        if (t == tj) {                                   // row j is final: move it out of the tile
-            RQR_SWITCH16(pj,
-                _Pragma("unroll")
-                for (int qq = 0; qq < 2; ++qq) {
-                    const int c = 8 * w + 4 * qq + g;
-                    const double val = a[qq][P];
-                    a[qq][P] = 0.0;
-                    if (c > j && c < n) R0[(int64_t)j * n + c] = (sg > 0.0) ? -val : val;
-                })
-        }
-    }
+    geqrf_g8_steps<0>(a, n, w, lane, vbuf, den_s, sgn_s, R0, d_info);
 }
 
 // Generic fallback, any 2 <= n <= 256, s2 <= 512: W stays in global memory (L2-resident) and is
