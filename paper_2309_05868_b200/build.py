@@ -7,7 +7,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "librqr.so")
-SOURCES = ["rqr_sketch.cu", "rqr_small.cu", "rqr_tall.cu", "rqr_tall_mma.cu", "rqr_tall_panel.cu", "rqr_api.cu", "rqr_probe.cu"]
+SOURCES = ["rqr_sketch.cu", "rqr_gauss_mma.cu", "rqr_small.cu", "rqr_tall.cu", "rqr_tall_mma.cu", "rqr_tall_panel.cu", "rqr_api.cu", "rqr_probe.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 

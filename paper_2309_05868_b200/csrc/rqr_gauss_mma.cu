@@ -1,0 +1,136 @@
+// rqr_gauss_mma.cu -- A2 for n >= 128: W = S2 W1 as a split-K FP64 DMMA GEMM.
+// At n = 256 this step is 34 GFLOP over 0.8 GB (C4): FP64-bound, 8% of the path's flops.
+// CTA (y = 64-row tile of S2, z = K chunk): 8 consumer warps, warp w owns rows 8w..8w+7 of the tile and
+// all n columns (NBN accumulator blocks in registers); a producer warp stages 16-deep K slices of the S2
+// tile (64 x 16) and of W1 (16 x n) with per-row bulk async copies into padded rows (strides 20 and
+// n+4 doubles: the A- and B-fragment reads are bank-conflict free); 4 stages, full/empty mbarriers.
+// Partials go to the caller's buffer and are reduced in fixed order by k_reduce_partials.
+#include "rqr_mma.cuh"
+
+#define GM_KB 16
+#define GM_STAGES 4
+#define GM_WARPS 8
+
+__device__ __forceinline__ void gm_arrive(uint64_t* bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(smem_u32(bar)) : "memory");
+}
+
+template <int NBN>
+struct GaussPlan {
+    static constexpr int LDA = GM_KB + 4, LDB = 8 * NBN + 4;
+    static constexpr size_t a_doubles = 64 * LDA, b_doubles = (size_t)GM_KB * LDB;
+    static constexpr size_t stage = a_doubles + b_doubles;
+    static constexpr size_t bars = GM_STAGES * stage;
+    static constexpr size_t bytes = (bars + 2 * GM_STAGES) * sizeof(double);
+};
+
+template <int NBN>
+__global__ void __launch_bounds__((GM_WARPS + 1) * 32, 1)
+k_gauss_gemm_mma(const double* __restrict__ S2, const double* __restrict__ W1, int64_t s1, int n, int s2,
+                 int64_t kchunk, double* __restrict__ part)
+{
+    using Plan = GaussPlan<NBN>;
+    constexpr int LDA = Plan::LDA, LDB = Plan::LDB;
+    extern __shared__ __align__(16) double smem[];
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem + Plan::bars);
+    uint64_t* empty = full + GM_STAGES;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int i = threadIdx.x; i < (int)Plan::bars; i += blockDim.x) smem[i] = 0.0;
+    if (threadIdx.x < GM_STAGES) mbar_init(full + threadIdx.x, 1);
+    else if (threadIdx.x < 2 * GM_STAGES) mbar_init(empty + (threadIdx.x - GM_STAGES), GM_WARPS);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    fence_proxy_async();
+    __syncthreads();
+
+    const int m0 = blockIdx.y * 64;
+    const int64_t k0 = (int64_t)blockIdx.z * kchunk;
+    const int64_t k1 = (k0 + kchunk < s1) ? k0 + kchunk : s1;
+    const int nsteps = (int)((k1 - k0) / GM_KB);
+    const int rows_a = (s2 - m0) < 64 ? (s2 - m0) : 64;
+
+    if (warp == GM_WARPS) {
+        int stage = 0;
+        uint32_t ph = 0;
+        for (int s = 0; s < nsteps; ++s) {
+            const int64_t k = k0 + (int64_t)s * GM_KB;
+            double* A = smem + (size_t)stage * Plan::stage;
+            double* B = A + Plan::a_doubles;
+            mbar_wait(empty + stage, ph ^ 1u);
+            if (lane == 0) mbar_expect_tx(full + stage, (uint32_t)(rows_a * GM_KB * 8 + GM_KB * n * 8));
+            __syncwarp();
+            for (int r = lane; r < rows_a; r += 32)
+                bulk_g2s(A + r * LDA, S2 + (int64_t)(m0 + r) * s1 + k, GM_KB * 8, full + stage);
+            if (lane < GM_KB) bulk_g2s(B + lane * LDB, W1 + (k + lane) * n, (uint32_t)(n * 8), full + stage);
+            if (++stage == GM_STAGES) { stage = 0; ph ^= 1u; }
+        }
+        return;
+    }
+    const int r = lane >> 2, q = lane & 3;
+    double acc[NBN][2];
+#pragma unroll
+    for (int b = 0; b < NBN; ++b) { acc[b][0] = 0.0; acc[b][1] = 0.0; }
+    int stage = 0;
+    uint32_t ph = 0;
+    for (int s = 0; s < nsteps; ++s) {
+        const double* A = smem + (size_t)stage * Plan::stage + (8 * warp + r) * LDA + q;
+        const double* B = smem + (size_t)stage * Plan::stage + Plan::a_doubles + q * LDB + r;
+        mbar_wait(full + stage, ph);
+#pragma unroll
+        for (int kk = 0; kk < GM_KB; kk += 4) {
+            const double a = A[kk];
+#pragma unroll
+            for (int b = 0; b < NBN; ++b) dmma(acc[b][0], acc[b][1], a, B[kk * LDB + 8 * b]);
+        }
+        __syncwarp();
+        if (lane == 0) gm_arrive(empty + stage);
+        if (++stage == GM_STAGES) { stage = 0; ph ^= 1u; }
+    }
+    double* P = part + (int64_t)blockIdx.z * s2 * n;
+    const int row = m0 + 8 * warp + r;
+    if (row < s2) {
+#pragma unroll
+        for (int b = 0; b < NBN; ++b) {
+            const int col = 8 * b + 2 * q;
+            if (col < n) P[(int64_t)row * n + col] = acc[b][0];
+            if (col + 1 < n) P[(int64_t)row * n + col + 1] = acc[b][1];
+        }
+    }
+}
+
+template <int NBN>
+static int launch_gauss_mma(const double* S2, const double* W1, int64_t s1, int n, int s2, double* part,
+                            int64_t ks_cap, int* ks_out, cudaStream_t st)
+{
+    using Plan = GaussPlan<NBN>;
+    static_assert(Plan::bytes <= 227 * 1024, "k_gauss_gemm_mma shared memory plan too large");
+    static bool attr = false;
+    if (!attr) {
+        cudaFuncSetAttribute(k_gauss_gemm_mma<NBN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
+        attr = true;
+    }
+    const int tiles_m = (s2 + 63) / 64;
+    int64_t ks = 296 / tiles_m;
+    if (ks > ks_cap) ks = ks_cap;
+    const int64_t kblocks = s1 / GM_KB;
+    if (ks > kblocks) ks = kblocks;
+    if (ks < 1) ks = 1;
+    const int64_t kchunk = ((kblocks + ks - 1) / ks) * GM_KB;
+    ks = (s1 + kchunk - 1) / kchunk;
+    dim3 grid(1, tiles_m, (unsigned)ks);
+    k_gauss_gemm_mma<NBN><<<grid, (GM_WARPS + 1) * 32, Plan::bytes, st>>>(S2, W1, s1, n, s2, kchunk, part);
+    RQR_LAUNCH_CHECK();
+    *ks_out = (int)ks;
+    return RQR_OK;
+}
+
+// returns RQR_TALL_NOT_HANDLED when the shape is left to the DFMA kernel
+int rqr_gauss_gemm_mma(const double* S2, const double* W1, int64_t s1, int n, int s2, double* part,
+                       int64_t ks_cap, int* ks_out, cudaStream_t st)
+{
+    if (n < 96 || n > 256 || (n & 1) || (s1 % GM_KB) != 0) return RQR_TALL_NOT_HANDLED;
+    if ((((uintptr_t)S2 | (uintptr_t)W1) & 15) != 0) return RQR_TALL_NOT_HANDLED;
+    if (n <= 128) return launch_gauss_mma<16>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st);
+    if (n <= 192) return launch_gauss_mma<24>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st);
+    return launch_gauss_mma<32>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st);
+}

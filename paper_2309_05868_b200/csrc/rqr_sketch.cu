@@ -2,6 +2,10 @@
 // single dense Gaussian sketch comparator.  See include/rqr.h for the contracts and DESIGN.md
 // for the kernel designs.  sm_100a.
 #include "rqr_common.cuh"
+#include "rqr_tall.cuh"
+
+int rqr_gauss_gemm_mma(const double* S2, const double* W1, int64_t s1, int n, int s2, double* part,
+                       int64_t ks_cap, int* ks_out, cudaStream_t st);
 
 // =========================================================================================
 // A0: sketch generation (off the paper's clock)
@@ -441,9 +445,20 @@ extern "C" int rqr_gauss_sketch(const double* W1, int64_t s1, int n, int s2, uin
         int rc = launch_prepare_S2(s1, s2, seed, S2, st);
         if (rc != RQR_OK) return rc;
     }
+    int64_t ks_cap = RQR_GAUSS_PARTIAL_ROWS / s2;
+    int64_t elems = (int64_t)s2 * n;
+    {
+        int ks_mma = 0;                           // n >= 128: FP64 DMMA GEMM (rqr_gauss_mma.cu)
+        int rc = rqr_gauss_gemm_mma(S2, W1, s1, n, s2, part, ks_cap, &ks_mma, st);
+        if (rc == RQR_OK) {
+            k_reduce_partials<<<(int)((elems + 63) / 64), 256, 0, st>>>(part, ks_mma, elems, W);
+            RQR_LAUNCH_CHECK();
+            return RQR_OK;
+        }
+        if (rc != RQR_TALL_NOT_HANDLED) return rc;
+    }
     int tiles_m = (s2 + GS_BM - 1) / GS_BM, tiles_n = (n + GS_BN - 1) / GS_BN;
     int64_t ks = 296 / (tiles_m * tiles_n);
-    int64_t ks_cap = RQR_GAUSS_PARTIAL_ROWS / s2;
     if (ks > ks_cap) ks = ks_cap;
     int64_t kblocks = (s1 + GS_BK - 1) / GS_BK;
     if (ks > kblocks) ks = kblocks;
@@ -453,7 +468,6 @@ extern "C" int rqr_gauss_sketch(const double* W1, int64_t s1, int n, int s2, uin
     dim3 grid(tiles_n, tiles_m, (unsigned)ks);
     k_gauss_gemm_splitk<<<grid, 256, 0, st>>>(S2, W1, s1, n, s2, kchunk, part);
     RQR_LAUNCH_CHECK();
-    int64_t elems = (int64_t)s2 * n;
     k_reduce_partials<<<(int)((elems + 63) / 64), 256, 0, st>>>(part, (int)ks, elems, W);
     RQR_LAUNCH_CHECK();
     return RQR_OK;

@@ -84,7 +84,7 @@ def run_point(m, n, reps, p64, hbm):
         "scholqr3": (6.0 * m * n * n, 48.0 * m * n, lambda: rq.scholqr3(V, Q, R, work, info)),
     }
     for name, (F, B, fn) in models.items():
-        ms = _time(fn, reps)
+        ms = _time(fn, reps if name != "gauss_rand_cholqr" else max(1, reps // 5))   # the dense sketch is slow
         st = int(info.item())
         t_roof = max(F / (p64 * 1e12), B / (hbm * 1e9))
         orth, res = _checks(V, Q, R) if st == 0 else (None, None)

@@ -89,7 +89,8 @@ def test_countsketch_strided_and_row_offset(rq, orc):
 
 
 @pytest.mark.parametrize("s1,n,s2", [(512, 16, 32), (8192, 64, 128), (9940, 70, 140), (300, 5, 7),
-                                     (4096, 256, 512)])
+                                     (4096, 256, 512), (32768, 128, 256), (9984, 200, 401), (40000, 98, 130),
+                                     (65536, 256, 512)])
 def test_gauss_sketch_parity(rq, orc, s1, n, s2):
     rng = np.random.default_rng(s1 + n)
     W1 = rng.standard_normal((s1, n))
