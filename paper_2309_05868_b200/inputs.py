@@ -108,13 +108,19 @@ def make_upper(n: int, seed: int, cond_decades: float = 0.0, device="cpu") -> to
 
 def make_V_reflectors(m: int, n: int, kappa: float, seed: int, device="cpu", k: int = 4) -> torch.Tensor:
     """Same recipe with a cheaper orthonormal U for the largest sweep points (2^24, 2^25 rows), where a
-    library QR of an m x n Gaussian needs more workspace than the matrix: U = H_1 ... H_k [I_n; 0] with k
-    random Householder reflectors (Gaussian vectors), orthonormal to rounding by construction
-    ("Haar-like"); W Haar as in make_V.  O(k m n) work, in place."""
+    library QR of an m x n Gaussian needs more workspace than the matrix: U = H_1 ... H_k D E with
+    E = sqrt(n/m) [I_n; I_n; ...] (stacked identities: orthonormal columns, all rows of equal norm, like a
+    Haar U), D random signs, and k random Householder reflectors (Gaussian vectors): orthonormal to rounding
+    by construction ("Haar-like"); W Haar as in make_V.  O(k m n) work, in place.
+    m must be a multiple of n."""
+    assert m % n == 0
     gen = torch.Generator(device=device)
     gen.manual_seed(int(seed))
+    sgn = torch.randint(0, 2, (m,), generator=gen, device=device).to(torch.float64) * 2.0 - 1.0
     U = torch.zeros(m, n, dtype=torch.float64, device=device)
-    U[:n] = torch.eye(n, dtype=torch.float64, device=device)
+    idx = torch.arange(m, device=device)
+    U[idx, idx % n] = sgn * (n / m) ** 0.5
+    del idx, sgn
     for _ in range(k):
         v = torch.randn(m, generator=gen, dtype=torch.float64, device=device)
         v /= torch.linalg.norm(v)
