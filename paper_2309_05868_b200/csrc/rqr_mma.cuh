@@ -259,6 +259,40 @@ __device__ __forceinline__ void trsm_rowblock(double (&acc)[NB][2], double* __re
     if constexpr (XS) __syncwarp();
 }
 
+// The same routine (same instruction sequence on acc, Tf, nRf: H1) with the interleaved independent
+// work given as a functor: gf.template chunk<J, PART>() is called at the four gaps of step J.
+template <int NB, bool XS, bool FULL, class Hook, class GF>
+__device__ __forceinline__ void trsm_rowblock_gf(double (&acc)[NB][2], double* __restrict__ xsc,
+                                                 const XsAddr<8 * NB>& ad, const double* __restrict__ Tf,
+                                                 const double* __restrict__ nRf, double* __restrict__ gp,
+                                                 uint32_t colmask, int lane, Hook&& after_first, GF&& gf)
+{
+    static_for<0, NB>([&](auto Jc) {
+        constexpr int J = decltype(Jc)::value;
+        double x0 = 0.0, x1 = 0.0;
+        dmma(x0, x1, acc[J][0], Tf[J * 64 + lane]);
+        gf.template chunk<J, 0>();
+        dmma(x0, x1, acc[J][1], Tf[J * 64 + 32 + lane]);
+        gf.template chunk<J, 1>();
+#pragma unroll
+        for (int Jp = J + 1; Jp < NB; ++Jp)
+            dmma(acc[Jp][0], acc[Jp][1], x0, nRf[TriFrags<NB>::pair(J, Jp) * 64 + lane]);
+        gf.template chunk<J, 2>();
+#pragma unroll
+        for (int Jp = J + 1; Jp < NB; ++Jp)
+            dmma(acc[Jp][0], acc[Jp][1], x1, nRf[TriFrags<NB>::pair(J, Jp) * 64 + 32 + lane]);
+        acc[J][0] = x0; acc[J][1] = x1;
+        if constexpr (J == 0) after_first();
+        gf.template chunk<J, 3>();
+        if constexpr (XS) *reinterpret_cast<double2*>(xsc + ad.c(J)) = make_double2(x0, x1);
+        if (gp != nullptr) {
+            if (FULL || ((colmask >> (2 * J)) & 1u)) *reinterpret_cast<double2*>(gp + 8 * J) = make_double2(x0, x1);
+            else if ((colmask >> (2 * J + 1)) & 1u) gp[8 * J] = x0;
+        }
+    });
+    if constexpr (XS) __syncwarp();
+}
+
 // Per-warp ring of landing row-blocks fed by bulk async copies.
 template <int LD>
 struct WarpRing {

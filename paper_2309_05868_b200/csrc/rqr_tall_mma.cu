@@ -22,6 +22,7 @@
 //     register (lane l holds X[l%4][l/4] of a 4-row slab).
 // The same trsm routine serves rqr_apply, so V1 re-formed there has the same bits (H1).
 #include "rqr_mma.cuh"
+#include <stdlib.h>
 
 // ------------------------------------------------------------------------------------------
 // A4: V1 = V R0^-1 (optional), store V1 (optional), partial Gram per CTA.
@@ -133,6 +134,197 @@ k_trsm_gram_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
         while (rem >= NB - a) { rem -= NB - a; ++a; }
         const int bb = a + rem;
         const int row = 8 * a + (l >> 2), col = 8 * bb + 2 * (l & 3) + k;
+        if (row < n && col < n) P[row * n + col] = s;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// A4, pair version for 32 < n <= 64 (NB = 8).  The single-warp kernel above needs 248 registers
+// (36 Gram accumulators), i.e. 2 warps per SM sub-partition, and loses ~15% of the DMMA pipe to
+// moments when both are stalled.  Here two warps form a PAIR: each runs the substitution chain of its
+// own row-block, both write X into a pair-shared staging block, and each accumulates HALF of the
+// Gram blocks -- fold sets {0,7,1,6} / {2,5,3,4} of block rows, 18 blocks each -- over BOTH row-blocks.
+// Same DMMA count per warp (72 chain + 72 Gram per iteration), half the accumulator registers:
+// 12 warps per SM (3 per sub-partition).  One named barrier per pair and iteration.
+// ------------------------------------------------------------------------------------------
+#define PAIR_WARPS 12
+#define PAIR_STAGES 2
+
+template <int SIDE>
+struct PairSet {
+    __host__ __device__ static constexpr int row(int i)
+    {
+        return SIDE == 0 ? (i == 0 ? 0 : (i == 1 ? 7 : (i == 2 ? 1 : 6))) : (i == 0 ? 2 : (i == 1 ? 5 : (i == 2 ? 3 : 4)));
+    }
+    __host__ __device__ static constexpr int a(int k)
+    {
+        int i = 0;
+        while (k >= 8 - row(i)) { k -= 8 - row(i); ++i; }
+        return row(i);
+    }
+    __host__ __device__ static constexpr int b(int k)
+    {
+        int i = 0;
+        while (k >= 8 - row(i)) { k -= 8 - row(i); ++i; }
+        return row(i) + k;
+    }
+};
+
+// Gram DMMAs [T0, T1) of an iteration: t -> row-block t / 36 of the pair, slab (t % 36) / 18, block t % 18
+template <int SIDE, int T0, int T1>
+__device__ __forceinline__ void pair_gram_chunk(const double* __restrict__ xsp, const XsAddr<64>& ad,
+                                                double (&g)[8], double (&G)[18][2])
+{
+    static_for<T0, T1>([&](auto tc) {
+        constexpr int t = decltype(tc)::value;
+        if constexpr (t % 18 == 0) {
+            constexpr int rbk = t / 36, h = (t % 36) / 18;
+#pragma unroll
+            for (int a_ = (SIDE ? 2 : 0); a_ < 8; ++a_) g[a_] = xsp[rbk * 512 + ad.g(h, a_)];
+        }
+        constexpr int k = t % 18;
+        dmma(G[k][0], G[k][1], g[PairSet<SIDE>::a(k)], g[PairSet<SIDE>::b(k)]);
+    });
+}
+
+template <int SIDE, bool ON>
+struct PairGram {
+    const double* xsp;
+    const XsAddr<64>& ad;
+    double (&g)[8];
+    double (&G)[18][2];
+    template <int J, int PART>
+    __device__ __forceinline__ void chunk()
+    {
+        if constexpr (ON) {
+            constexpr int E[5] = {0, 2, 4, 6, 9};
+            pair_gram_chunk<SIDE, 9 * J + E[PART], 9 * J + E[PART + 1]>(xsp, ad, g, G);
+        }
+    }
+};
+
+struct PairPlan {
+    static constexpr int LDL = 64 + LDL_PAD;
+    static constexpr size_t scratch = TriFrags<8>::DOUBLES;                      // after Tf, nRf
+    static constexpr size_t bars = scratch + 8 * 64;
+    static constexpr size_t xs = bars + PAIR_WARPS * PAIR_STAGES;
+    static constexpr size_t ring = xs + (size_t)(PAIR_WARPS / 2) * 2 * 2 * 512;  // pair x buffer x row-block
+    static constexpr size_t ring_doubles = (size_t)PAIR_WARPS * PAIR_STAGES * 8 * LDL;
+    static constexpr size_t red_doubles = (size_t)PAIR_WARPS * 18 * 64;
+    static constexpr size_t total = (ring + ring_doubles) > red_doubles ? (ring + ring_doubles) : red_doubles;
+    static constexpr size_t bytes = total * sizeof(double);
+};
+
+template <int SIDE, bool FULL>
+__device__ __forceinline__ void pair_body(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
+                                          double* __restrict__ V1, int64_t ldq, double* smem, double (&G)[18][2])
+{
+    constexpr int LDL = PairPlan::LDL;
+    const double* Tf = smem;
+    const double* nRf = smem + 8 * 64;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + PairPlan::bars);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, pair = warp >> 1;
+    double* xs = smem + PairPlan::xs + (size_t)pair * 2 * 2 * 512;
+    WarpRing<LDL> wr{smem + PairPlan::ring + (size_t)warp * PAIR_STAGES * 8 * LDL, bars + warp * PAIR_STAGES, V, ldv, m, n};
+    const XsAddr<64> ad(lane);
+    const int64_t nrb = (m + 7) / 8;
+    const int64_t npairs = (int64_t)gridDim.x * (PAIR_WARPS / 2);
+    const int64_t pg = (int64_t)blockIdx.x * (PAIR_WARPS / 2) + pair;
+#pragma unroll
+    for (int s = 0; s < PAIR_STAGES; ++s) {
+        const int64_t rb = (s * npairs + pg) * 2 + SIDE;
+        if (rb < nrb) wr.issue(s, rb, lane);
+    }
+    double g[8];
+    double acc[8][2];
+    const uint32_t colmask = col_mask<8>(n, lane);
+    const int64_t lane_off = (int64_t)(lane >> 2) * ldq + 2 * (lane & 3);
+    int t = 0, stage = 0;
+    uint32_t phase = 0;
+    for (;; ++t) {
+        const int64_t base = ((int64_t)t * npairs + pg) * 2;
+        if (base >= nrb) break;                              // pair-uniform
+        const int64_t rblk = base + SIDE;
+        const bool active = rblk < nrb;
+        int valid = 0;
+        if (active) {
+            mbar_wait(wr.bar + stage, phase);
+            double* rb = wr.buf + stage * 8 * LDL;
+            valid = (int)((m - rblk * 8) < 8 ? (m - rblk * 8) : 8);
+            if (valid < 8) {
+                for (int e = lane; e < (8 - valid) * LDL; e += 32) rb[valid * LDL + e] = 0.0;
+                __syncwarp();
+            }
+            load_acc<8, LDL>(acc, rb, lane);
+        } else {
+#pragma unroll
+            for (int J = 0; J < 8; ++J) { acc[J][0] = 0.0; acc[J][1] = 0.0; }
+        }
+        auto refill = [&]() {
+            const int64_t next = (((int64_t)t + PAIR_STAGES) * npairs + pg) * 2 + SIDE;
+            if (active && next < nrb) {
+                fence_proxy_async();
+                __syncwarp();
+                wr.issue(stage, next, lane);
+            }
+        };
+        double* xsc = xs + (t & 1) * 1024 + SIDE * 512;
+        const double* xsp = xs + ((t & 1) ^ 1) * 1024;
+        double* gp = (V1 && active && (lane >> 2) < valid) ? V1 + rblk * 8 * ldq + lane_off : nullptr;
+        if (t > 0) {
+            PairGram<SIDE, true> gf{xsp, ad, g, G};
+            trsm_rowblock_gf<8, true, FULL>(acc, xsc, ad, Tf, nRf, gp, colmask, lane, refill, gf);
+        } else {
+            PairGram<SIDE, false> gf{xsp, ad, g, G};
+            trsm_rowblock_gf<8, true, FULL>(acc, xsc, ad, Tf, nRf, gp, colmask, lane, refill, gf);
+        }
+        // both X blocks of this iteration are complete, and the blocks read by this iteration's Gram may be reused
+        asm volatile("bar.sync %0, 64;" :: "r"(1 + pair) : "memory");
+        if (++stage == PAIR_STAGES) { stage = 0; phase ^= 1u; }
+    }
+    if (t > 0) pair_gram_chunk<SIDE, 0, 72>(xs + ((t - 1) & 1) * 1024, ad, g, G);
+}
+
+template <bool FULL>
+__global__ void __launch_bounds__(PAIR_WARPS * 32, 1)
+k_trsm_gram_pair(const double* __restrict__ V, int64_t m, int n, int64_t ldv, const double* __restrict__ R0,
+                 double* __restrict__ V1, int64_t ldq, double* __restrict__ part)
+{
+    extern __shared__ __align__(16) double smem[];
+    double* ring = smem + PairPlan::ring;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + PairPlan::bars);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int i = threadIdx.x; i < (int)PairPlan::ring_doubles; i += blockDim.x) ring[i] = 0.0;
+    if (threadIdx.x < PAIR_WARPS * PAIR_STAGES) mbar_init(bars + threadIdx.x, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    fence_proxy_async();
+    __syncthreads();
+    build_tri_frags<8>(R0, n, smem, smem + 8 * 64, smem + PairPlan::scratch);
+
+    double G[18][2];
+#pragma unroll
+    for (int b = 0; b < 18; ++b) { G[b][0] = 0.0; G[b][1] = 0.0; }
+    if (warp & 1) pair_body<1, FULL>(V, m, n, ldv, V1, ldq, smem, G);
+    else          pair_body<0, FULL>(V, m, n, ldv, V1, ldq, smem, G);
+
+    // fixed-order reduction over the pairs, then this CTA's partial (upper blocks)
+    __syncthreads();
+    double* red = smem;
+#pragma unroll
+    for (int b = 0; b < 18; ++b) {
+        red[((size_t)warp * 18 + b) * 64 + 2 * lane] = G[b][0];
+        red[((size_t)warp * 18 + b) * 64 + 2 * lane + 1] = G[b][1];
+    }
+    __syncthreads();
+    double* P = part + (size_t)blockIdx.x * n * n;
+    for (int e = threadIdx.x; e < 2 * 18 * 64; e += blockDim.x) {
+        const int side = e / (18 * 64), k = (e / 64) % 18, l = (e >> 1) & 31, kk = e & 1;
+        double s = 0.0;
+#pragma unroll
+        for (int p = 0; p < PAIR_WARPS / 2; ++p) s += red[((size_t)(2 * p + side) * 18 + k) * 64 + 2 * l + kk];
+        const int a = side ? PairSet<1>::a(k) : PairSet<0>::a(k);
+        const int bb = side ? PairSet<1>::b(k) : PairSet<0>::b(k);
+        const int row = 8 * a + (l >> 2), col = 8 * bb + 2 * (l & 3) + kk;
         if (row < n && col < n) P[row * n + col] = s;
     }
 }
@@ -252,11 +444,38 @@ static int launch_trsm_gram(const double* V, int64_t m, int n, int64_t ldv, cons
     return RQR_OK;
 }
 
+static int g_a4_pair = -1;       // -1: read RQR_A4_PAIR from the environment once (default on)
+
+static int launch_trsm_gram_pair(const double* V, int64_t m, int n, int64_t ldv, const double* R0, double* V1,
+                                 int64_t ldq, double* part, int* nparts, cudaStream_t st)
+{
+    static_assert(PairPlan::bytes <= 227 * 1024, "A4 pair shared memory plan too large");
+    static bool attr = false;
+    if (!attr) {
+        cudaFuncSetAttribute(k_trsm_gram_pair<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PairPlan::bytes);
+        cudaFuncSetAttribute(k_trsm_gram_pair<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PairPlan::bytes);
+        attr = true;
+    }
+    const int64_t npair_blocks = ((m + 7) / 8 + 1) / 2;
+    int64_t g = (npair_blocks + PAIR_WARPS / 2 - 1) / (PAIR_WARPS / 2);
+    const int grid = (int)(g < 148 ? (g < 1 ? 1 : g) : 148);
+    *nparts = grid;
+    if (n == 64) k_trsm_gram_pair<true><<<grid, PAIR_WARPS * 32, PairPlan::bytes, st>>>(V, m, n, ldv, R0, V1, ldq, part);
+    else         k_trsm_gram_pair<false><<<grid, PAIR_WARPS * 32, PairPlan::bytes, st>>>(V, m, n, ldv, R0, V1, ldq, part);
+    RQR_LAUNCH_CHECK();
+    return RQR_OK;
+}
+
 int rqr_trsm_gram_mma(const double* V, int64_t m, int n, int64_t ldv, const double* R0, double* V1,
                       int64_t ldq, double* part, int* nparts, cudaStream_t st)
 {
     if (!fast_ok(V, n, ldv, V1, ldq)) return RQR_TALL_NOT_HANDLED;
     if (!R0 && V1) return RQR_TALL_NOT_HANDLED;       // plain copy + Gram: generic kernel
+    if (g_a4_pair < 0) {
+        const char* e = getenv("RQR_A4_PAIR");
+        g_a4_pair = (e && e[0] == '0') ? 0 : 1;
+    }
+    if (g_a4_pair && R0 && n > 32) return launch_trsm_gram_pair(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
     if (n <= 16) return launch_trsm_gram<2>(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
     if (n <= 32) return launch_trsm_gram<4>(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
     return launch_trsm_gram<8>(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
