@@ -99,9 +99,9 @@ class ClockSampler(threading.Thread):
 def launches_per_step(n):
     """Kernels of ours launched by one rqr_rand_cholqr with a prepared sketch (sorted variant, stored V1):
     countsketch 1, Gaussian GEMM + reduce 2, Householder 1, A4 2 (n <= 64: fused kernel + partial reduce) or
-    4 (n > 64: fragment build, panel substitution, syrk, reduce), Cholesky 1, A6 1 (n > 64: + fragment build),
-    triangular product 1."""
-    return 9 if n <= 64 else 12
+    4 (n > 64: fragment build, panel substitution, syrk, reduce), Cholesky 1 (the product R = R1 R0 is fused into
+    it for n <= 128; a separate launch above), A6 1 (n > 64: + fragment build)."""
+    return 8 if n <= 64 else (11 if n <= 128 else 12)
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed

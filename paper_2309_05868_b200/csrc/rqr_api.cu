@@ -4,7 +4,7 @@
 #include "rqr_common.cuh"
 
 int rqr_chol_dev(const double* G, int n, double shift, const double* d_shift, double* R1,
-                 int* d_info, cudaStream_t st);
+                 int* d_info, cudaStream_t st, const double* Rprev, double* Rprod);
 int rqr_scholqr3_shift(const double* G, int n, int64_t m, double* d_out, cudaStream_t st);
 
 extern "C" const char* rqr_version(void) { return "rqr 0.1 (sm_100a)"; }
@@ -36,18 +36,18 @@ static int check_common(const double* V, int64_t m, int n, double* Q, double* R,
     return RQR_OK;
 }
 
-// cholQR of the matrix held in X (m x n, ld n), given its Gram partial state: shared tail of
-// every driver.  A4 with R_prev (may be NULL) writes V1 into Q, A5, A6 in place.
+// cholQR of V R0^-1: shared tail of every driver.  A4 with R0 writes V1 into Q, A5 (which also forms
+// Rprod = R1 R0, the drivers' A7, when Rprod != NULL), A6 in place.
 static int tail_cholqr(const double* V, int64_t m, int n, const double* R0, double* Q, double* R1,
-                       double* G, void* work, int* d_info, int recompute, cudaStream_t st)
+                       double* G, void* work, int* d_info, int recompute, cudaStream_t st, double* Rprod)
 {
     if (recompute && R0 && n <= 64) {     // n > 64: A4 is FP64-bound either way and V1 is always stored
         RQR_TRY(rqr_trsm_gram(V, m, n, n, R0, G, nullptr, n, work, st));
-        RQR_TRY(rqr_chol_dev(G, n, 0.0, nullptr, R1, d_info, st));
+        RQR_TRY(rqr_chol_dev(G, n, 0.0, nullptr, R1, d_info, st, R0, Rprod));
         RQR_TRY(rqr_apply(V, m, n, n, R0, R1, Q, n, work, st));
     } else {
         RQR_TRY(rqr_trsm_gram(V, m, n, n, R0, G, Q, n, work, st));
-        RQR_TRY(rqr_chol_dev(G, n, 0.0, nullptr, R1, d_info, st));
+        RQR_TRY(rqr_chol_dev(G, n, 0.0, nullptr, R1, d_info, st, R0, Rprod));
         RQR_TRY(rqr_apply(Q, m, n, n, nullptr, R1, Q, n, work, st));
     }
     return RQR_OK;
@@ -78,8 +78,7 @@ extern "C" int rqr_rand_cholqr(const double* V, int64_t m, int n, int64_t s1, in
     RQR_TRY(rqr_gauss_sketch(W1, s1, n, s2, seed, W, work, RQR_FLAG_PREPARED, st));
     RQR_TRY(rqr_small_geqrf(W, s2, n, R0, d_info, st));
     // Alg. 2 cholQR of V1; Alg. 3 step 3
-    RQR_TRY(tail_cholqr(V, m, n, R0, Q, R1, G, work, d_info, flags & RQR_FLAG_RECOMPUTE_V1, st));
-    RQR_TRY(rqr_triu_mul(R1, R0, n, R, st));
+    RQR_TRY(tail_cholqr(V, m, n, R0, Q, R1, G, work, d_info, flags & RQR_FLAG_RECOMPUTE_V1, st, R));
     return RQR_OK;
 }
 
@@ -99,8 +98,7 @@ extern "C" int rqr_gauss_randcholqr(const double* V, int64_t m, int n, int s, ui
     if (d_info && cudaMemsetAsync(d_info, 0, sizeof(int), st) != cudaSuccess) return RQR_ERR_LAUNCH;
     RQR_TRY(rqr_dense_gauss_sketch(V, m, n, n, 0, m, s, seed, W, work, st));
     RQR_TRY(rqr_small_geqrf(W, s, n, R0, d_info, st));
-    RQR_TRY(tail_cholqr(V, m, n, R0, Q, R1, G, work, d_info, 0, st));
-    RQR_TRY(rqr_triu_mul(R1, R0, n, R, st));
+    RQR_TRY(tail_cholqr(V, m, n, R0, Q, R1, G, work, d_info, 0, st, R));
     return RQR_OK;
 }
 
@@ -118,10 +116,9 @@ extern "C" int rqr_cholqr2(const double* V, int64_t m, int n, double* Q, double*
     if (d_info && cudaMemsetAsync(d_info, 0, sizeof(int), st) != cudaSuccess) return RQR_ERR_LAUNCH;
     // Alg. 4 step 1: cholQR(V): G = V^T V, RA = chol(G); Q0 = V RA^-1 is formed inside step 2's A4
     RQR_TRY(rqr_trsm_gram(V, m, n, n, nullptr, G, nullptr, n, work, st));
-    RQR_TRY(rqr_chol_dev(G, n, 0.0, nullptr, RA, d_info, st));
-    // step 2: cholQR(Q0)
-    RQR_TRY(tail_cholqr(V, m, n, RA, Q, RB, G, work, d_info, 0, st));
-    RQR_TRY(rqr_triu_mul(RB, RA, n, R, st));
+    RQR_TRY(rqr_chol_dev(G, n, 0.0, nullptr, RA, d_info, st, nullptr, nullptr));
+    // step 2: cholQR(Q0); R = RB RA
+    RQR_TRY(tail_cholqr(V, m, n, RA, Q, RB, G, work, d_info, 0, st, R));
     return RQR_OK;
 }
 
@@ -142,12 +139,11 @@ extern "C" int rqr_scholqr3(const double* V, int64_t m, int n, double* Q, double
     if (d_info && cudaMemsetAsync(d_info, 0, sizeof(int), st) != cudaSuccess) return RQR_ERR_LAUNCH;
     RQR_TRY(rqr_trsm_gram(V, m, n, n, nullptr, G, nullptr, n, work, st));
     RQR_TRY(rqr_scholqr3_shift(G, n, m, d_shift, st));
-    RQR_TRY(rqr_chol_dev(G, n, 0.0, d_shift, RA, d_info, st));
+    RQR_TRY(rqr_chol_dev(G, n, 0.0, d_shift, RA, d_info, st, nullptr, nullptr));
     // Q1 = V RA^-1 and its Gram; then cholQR2 of Q1
     RQR_TRY(rqr_trsm_gram(V, m, n, n, RA, G, Q, n, work, st));
-    RQR_TRY(rqr_chol_dev(G, n, 0.0, nullptr, RB, d_info, st));
-    RQR_TRY(tail_cholqr(Q, m, n, RB, Q, RC, G, work, d_info, 0, st));
-    RQR_TRY(rqr_triu_mul(RC, RB, n, T, st));
+    RQR_TRY(rqr_chol_dev(G, n, 0.0, nullptr, RB, d_info, st, nullptr, nullptr));
+    RQR_TRY(tail_cholqr(Q, m, n, RB, Q, RC, G, work, d_info, 0, st, T));       // T = RC RB
     RQR_TRY(rqr_triu_mul(T, RA, n, R, st));
     return RQR_OK;
 }

@@ -481,7 +481,7 @@ extern "C" int rqr_small_geqrf(double* W, int s2, int n, double* R0, int* d_info
 template <int RPL, int CPW, int NW>
 __global__ void __launch_bounds__(NW * 32, 1)
 k_chol_small(const double* __restrict__ G, int n, double shift_h, const double* __restrict__ d_shift,
-             double* __restrict__ R1, int* d_info)
+             double* R1, int* d_info, const double* __restrict__ Rprev, double* __restrict__ Rprod)
 {
     __shared__ double srow[2][CHOL_ROW_LD];
     const double shift = shift_h + (d_shift ? *d_shift : 0.0);
@@ -542,6 +542,17 @@ k_chol_small(const double* __restrict__ G, int n, double shift_h, const double* 
         }
     }
     if (fail && threadIdx.x == 0) rqr_set_info(d_info, RQR_INFO_NOT_SPD + fail);
+    if (Rprod != nullptr) {
+        // fused A7 of the one-shot drivers: Rprod = R1 Rprev (upper x upper, Alg. 3 step 3 PAPER.md:206);
+        // R1 was written by this CTA: visible after the barrier
+        __syncthreads();
+        for (int e = threadIdx.x; e < n * n; e += NW * 32) {
+            const int a_ = e / n, c = e - a_ * n;
+            double acc = 0.0;
+            for (int k = a_; k <= c; ++k) acc = fma(R1[a_ * n + k], __ldg(Rprev + k * n + c), acc);
+            Rprod[e] = (c >= a_) ? acc : 0.0;
+        }
+    }
 }
 
 template <int RPL, int CPW, int NW, bool CL>
@@ -628,11 +639,11 @@ k_chol_cols(const double* __restrict__ G, int n, double shift_h, const double* _
 }
 
 int rqr_chol_dev(const double* G, int n, double shift, const double* d_shift, double* R1,
-                 int* d_info, cudaStream_t st);
+                 int* d_info, cudaStream_t st, const double* Rprev, double* Rprod);
 
 extern "C" int rqr_chol(const double* G, int n, double shift, double* R1, int* d_info, void* stream)
 {
-    return rqr_chol_dev(G, n, shift, nullptr, R1, d_info, (cudaStream_t)stream);
+    return rqr_chol_dev(G, n, shift, nullptr, R1, d_info, (cudaStream_t)stream, nullptr, nullptr);
 }
 
 // shift = 11 (m n + n (n+1)) 2^-53 tr(G)   (shifted CholeskyQR3, reading S9)
@@ -652,16 +663,22 @@ int rqr_scholqr3_shift(const double* G, int n, int64_t m, double* d_out, cudaStr
     return RQR_OK;
 }
 
+// Rprod != NULL: also Rprod = R1 Rprev (the one-shot drivers' A7), fused into the single-CTA kernel
+// for n <= 128, a separate k_triu_mul launch above that.
 int rqr_chol_dev(const double* G, int n, double shift, const double* d_shift, double* R1,
-                 int* d_info, cudaStream_t st)
+                 int* d_info, cudaStream_t st, const double* Rprev, double* Rprod)
 {
     if (!G) return -1;
     if (n < 2 || n > RQR_MAX_N) return -2;
     if (!R1) return -4;
     if (G == R1) return -4;
-    if (n <= 64)       k_chol_small<2, 8, 8><<<1, 256, 0, st>>>(G, n, shift, d_shift, R1, d_info);
-    else if (n <= 128) k_chol_small<4, 8, 16><<<1, 512, 0, st>>>(G, n, shift, d_shift, R1, d_info);
-    else return launch_cluster(k_chol_cols<8, 4, 8, true>, 8, 256, st, G, n, shift, d_shift, R1, d_info);
+    if (n <= 64)       k_chol_small<2, 8, 8><<<1, 256, 0, st>>>(G, n, shift, d_shift, R1, d_info, Rprev, Rprod);
+    else if (n <= 128) k_chol_small<4, 8, 16><<<1, 512, 0, st>>>(G, n, shift, d_shift, R1, d_info, Rprev, Rprod);
+    else {
+        int rc = launch_cluster(k_chol_cols<8, 4, 8, true>, 8, 256, st, G, n, shift, d_shift, R1, d_info);
+        if (rc != RQR_OK || !Rprod) return rc;
+        return rqr_triu_mul(R1, Rprev, n, Rprod, st);
+    }
     RQR_LAUNCH_CHECK();
     return RQR_OK;
 }
