@@ -481,7 +481,7 @@ extern "C" int rqr_small_geqrf(double* W, int s2, int n, double* R0, int* d_info
 template <int RPL, int CPW, int NW>
 __global__ void __launch_bounds__(NW * 32, 1)
 k_chol_small(const double* __restrict__ G, int n, double shift_h, const double* __restrict__ d_shift,
-             double* R1, int* d_info, const double* __restrict__ Rprev, double* __restrict__ Rprod)
+             double* R1, int* d_info, const double* __restrict__ Rprev, double* __restrict__ Rprod, int staged)
 {
     __shared__ double srow[2][CHOL_ROW_LD];
     const double shift = shift_h + (d_shift ? *d_shift : 0.0);
@@ -543,14 +543,33 @@ k_chol_small(const double* __restrict__ G, int n, double shift_h, const double* 
     }
     if (fail && threadIdx.x == 0) rqr_set_info(d_info, RQR_INFO_NOT_SPD + fail);
     if (Rprod != nullptr) {
-        // fused A7 of the one-shot drivers: Rprod = R1 Rprev (upper x upper, Alg. 3 step 3 PAPER.md:206);
-        // R1 was written by this CTA: visible after the barrier
+        // fused A7 of the one-shot drivers: Rprod = R1 Rprev (upper x upper, Alg. 3 step 3 PAPER.md:206).
+        // R1 was written by this CTA: visible after the barrier.  Both factors are staged in shared
+        // memory when the launch provided room for them (n <= 64), rows of Rprev padded against conflicts.
+        extern __shared__ double stage[];
         __syncthreads();
-        for (int e = threadIdx.x; e < n * n; e += NW * 32) {
-            const int a_ = e / n, c = e - a_ * n;
-            double acc = 0.0;
-            for (int k = a_; k <= c; ++k) acc = fma(R1[a_ * n + k], __ldg(Rprev + k * n + c), acc);
-            Rprod[e] = (c >= a_) ? acc : 0.0;
+        if (staged) {
+            double* s1_ = stage;                         // R1, row-major, ld n
+            double* s0_ = stage + n * n;                 // Rprev, row-major, ld n + 1
+            for (int e = threadIdx.x; e < n * n; e += NW * 32) {
+                const int a_ = e / n, c = e - a_ * n;
+                s1_[e] = R1[e];
+                s0_[a_ * (n + 1) + c] = __ldg(Rprev + e);
+            }
+            __syncthreads();
+            for (int e = threadIdx.x; e < n * n; e += NW * 32) {
+                const int a_ = e / n, c = e - a_ * n;
+                double acc = 0.0;
+                for (int k = a_; k <= c; ++k) acc = fma(s1_[a_ * n + k], s0_[k * (n + 1) + c], acc);
+                Rprod[e] = (c >= a_) ? acc : 0.0;
+            }
+        } else {
+            for (int e = threadIdx.x; e < n * n; e += NW * 32) {
+                const int a_ = e / n, c = e - a_ * n;
+                double acc = 0.0;
+                for (int k = a_; k <= c; ++k) acc = fma(__ldcg(R1 + a_ * n + k), __ldg(Rprev + k * n + c), acc);
+                Rprod[e] = (c >= a_) ? acc : 0.0;
+            }
         }
     }
 }
@@ -672,8 +691,15 @@ int rqr_chol_dev(const double* G, int n, double shift, const double* d_shift, do
     if (n < 2 || n > RQR_MAX_N) return -2;
     if (!R1) return -4;
     if (G == R1) return -4;
-    if (n <= 64)       k_chol_small<2, 8, 8><<<1, 256, 0, st>>>(G, n, shift, d_shift, R1, d_info, Rprev, Rprod);
-    else if (n <= 128) k_chol_small<4, 8, 16><<<1, 512, 0, st>>>(G, n, shift, d_shift, R1, d_info, Rprev, Rprod);
+    if (n <= 64) {
+        const size_t sm = Rprod ? (size_t)(2 * n * n + n) * sizeof(double) : 0;      // <= 66 KB
+        static bool attr = false;
+        if (!attr) {
+            cudaFuncSetAttribute(k_chol_small<2, 8, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 72 * 1024);
+            attr = true;
+        }
+        k_chol_small<2, 8, 8><<<1, 256, sm, st>>>(G, n, shift, d_shift, R1, d_info, Rprev, Rprod, 1);
+    } else if (n <= 128) k_chol_small<4, 8, 16><<<1, 512, 0, st>>>(G, n, shift, d_shift, R1, d_info, Rprev, Rprod, 0);
     else {
         int rc = launch_cluster(k_chol_cols<8, 4, 8, true>, 8, 256, st, G, n, shift, d_shift, R1, d_info);
         if (rc != RQR_OK || !Rprod) return rc;
