@@ -106,7 +106,7 @@ def launches_per_step(n):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # ncu --set full captures (profiles/): workload -> bytes
-NCU_TRAFFIC = {"C2": 536.9e6 + 493.3e6}
+NCU_TRAFFIC = {"C2": 537.1e6 + 491.1e6}
 
 
 def measured_peaks():
@@ -329,7 +329,7 @@ def main():
         ach = flops.trsm_gram_flops(m, n) / (bd[dom] * 1e-3) / 1e12
         roof = {"kernel": "rqr_trsm_gram", "bound": "tensor", "achieved": ach, "peak": p64, "unit": "TFLOP/s",
                 "frac": ach / p64, "traffic": NCU_TRAFFIC.get(args.workload),
-                "traffic_source": "profiles/r1_baseline_summary.md (ncu --set full, per launch)",
+                "traffic_source": "profiles/r1_final_summary.md section 2 (ncu --set full, per launch)",
                 "algorithmic": "2 m n^2 flops per launch (n^2 substitution + n^2 symmetric Gram per row); "
                                "16 m n bytes (read V, write V1)",
                 "peak_source": "FP64 probe measured live in this run (max of DFMA %.1f / DMMA %.1f TFLOP/s); "
