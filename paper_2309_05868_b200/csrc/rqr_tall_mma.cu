@@ -332,13 +332,22 @@ k_trsm_gram_pair(const double* __restrict__ V, int64_t m, int n, int64_t ldv, co
 // ------------------------------------------------------------------------------------------
 // A6: Q = (V R0^-1) R1^-1  (TWO) or Q = V R1^-1.
 // ------------------------------------------------------------------------------------------
+// A6 launch shape, measured at 2^23 x 64 (profiles/r1_final_summary.md): the in-place pass (one chain per
+// row-block, HBM-bound) is fastest with 8 warps x 3 stages (1.31 ms = 6.56 TB/s; 12 x 2: 1.44, 10 x 3: 1.53,
+// 6 x 4: 1.71), the two-pass recompute mode (DMMA-bound) with 12 x 2 (2.22 ms; 8 x 3: 2.42).
+// n <= 16 (tiny row-blocks) keeps 12 x 2 in both modes (2^22 x 16: 0.21 vs 0.25 ms).
+template <int NB, bool TWO> struct ApplyCfg {
+    static constexpr int WARPS = (TWO || NB < 4) ? 12 : 8;
+    static constexpr int STAGES = (TWO || NB < 4) ? 2 : 3;
+};
+
 template <int NB, bool TWO, bool FULL>
-__global__ void __launch_bounds__(APPLY_WARPS * 32, 1)
+__global__ void __launch_bounds__(ApplyCfg<NB, TWO>::WARPS * 32, 1)
 k_apply_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
             const double* __restrict__ R0, const double* __restrict__ R1,
             double* __restrict__ Q, int64_t ldq)
 {
-    using Plan = SmemPlan<NB, APPLY_WARPS, APPLY_STAGES, 2, 0>;
+    using Plan = SmemPlan<NB, ApplyCfg<NB, TWO>::WARPS, ApplyCfg<NB, TWO>::STAGES, 2, 0>;
     constexpr int LDL = Plan::LDL, N8 = Plan::N8;
     constexpr int FD = TallCfg<NB>::FRAG_DOUBLES;
     constexpr int NBLK = TallCfg<NB>::NBLK;
@@ -353,20 +362,20 @@ k_apply_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 
     for (int i = threadIdx.x; i < (int)Plan::ring_doubles; i += blockDim.x) ring[i] = 0.0;
-    if (threadIdx.x < APPLY_WARPS * APPLY_STAGES) mbar_init(bars + threadIdx.x, 1);
+    if (threadIdx.x < ApplyCfg<NB, TWO>::WARPS * ApplyCfg<NB, TWO>::STAGES) mbar_init(bars + threadIdx.x, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     fence_proxy_async();
     __syncthreads();
     build_tri_frags<NB>(R1, n, Tf1, nRf1, scratch);
     if (TWO) build_tri_frags<NB>(R0, n, Tf0, nRf0, scratch);
 
-    WarpRing<LDL> wr{ring + (size_t)warp * APPLY_STAGES * 8 * LDL, bars + warp * APPLY_STAGES, V, ldv, m, n};
+    WarpRing<LDL> wr{ring + (size_t)warp * ApplyCfg<NB, TWO>::STAGES * 8 * LDL, bars + warp * ApplyCfg<NB, TWO>::STAGES, V, ldv, m, n};
     const XsAddr<N8> ad(lane);
     const int64_t nrb = (m + 7) / 8;
-    const int64_t gw = (int64_t)blockIdx.x * APPLY_WARPS + warp;
-    const int64_t stride = (int64_t)gridDim.x * APPLY_WARPS;
+    const int64_t gw = (int64_t)blockIdx.x * ApplyCfg<NB, TWO>::WARPS + warp;
+    const int64_t stride = (int64_t)gridDim.x * ApplyCfg<NB, TWO>::WARPS;
 #pragma unroll
-    for (int s = 0; s < APPLY_STAGES; ++s)
+    for (int s = 0; s < ApplyCfg<NB, TWO>::STAGES; ++s)
         if (gw + s * stride < nrb) wr.issue(s, gw + s * stride, lane);
     double acc[NB][2];
     double g[NB];
@@ -385,7 +394,7 @@ k_apply_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
         }
         load_acc<NB, LDL>(acc, rb, lane);
         auto refill = [&]() {
-            const int64_t next = rblk + (int64_t)APPLY_STAGES * stride;
+            const int64_t next = rblk + (int64_t)ApplyCfg<NB, TWO>::STAGES * stride;
             if (next < nrb) {
                 fence_proxy_async();
                 __syncwarp();
@@ -400,7 +409,7 @@ k_apply_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
         } else {
             trsm_rowblock<NB, false, false, FULL>(acc, nullptr, nullptr, ad, Tf1, nRf1, gp, colmask, lane, g, G, refill);
         }
-        if (++stage == APPLY_STAGES) { stage = 0; phase ^= 1u; }
+        if (++stage == ApplyCfg<NB, TWO>::STAGES) { stage = 0; phase ^= 1u; }
     }
 }
 
@@ -481,28 +490,32 @@ int rqr_trsm_gram_mma(const double* V, int64_t m, int n, int64_t ldv, const doub
     return launch_trsm_gram<8>(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
 }
 
+template <int NB, bool TWO>
+static int launch_apply_mode(const double* V, int64_t m, int n, int64_t ldv, const double* R0, const double* R1,
+                             double* Q, int64_t ldq, cudaStream_t st)
+{
+    constexpr int W = ApplyCfg<NB, TWO>::WARPS;
+    using Plan = SmemPlan<NB, W, ApplyCfg<NB, TWO>::STAGES, 2, 0>;
+    static_assert(Plan::bytes <= 227 * 1024, "A6 shared memory plan too large");
+    static bool attr = false;
+    if (!attr) {
+        cudaFuncSetAttribute(k_apply_mma<NB, TWO, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
+        cudaFuncSetAttribute(k_apply_mma<NB, TWO, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
+        attr = true;
+    }
+    const int grid = grid_for(m, W);
+    if (n == 8 * NB) k_apply_mma<NB, TWO, true><<<grid, W * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, R1, Q, ldq);
+    else             k_apply_mma<NB, TWO, false><<<grid, W * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, R1, Q, ldq);
+    RQR_LAUNCH_CHECK();
+    return RQR_OK;
+}
+
 template <int NB>
 static int launch_apply(const double* V, int64_t m, int n, int64_t ldv, const double* R0, const double* R1,
                         double* Q, int64_t ldq, cudaStream_t st)
 {
-    using Plan = SmemPlan<NB, APPLY_WARPS, APPLY_STAGES, 2, 0>;
-    static_assert(Plan::bytes <= 227 * 1024, "A6 shared memory plan too large");
-    static bool attr = false;
-    if (!attr) {
-        cudaFuncSetAttribute(k_apply_mma<NB, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
-        cudaFuncSetAttribute(k_apply_mma<NB, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
-        cudaFuncSetAttribute(k_apply_mma<NB, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
-        cudaFuncSetAttribute(k_apply_mma<NB, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
-        attr = true;
-    }
-    const int grid = grid_for(m, APPLY_WARPS);
-    const bool full = (n == 8 * NB);
-    if (R0 && full)  k_apply_mma<NB, true, true><<<grid, APPLY_WARPS * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, R1, Q, ldq);
-    else if (R0)     k_apply_mma<NB, true, false><<<grid, APPLY_WARPS * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, R1, Q, ldq);
-    else if (full)   k_apply_mma<NB, false, true><<<grid, APPLY_WARPS * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, R1, Q, ldq);
-    else             k_apply_mma<NB, false, false><<<grid, APPLY_WARPS * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, R1, Q, ldq);
-    RQR_LAUNCH_CHECK();
-    return RQR_OK;
+    return R0 ? launch_apply_mode<NB, true>(V, m, n, ldv, R0, R1, Q, ldq, st)
+              : launch_apply_mode<NB, false>(V, m, n, ldv, R0, R1, Q, ldq, st);
 }
 
 int rqr_apply_mma(const double* V, int64_t m, int n, int64_t ldv, const double* R0, const double* R1,
