@@ -37,6 +37,8 @@ def parse():
     ap.add_argument("--recompute-v1", action="store_true")
     ap.add_argument("--no-probe", action="store_true", help="skip the FP64 peak probe (profiling runs)")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--force-sharded", action="store_true",
+                    help="run the row-sharded N > 1 code path even at one rank (self-test of that path)")
     return ap.parse_args()
 
 
@@ -298,9 +300,12 @@ def main():
     torch.cuda.set_device(local)
     if rank == 0:
         ge.build()
-    if world > 1:
+    if world > 1 or args.force_sharded:
         import torch.distributed as dist
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29533")
+        os.environ.setdefault("RANK", "0")
+        os.environ.setdefault("WORLD_SIZE", "1")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
         dist.barrier()
         run_sharded(torch, rq, args, world, rank)
@@ -391,6 +396,9 @@ def run_sharded(torch, rq, args, world, rank):
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
     ms = float(t.item()) / args.steps
     F = flops.rand_cholqr_flops(m_total, n, s1, s2)
+    QtQ = Q.T @ Q                                   # check with library ops: || I - Q^T Q ||_F over all ranks
+    dist.all_reduce(QtQ, op=dist.ReduceOp.SUM)
+    orth = float(torch.linalg.norm(QtQ - torch.eye(n, dtype=torch.float64, device="cuda")))
     if rank == 0:
         line = {"metric": "rand_cholQR FP64 GFLOP/s", "value": F / ms / 1e6, "unit": "GFLOP/s", "n_gpus": world,
                 "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
@@ -398,7 +406,8 @@ def run_sharded(torch, rq, args, world, rank):
                 "config": {"workload": args.workload, "m_per_gpu": m, "m_total": m_total, "n": n, "s1": s1, "s2": s2,
                            "parallelism": "row-sharded, 2 all-reduces (W, G) per step",
                            "l2": "inputs_exceed_L2"},
-                "gpu_launches": launches_per_step(n) * args.steps, "info": int(bufs["info"].item())}
+                "gpu_launches": (launches_per_step(n) + 1) * args.steps,      # step entry points: A7 is its own launch
+                "info": int(bufs["info"].item()), "orth_err": orth}
         print(json.dumps(line))
 
 
