@@ -28,8 +28,13 @@
  *    one-shot drivers zero it themselves).  Outputs are undefined when *d_info != 0.
  *  - Argument limits: 2 <= n <= 256, n <= s2 <= s1 <= m_total (eq. (20)),
  *    s2 <= 512, s1 < 2^31, m < 2^31 per call.
- *  - Thread safety: no global mutable state; calls on different streams with different
- *    buffers are independent.
+ *  - Fast paths: the FP64 DMMA kernels of rqr_trsm_gram / rqr_apply need an even n, even leading
+ *    dimensions and 16-byte aligned bases (2 <= n <= 64: fused kernels; 64 < n <= 256: panel
+ *    kernels); rqr_gauss_sketch uses its DMMA GEMM for even n >= 96 with s1 % 16 == 0.  Any other
+ *    shape runs the generic kernels: same results to rounding, much slower.
+ *  - Thread safety: calls on different streams with different buffers are independent.  The only
+ *    global state is one-time kernel-attribute initialisation and the two debug switches
+ *    (rqr_debug_force_generic, environment variable RQR_A4_PAIR=0 read once).
  */
 #ifndef RQR_H
 #define RQR_H
@@ -84,7 +89,8 @@ int rqr_gauss_sketch(const double* W1, int64_t s1, int n, int s2, uint64_t seed,
                      void* work, int flags, void* stream);
 
 /* A3 -- R factor of the Householder QR of W (Alg. 1 step 2).  W (s2 x n) is
- * destroyed.  R0 is n x n upper triangular with diag > 0 and exact zeros below.             */
+ * destroyed (for n > 64 its storage carries the reflectors between the CTAs of the cluster).
+ * R0 is n x n upper triangular with diag > 0 and exact zeros below.                         */
 int rqr_small_geqrf(double* W, int s2, int n, double* R0, int* d_info, void* stream);
 
 /* A4 -- fused V1 = V R0^-1 (Alg. 1 step 3; row-wise substitution, eq. (42)
@@ -98,7 +104,9 @@ int rqr_small_geqrf(double* W, int s2, int n, double* R0, int* d_info, void* str
 int rqr_trsm_gram(const double* V, int64_t m, int n, int64_t ldv, const double* R0, double* G,
                   double* V1, int64_t ldq, void* work, void* stream);
 
-/* A5 -- upper Cholesky factor, G + shift I = R1^T R1 (Alg. 2 step 2).          */
+/* A5 -- upper Cholesky factor, G + shift I = R1^T R1 (Alg. 2 step 2).  R1 is n x n
+ * upper triangular with diag > 0 and exact zeros below; it must not alias G (its storage is the
+ * exchange buffer of the cluster kernel for n > 128).                                        */
 int rqr_chol(const double* G, int n, double shift, double* R1, int* d_info, void* stream);
 
 /* A6 -- Q = (V R0^-1) R1^-1 (Alg. 2 step 3), never V (R0^-1 R1^-1).
