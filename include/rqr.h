@@ -27,7 +27,8 @@
  *    d_info is written only on failure (first failure wins); the caller zeroes it (the
  *    one-shot drivers zero it themselves).  Outputs are undefined when *d_info != 0.
  *  - Argument limits: 2 <= n <= 256, n <= s2 <= s1 <= m_total (eq. (20)),
- *    s2 <= 512, s1 < 2^31, m < 2^31 per call.
+ *    s2 <= 1024 (s2 > 512 needs n <= 128 for the register-resident Householder kernel, else a
+ *    slow fallback runs), s1 < 2^31, m < 2^31 per call.
  *  - Fast paths: the FP64 DMMA kernels of rqr_trsm_gram / rqr_apply need an even n, even leading
  *    dimensions and 16-byte aligned bases (2 <= n <= 64: fused kernels; 64 < n <= 256: panel
  *    kernels); rqr_gauss_sketch uses its DMMA GEMM for even n >= 96 with s1 % 16 == 0.  Any other

@@ -7,7 +7,7 @@
 #include "../../include/rqr.h"
 
 #define RQR_MAX_N 256
-#define RQR_MAX_S2 512
+#define RQR_MAX_S2 1024
 #define RQR_MAX_GRAM_PARTIALS 304        // >= 2 CTAs per SM on 148 SMs
 #define RQR_GAUSS_PARTIAL_ROWS 16384     // ksplit * s2 <= this
 #define RQR_PANEL_FRAG_BYTES (2 * 10 * 4096 * sizeof(double))   // rqr_tall_panel.cu

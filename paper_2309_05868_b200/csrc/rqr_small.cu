@@ -313,11 +313,11 @@ __device__ __forceinline__ void cluster_sync_all()
 // slot (c / ncta) / 16; lane l owns rows l + 32 p.  512 threads per CTA.  After the load W's own
 // storage is scratch: the reflector v (double-buffered), beta and the sign flags travel through
 // it (L2) with ONE cluster barrier per Householder step.
-template <int RPL>
+template <int RPL, int CPW>
 __global__ void __launch_bounds__(512, 1)
 k_geqrf_cluster(double* W, int s2, int n, double* __restrict__ R0, int* d_info)
 {
-    constexpr int CPW = 2;
+    __shared__ double vs[32 * RPL];          // this step's reflector (registers hold the columns only)
     const int ncta = (int)cluster_size(), rank = (int)cluster_rank();
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     double a[CPW][RPL];
@@ -370,17 +370,20 @@ k_geqrf_cluster(double* W, int s2, int n, double* __restrict__ R0, int* d_info)
             }
         }
         cluster_sync_all();
-        double v[RPL];
-#pragma unroll
-        for (int p = 0; p < RPL; ++p) v[p] = __ldcg(vj_buf + lane + 32 * p);
+        for (int i = threadIdx.x; i < 32 * RPL; i += 512) vs[i] = __ldcg(vj_buf + i);
         const double beta = __ldcg(gbeta + (j & 1));
+        __syncthreads();
+        const double* v = vs + lane;
         double dot[CPW];
 #pragma unroll
         for (int q = 0; q < CPW; ++q) {
-            double sacc = 0.0;
+            double s0 = 0.0, s1_ = 0.0;
 #pragma unroll
-            for (int p = 0; p < RPL; ++p) sacc = fma(v[p], a[q][p], sacc);
-            dot[q] = sacc;
+            for (int p = 0; p < RPL; p += 2) {
+                s0 = fma(v[32 * p], a[q][p], s0);
+                s1_ = fma(v[32 * (p + 1)], a[q][p + 1], s1_);
+            }
+            dot[q] = s0 + s1_;
         }
 #pragma unroll
         for (int q = 0; q < CPW; ++q) dot[q] = warp_sum(dot[q]);
@@ -390,7 +393,7 @@ k_geqrf_cluster(double* W, int s2, int n, double* __restrict__ R0, int* d_info)
             if (c > j && c < n) {
                 const double ws = beta * dot[q];
 #pragma unroll
-                for (int p = 0; p < RPL; ++p) a[q][p] = fma(-ws, v[p], a[q][p]);
+                for (int p = 0; p < RPL; ++p) a[q][p] = fma(-ws, v[32 * p], a[q][p]);
             }
         }
     }
@@ -450,10 +453,14 @@ extern "C" int rqr_small_geqrf(double* W, int s2, int n, double* R0, int* d_info
 #undef GEQRF_CASE
     // n > 64: the register tile is spread over a cluster of 4 or 8 CTAs.  W's storage doubles as
     // the exchange buffer (2 * 32 * RPL + 2 + n doubles), which it always has room for here.
-    if ((int64_t)s2 * n >= 2 * 512 + 2 + n) {
-        const int ncta = n <= 128 ? 4 : 8;
-        if (rpl <= 8) return launch_cluster(k_geqrf_cluster<8>, ncta, 512, st, W, s2, n, R0, d_info);
-        return launch_cluster(k_geqrf_cluster<16>, ncta, 512, st, W, s2, n, R0, d_info);
+    if ((int64_t)s2 * n >= 2 * 32 * rpl + 2 + n) {
+        if (rpl <= 16) {
+            const int ncta = n <= 128 ? 4 : 8;                     // 16 warps x 2 columns per CTA
+            if (rpl <= 8) return launch_cluster(k_geqrf_cluster<8, 2>, ncta, 512, st, W, s2, n, R0, d_info);
+            return launch_cluster(k_geqrf_cluster<16, 2>, ncta, 512, st, W, s2, n, R0, d_info);
+        }
+        if (n <= 128)                                              // tall sketches of the paper's grid (s2 <= 1024)
+            return launch_cluster(k_geqrf_cluster<32, 1>, n <= 64 ? 4 : 8, 512, st, W, s2, n, R0, d_info);
     }
     k_geqrf_gmem<<<1, 1024, 0, st>>>(W, s2, n, R0, d_info);
     RQR_LAUNCH_CHECK();

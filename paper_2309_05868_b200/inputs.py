@@ -112,15 +112,16 @@ def make_V_reflectors(m: int, n: int, kappa: float, seed: int, device="cpu", k: 
     E = sqrt(n/m) [I_n; I_n; ...] (stacked identities: orthonormal columns, all rows of equal norm, like a
     Haar U), D random signs, and k random Householder reflectors (Gaussian vectors): orthonormal to rounding
     by construction ("Haar-like"); W Haar as in make_V.  O(k m n) work, in place.
-    m must be a multiple of n."""
-    assert m % n == 0
+    (If n does not divide m the columns of E have counts that differ by one and are normalised one by one.)"""
     gen = torch.Generator(device=device)
     gen.manual_seed(int(seed))
     sgn = torch.randint(0, 2, (m,), generator=gen, device=device).to(torch.float64) * 2.0 - 1.0
     U = torch.zeros(m, n, dtype=torch.float64, device=device)
     idx = torch.arange(m, device=device)
-    U[idx, idx % n] = sgn * (n / m) ** 0.5
-    del idx, sgn
+    col = idx % n
+    cnt = torch.bincount(col, minlength=n).to(torch.float64)
+    U[idx, col] = sgn / torch.sqrt(cnt[col])
+    del idx, sgn, col, cnt
     for _ in range(k):
         v = torch.randn(m, generator=gen, dtype=torch.float64, device=device)
         v /= torch.linalg.norm(v)

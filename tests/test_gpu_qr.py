@@ -226,3 +226,23 @@ def test_full_size_config_matches_oracle(rq, orc, name):
     Qs = Q[torch.from_numpy(rows).cuda()].cpu().numpy()
     scale = np.linalg.norm(Vh) / np.sqrt(m)
     assert np.abs(Qs @ Ro - Vh[rows]).max() <= 1e-11 * scale
+
+
+@pytest.mark.parametrize("m,n", [(100000, 70), (100000, 30), (60000, 100)])
+def test_paper_grid_shape_and_sketch_sizes(rq, orc, m, n):
+    """the paper's own shapes with its "Multi (0.9, 0.49)" sketch sizes
+    s1 = ceil(8.24 (n^2 + n)), s2 = ceil(74.3 log s1): non-power-of-two s1 (general bucket map),
+    s2 up to 842 rows (tall Householder kernel), ragged column blocks."""
+    from paper_2309_05868_b200.paper_grid import paper_sketch_sizes
+    s1, s2 = paper_sketch_sizes(n)
+    if s1 > m:
+        pytest.skip("s1 > m")
+    V = inputs.make_V(m, n, 1e9, 4321)
+    Vd = V.cuda()
+    Q, R, info = run_rand(rq, Vd, s1, s2, 42, 0, 0, True)
+    assert info == 0
+    assert orth_err(Q) <= ORTH_TOL and resid(Vd, Q, R) <= RES_TOL
+    check_R(R)
+    _, Ro, io = orc.rand_cholqr(V.numpy(), s1, s2, 42)
+    assert io == 0
+    assert np.linalg.norm(R.cpu().numpy() - Ro) <= R_TOL * np.linalg.norm(Ro)

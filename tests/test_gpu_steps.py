@@ -90,7 +90,7 @@ def test_countsketch_strided_and_row_offset(rq, orc):
 
 @pytest.mark.parametrize("s1,n,s2", [(512, 16, 32), (8192, 64, 128), (9940, 70, 140), (300, 5, 7),
                                      (4096, 256, 512), (32768, 128, 256), (9984, 200, 401), (40000, 98, 130),
-                                     (65536, 256, 512)])
+                                     (65536, 256, 512), (40953, 70, 789)])
 def test_gauss_sketch_parity(rq, orc, s1, n, s2):
     rng = np.random.default_rng(s1 + n)
     W1 = rng.standard_normal((s1, n))
@@ -112,7 +112,7 @@ def test_dense_gauss_sketch_parity(rq, orc):
 
 
 @pytest.mark.parametrize("s2,n", [(32, 16), (128, 64), (140, 70), (256, 128), (512, 256), (9, 9),
-                                  (64, 2), (300, 37)])
+                                  (64, 2), (300, 37), (789, 70), (1000, 100), (700, 30), (1024, 128), (600, 200)])
 def test_small_geqrf_parity(rq, orc, s2, n):
     rng = np.random.default_rng(s2 * 1000 + n)
     W = rng.standard_normal((s2, n)) * np.logspace(0, -10, n)
