@@ -147,7 +147,8 @@ int rqr_debug_hash_sign(uint64_t seed, int64_t row0, int64_t count, int64_t s1, 
                         int8_t* sign, void* stream);
 int rqr_debug_gauss(uint64_t seed, uint32_t stream_id, uint64_t first, int64_t count, double* z,
                     void* stream);
-/* Pointer to S2 (s2 x s1) inside a workspace prepared for (n, s1).                            */
+/* Pointer to S2 (s2 x s1) inside a workspace prepared for (n, s1).  Row r starts at r * ld with
+ * ld = s1 rounded up to a multiple of 16; the pad columns hold zeros.                         */
 const double* rqr_workspace_S2(void* work, int n, int64_t s1);
 
 /* Test hook: on != 0 forces the generic (non-DMMA) kernels in rqr_trsm_gram / rqr_apply.       */

@@ -213,7 +213,8 @@ def workspace_S2(work, n, s1, s2):
     """View of S2 (s2 x s1) inside a prepared workspace."""
     base = lib().rqr_workspace_S2(_ptr(work), n, s1)
     off = base - work.data_ptr()
-    return work[off: off + s2 * s1 * 8].view(torch.float64).view(s2, s1)
+    ld = (s1 + 15) & ~15                  # rows are padded with zeros to a multiple of 16 doubles
+    return work[off: off + s2 * ld * 8].view(torch.float64).view(s2, ld)[:, :s1]
 
 
 def force_generic(on: bool):

@@ -22,6 +22,9 @@
     } while (0)
 
 static inline size_t rqr_align256(size_t x) { return (x + 255) & ~(size_t)255; }
+// leading dimension of S2 in the workspace: s1 rounded up to 16 doubles, pad columns zero, so that every
+// row is 128-byte aligned for the bulk copies of the DMMA GEMM whatever s1 is (paper grid: odd s1)
+__host__ __device__ static inline int64_t rqr_s2_ld(int64_t s1) { return (s1 + 15) & ~(int64_t)15; }
 
 // ---------------------------------------------------------------------------------------
 // Workspace layout.  Offsets of a region depend only on
@@ -50,7 +53,7 @@ static inline RqrLayout rqr_layout(int64_t m, int n, int64_t s1)
     L.B_off = L.A_frags + RQR_PANEL_FRAG_BYTES;
     L.B_cur = L.B_off + rqr_align256((size_t)(s1 + 1) * 4);
     L.C = L.B_cur + rqr_align256((size_t)s1 * 4);
-    L.D = L.C + rqr_align256((size_t)RQR_MAX_S2 * (size_t)s1 * sizeof(double));
+    L.D = L.C + rqr_align256((size_t)RQR_MAX_S2 * (size_t)rqr_s2_ld(s1) * sizeof(double));
     L.E = L.D + rqr_align256((size_t)RQR_GAUSS_PARTIAL_ROWS * n * sizeof(double));
     L.F_W1 = L.E + rqr_align256((size_t)m * 4);
     L.F_W = L.F_W1 + rqr_align256((size_t)s1 * n * sizeof(double));

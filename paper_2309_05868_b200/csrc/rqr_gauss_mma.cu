@@ -46,7 +46,8 @@ k_gauss_gemm_mma(const double* __restrict__ S2, const double* __restrict__ W1, i
     const int m0 = blockIdx.y * 64;
     const int64_t k0 = (int64_t)blockIdx.z * kchunk;
     const int64_t k1 = (k0 + kchunk < s1) ? k0 + kchunk : s1;
-    const int nsteps = (int)((k1 - k0) / GM_KB);
+    const int nsteps = (int)((k1 - k0 + GM_KB - 1) / GM_KB);
+    const int64_t lds2 = rqr_s2_ld(s1);                 // rows of S2 are padded with zeros to a multiple of 16
     const int rows_a = (s2 - m0) < 64 ? (s2 - m0) : 64;
 
     if (warp == GM_WARPS) {
@@ -57,11 +58,14 @@ k_gauss_gemm_mma(const double* __restrict__ S2, const double* __restrict__ W1, i
             double* A = smem + (size_t)stage * Plan::stage;
             double* B = A + Plan::a_doubles;
             mbar_wait(empty + stage, ph ^ 1u);
-            if (lane == 0) mbar_expect_tx(full + stage, (uint32_t)(rows_a * GM_KB * 8 + GM_KB * n * 8));
+            // the last slice may run past s1: S2's pad columns are zero, the matching rows of the B stage
+            // keep finite data of an earlier slice (0 x finite = 0), so only the existing rows of W1 are copied
+            const int rows_b = (int)((s1 - k) < GM_KB ? (s1 - k) : GM_KB);
+            if (lane == 0) mbar_expect_tx(full + stage, (uint32_t)(rows_a * GM_KB * 8 + rows_b * n * 8));
             __syncwarp();
             for (int r = lane; r < rows_a; r += 32)
-                bulk_g2s(A + r * LDA, S2 + (int64_t)(m0 + r) * s1 + k, GM_KB * 8, full + stage);
-            if (lane < GM_KB) bulk_g2s(B + lane * LDB, W1 + (k + lane) * n, (uint32_t)(n * 8), full + stage);
+                bulk_g2s(A + r * LDA, S2 + (int64_t)(m0 + r) * lds2 + k, GM_KB * 8, full + stage);
+            if (lane < rows_b) bulk_g2s(B + lane * LDB, W1 + (k + lane) * n, (uint32_t)(n * 8), full + stage);
             if (++stage == GM_STAGES) { stage = 0; ph ^= 1u; }
         }
         return;
@@ -112,7 +116,7 @@ static int launch_gauss_mma(const double* S2, const double* W1, int64_t s1, int 
     const int tiles_m = (s2 + 63) / 64;
     int64_t ks = 296 / tiles_m;
     if (ks > ks_cap) ks = ks_cap;
-    const int64_t kblocks = s1 / GM_KB;
+    const int64_t kblocks = (s1 + GM_KB - 1) / GM_KB;
     if (ks > kblocks) ks = kblocks;
     if (ks < 1) ks = 1;
     const int64_t kchunk = ((kblocks + ks - 1) / ks) * GM_KB;
@@ -128,7 +132,7 @@ static int launch_gauss_mma(const double* S2, const double* W1, int64_t s1, int 
 int rqr_gauss_gemm_mma(const double* S2, const double* W1, int64_t s1, int n, int s2, double* part,
                        int64_t ks_cap, int* ks_out, cudaStream_t st)
 {
-    if (n < 96 || n > 256 || (n & 1) || (s1 % GM_KB) != 0) return RQR_TALL_NOT_HANDLED;
+    if (n < 96 || n > 256 || (n & 1)) return RQR_TALL_NOT_HANDLED;
     if ((((uintptr_t)S2 | (uintptr_t)W1) & 15) != 0) return RQR_TALL_NOT_HANDLED;
     if (n <= 128) return launch_gauss_mma<16>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st);
     if (n <= 192) return launch_gauss_mma<24>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st);

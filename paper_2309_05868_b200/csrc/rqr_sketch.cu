@@ -12,7 +12,7 @@ int rqr_gauss_gemm_mma(const double* S2, const double* W1, int64_t s1, int n, in
 // =========================================================================================
 
 // S2[e] = z(e) / sqrt(s2), one Box-Muller pair per thread (entries 2q, 2q+1).
-__global__ void k_gen_S2(uint64_t seed, int s2, int64_t total, double* __restrict__ S2)
+__global__ void k_gen_S2(uint64_t seed, int s2, int64_t s1, int64_t ld, int64_t total, double* __restrict__ S2)
 {
     const double d = sqrt((double)s2);
     int64_t npairs = (total + 1) >> 1;
@@ -20,9 +20,9 @@ __global__ void k_gen_S2(uint64_t seed, int s2, int64_t total, double* __restric
          q += (int64_t)gridDim.x * blockDim.x) {
         double z0, z1;
         rqr_gauss_pair(seed, (uint64_t)q, RQR_PHILOX_STREAM_S2, z0, z1);
-        int64_t e = 2 * q;
-        S2[e] = z0 / d;
-        if (e + 1 < total) S2[e + 1] = z1 / d;
+        int64_t e = 2 * q;                      // logical entry e = r * s1 + c lives at r * ld + c
+        S2[(e / s1) * ld + e % s1] = z0 / d;
+        if (e + 1 < total) S2[((e + 1) / s1) * ld + (e + 1) % s1] = z1 / d;
     }
 }
 
@@ -141,7 +141,9 @@ static int launch_prepare_S2(int64_t s1, int s2, uint64_t seed, double* S2, cuda
     int64_t npairs = (total + 1) / 2;
     int blocks = (int)((npairs + 255) / 256 < 148 * 16 ? (npairs + 255) / 256 : 148 * 16);
     if (blocks < 1) blocks = 1;
-    k_gen_S2<<<blocks, 256, 0, st>>>(seed, s2, total, S2);
+    const int64_t ld = rqr_s2_ld(s1);
+    if (ld != s1 && cudaMemsetAsync(S2, 0, (size_t)s2 * ld * sizeof(double), st) != cudaSuccess) return RQR_ERR_LAUNCH;
+    k_gen_S2<<<blocks, 256, 0, st>>>(seed, s2, s1, ld, total, S2);
     RQR_LAUNCH_CHECK();
     return RQR_OK;
 }
@@ -335,6 +337,7 @@ __global__ void __launch_bounds__(256)
 k_gauss_gemm_splitk(const double* __restrict__ S2, const double* __restrict__ W1, int64_t s1,
                     int n, int s2, int64_t kchunk, double* __restrict__ part)
 {
+    const int64_t lds2 = rqr_s2_ld(s1);
     __shared__ double As[GS_BK][GS_BM + 1];
     __shared__ double Bs[GS_BK][GS_BN];
     const int tid = threadIdx.x;
@@ -354,7 +357,7 @@ k_gauss_gemm_splitk(const double* __restrict__ S2, const double* __restrict__ W1
             int idx = tid + t * 256;
             int r = idx >> 4, k = idx & 15;
             int gr = row_base + r; int64_t gk = kk + k;
-            As[k][r] = (gr < s2 && gk < k1) ? S2[(int64_t)gr * s1 + gk] : 0.0;
+            As[k][r] = (gr < s2 && gk < k1) ? S2[(int64_t)gr * lds2 + gk] : 0.0;
         }
         // B tile: 16 k x 64 cols
 #pragma unroll

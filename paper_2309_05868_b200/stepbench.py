@@ -36,9 +36,12 @@ def main(argv=None):
     ap.add_argument("--m", type=int, default=1 << 23)
     ap.add_argument("--n", type=int, default=64)
     ap.add_argument("--reps", type=int, default=10)
+    ap.add_argument("--s1", type=int, default=0, help="CountSketch rows (default 2 n^2)")
+    ap.add_argument("--s2", type=int, default=0, help="Gaussian sketch rows (default 2 n)")
     a = ap.parse_args(argv)
     m, n, reps = a.m, a.n, a.reps
     s1, s2 = inputs.sketch_sizes(n)
+    s1, s2 = (a.s1 or s1), (a.s2 or s2)
     rq.lib()
     torch.cuda.set_device(0)
     f = dict(dtype=torch.float64, device="cuda")
