@@ -41,15 +41,18 @@ __host__ __device__ __forceinline__ void panel_slot_decode(int s, int& Pp, int& 
 
 // One CTA per slot.  off(P',P)[((J'*8+J)*2+s)*32+lane] = -R[64P'+8J'+2(lane%4)+s][64P+8J+lane/4];
 // diag(P) = the Tf / nRf arrays of build_tri_frags for the 64x64 block R[P,P].  Padded with identity.
+// last_nb = 4: the last panel is 32 columns wide (n <= 64 (NP-1) + 32); its diagonal slot holds the NB = 4
+// arrays (Tf 4*64, nRf 6*64 doubles), its off-diagonal slots are used for J < 4 only.
 __global__ void __launch_bounds__(256)
-k_build_panel_frags(const double* __restrict__ R, int n, double* __restrict__ frags)
+k_build_panel_frags(const double* __restrict__ R, int n, double* __restrict__ frags, int np, int last_nb)
 {
     __shared__ double scratch[8 * 64];
     int Pp, P;
     panel_slot_decode(blockIdx.x, Pp, P);
     double* out = frags + (size_t)blockIdx.x * PANEL_SLOT;
     if (Pp == P) {
-        build_tri_frags<8>(R, n, out, out + 512, scratch, 64 * P);
+        if (P == np - 1 && last_nb == 4) build_tri_frags<4>(R, n, out, out + 256, scratch, 64 * P);
+        else build_tri_frags<8>(R, n, out, out + 512, scratch, 64 * P);
     } else {
         for (int t = threadIdx.x; t < PANEL_SLOT; t += blockDim.x) {
             const int jj = t >> 6, h = (t >> 5) & 1, lane = t & 31;
@@ -73,7 +76,8 @@ struct PanelPlan {
 };
 
 // X = V R^-1 (npass = 1) or (V Ra^-1) Rb^-1 (npass = 2; fragment sets Ra then Rb), X -> Q.
-template <int NP, bool FULL>
+// LASTNB = 4: the last panel has 4 column blocks (n <= 64 (NP-1) + 32): its DMMAs for J >= 4 are skipped.
+template <int NP, bool FULL, int LASTNB>
 __global__ void __launch_bounds__((PANEL_WARPS + 1) * 32, 1)
 k_trsm_panel(const double* V, int64_t m, int n, int64_t ldv, const double* __restrict__ frags,
              int npass, double* Q, int64_t ldq)
@@ -178,6 +182,7 @@ k_trsm_panel(const double* V, int64_t m, int n, int64_t ldv, const double* __res
             double* gpp = (pass == npass - 1) ? gp : nullptr;
             static_for<0, NP>([&](auto Pc) {
                 constexpr int P = decltype(Pc)::value;
+                constexpr int NBP = (P == NP - 1) ? LASTNB : 8;        // column blocks of this panel
                 static_for<0, P>([&](auto Ppc) {
                     constexpr int Pp = decltype(Ppc)::value;
                     mbar_wait(full + buf, fph);
@@ -185,10 +190,10 @@ k_trsm_panel(const double* V, int64_t m, int n, int64_t ldv, const double* __res
 #pragma unroll
                     for (int Jp = 0; Jp < 8; ++Jp) {
 #pragma unroll
-                        for (int J = 0; J < 8; ++J)
+                        for (int J = 0; J < NBP; ++J)
                             dmma(x[P][J][0], x[P][J][1], x[Pp][Jp][0], B[((Jp * 8 + J) * 2 + 0) * 32]);
 #pragma unroll
-                        for (int J = 0; J < 8; ++J)
+                        for (int J = 0; J < NBP; ++J)
                             dmma(x[P][J][0], x[P][J][1], x[Pp][Jp][1], B[((Jp * 8 + J) * 2 + 1) * 32]);
                     }
                     __syncwarp();
@@ -197,8 +202,17 @@ k_trsm_panel(const double* V, int64_t m, int n, int64_t ldv, const double* __res
                 });
                 mbar_wait(full + buf, fph);
                 const double* B = Bbuf + (size_t)buf * PANEL_SLOT;
-                trsm_rowblock<8, false, false, FULL>(x[P], nullptr, nullptr, ad, B, B + 512,
-                                                     gpp ? gpp + 64 * P : nullptr, colmask[P], lane, g, G, nohook);
+                if constexpr (NBP == 8) {
+                    trsm_rowblock<8, false, false, FULL>(x[P], nullptr, nullptr, ad, B, B + 512,
+                                                         gpp ? gpp + 64 * P : nullptr, colmask[P], lane, g, G, nohook);
+                } else {
+                    double g4[4];
+                    double G4[10][2];
+                    const XsAddr<32> ad4(lane);
+                    trsm_rowblock<4, false, false, FULL>(reinterpret_cast<double (&)[4][2]>(x[P]), nullptr, nullptr, ad4,
+                                                         B, B + 256, gpp ? gpp + 64 * P : nullptr, colmask[P], lane,
+                                                         g4, G4, nohook);
+                }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(empty + buf);
                 if (++buf == 2) { buf = 0; fph ^= 1u; }
@@ -310,9 +324,11 @@ k_syrk_fold(const double* __restrict__ X, int64_t m, int n, int64_t ldx, double*
         }
         return;
     }
-    const int f = blockIdx.y * PANEL_WARPS + warp;
+    // folds are split evenly over the gridDim.y CTAs of a walker (NB = 20: 5 + 5, not 8 + 2)
+    const int fpp = (NB / 2 + (int)gridDim.y - 1) / (int)gridDim.y;
+    const int f = blockIdx.y * fpp + warp;
     double* P = part + (size_t)blockIdx.x * n * n;
-    if (f < NB / 2) {
+    if (warp < fpp && f < NB / 2) {
         syrk_dispatch<NB, 0>(f, stages, full, empty, m, ntiles, n, lane, P);
     } else {
         // no fold for this warp (NB/2 not a multiple of 8): keep the empty-barrier protocol alive
@@ -337,25 +353,37 @@ static bool panel_ok(const void* V, int n, int64_t ldv, const void* Q, int64_t l
     return true;
 }
 
-template <int NP>
-static int launch_panel(const double* V, int64_t m, int n, int64_t ldv, const double* frags, int npass,
-                        double* Q, int64_t ldq, cudaStream_t st)
+template <int NP, int LASTNB>
+static int launch_panel_w(const double* V, int64_t m, int n, int64_t ldv, const double* frags, int npass,
+                          double* Q, int64_t ldq, cudaStream_t st)
 {
     using Plan = PanelPlan<NP>;
     static_assert(Plan::bytes <= 227 * 1024, "k_trsm_panel shared memory plan too large");
     static bool attr = false;
     if (!attr) {
-        cudaFuncSetAttribute(k_trsm_panel<NP, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
-        cudaFuncSetAttribute(k_trsm_panel<NP, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
+        cudaFuncSetAttribute(k_trsm_panel<NP, true, LASTNB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
+        cudaFuncSetAttribute(k_trsm_panel<NP, false, LASTNB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
         attr = true;
     }
     const int64_t ntiles = ((m + 7) / 8 + PANEL_WARPS - 1) / PANEL_WARPS;
     const int grid = (int)(ntiles < 148 ? ntiles : 148);
     const int threads = (PANEL_WARPS + 1) * 32;
-    if (n == 64 * NP) k_trsm_panel<NP, true><<<grid, threads, Plan::bytes, st>>>(V, m, n, ldv, frags, npass, Q, ldq);
-    else              k_trsm_panel<NP, false><<<grid, threads, Plan::bytes, st>>>(V, m, n, ldv, frags, npass, Q, ldq);
+    if (n == 64 * (NP - 1) + 8 * LASTNB)
+        k_trsm_panel<NP, true, LASTNB><<<grid, threads, Plan::bytes, st>>>(V, m, n, ldv, frags, npass, Q, ldq);
+    else
+        k_trsm_panel<NP, false, LASTNB><<<grid, threads, Plan::bytes, st>>>(V, m, n, ldv, frags, npass, Q, ldq);
     RQR_LAUNCH_CHECK();
     return RQR_OK;
+}
+
+static int panel_last_nb(int n, int NP) { return n <= 64 * (NP - 1) + 32 ? 4 : 8; }
+
+template <int NP>
+static int launch_panel(const double* V, int64_t m, int n, int64_t ldv, const double* frags, int npass,
+                        double* Q, int64_t ldq, cudaStream_t st)
+{
+    return panel_last_nb(n, NP) == 4 ? launch_panel_w<NP, 4>(V, m, n, ldv, frags, npass, Q, ldq, st)
+                                     : launch_panel_w<NP, 8>(V, m, n, ldv, frags, npass, Q, ldq, st);
 }
 
 template <int NB>
@@ -381,7 +409,7 @@ static int launch_syrk(const double* X, int64_t m, int n, int64_t ldx, double* p
 
 static int build_frags(const double* R, int n, int NP, double* frags, cudaStream_t st)
 {
-    k_build_panel_frags<<<NP * (NP + 1) / 2, 256, 0, st>>>(R, n, frags);
+    k_build_panel_frags<<<NP * (NP + 1) / 2, 256, 0, st>>>(R, n, frags, NP, panel_last_nb(n, NP));
     RQR_LAUNCH_CHECK();
     return RQR_OK;
 }
@@ -405,9 +433,14 @@ int rqr_trsm_gram_panel(const double* V, int64_t m, int n, int64_t ldv, const do
         X = V1;
         ldx = ldq;
     }
-    return NP == 2 ? launch_syrk<16>(X, m, n, ldx, part, nparts, st)
-         : NP == 3 ? launch_syrk<24>(X, m, n, ldx, part, nparts, st)
-                   : launch_syrk<32>(X, m, n, ldx, part, nparts, st);
+    switch (8 * (NP - 1) + panel_last_nb(n, NP)) {        // column blocks: 12, 16, 20, 24, 28, 32
+        case 12: return launch_syrk<12>(X, m, n, ldx, part, nparts, st);
+        case 16: return launch_syrk<16>(X, m, n, ldx, part, nparts, st);
+        case 20: return launch_syrk<20>(X, m, n, ldx, part, nparts, st);
+        case 24: return launch_syrk<24>(X, m, n, ldx, part, nparts, st);
+        case 28: return launch_syrk<28>(X, m, n, ldx, part, nparts, st);
+        default: return launch_syrk<32>(X, m, n, ldx, part, nparts, st);
+    }
 }
 
 int rqr_apply_panel(const double* V, int64_t m, int n, int64_t ldv, const double* R0, const double* R1,
