@@ -246,3 +246,19 @@ def test_paper_grid_shape_and_sketch_sizes(rq, orc, m, n):
     _, Ro, io = orc.rand_cholqr(V.numpy(), s1, s2, 42)
     assert io == 0
     assert np.linalg.norm(R.cpu().numpy() - Ro) <= R_TOL * np.linalg.norm(Ro)
+
+
+@pytest.mark.parametrize("m,n", [(300007, 64), (200000, 32), (120000, 128), (140000, 256), (150000, 96)])
+def test_one_shot_is_bit_reproducible(rq, m, n):
+    """Every reduction of the sorted-variant pipeline has a fixed order (DESIGN.md sections 7, 8), so repeated runs
+    must agree bit for bit.  compute-sanitizer is closed on this pool: this is the race check that can run --
+    a race in the warp-pair staging, the fragment-slot pipeline or the partial reductions shows up as differing
+    bits between runs."""
+    s1, s2 = inputs.sketch_sizes(n)
+    Vd = inputs.make_V(m, n, 1e10, 99, device="cuda")
+    Q0, R0, info = run_rand(rq, Vd, s1, s2, 42, 0, 0, True)
+    assert info == 0 and orth_err(Q0) <= ORTH_TOL
+    for _ in range(6):
+        Q, R, info = run_rand(rq, Vd, s1, s2, 42, 0, 0, True)
+        assert info == 0
+        assert torch.equal(R, R0) and torch.equal(Q, Q0)
