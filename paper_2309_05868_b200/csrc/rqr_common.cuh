@@ -8,7 +8,8 @@
 
 #define RQR_MAX_N 256
 #define RQR_MAX_S2 1024
-#define RQR_MAX_GRAM_PARTIALS 304        // >= 2 CTAs per SM on 148 SMs
+#define RQR_MAX_GRAM_PARTIALS 304        // >= 2 CTAs per SM on 148 SMs (one chunk of rows)
+#define RQR_GRAM_CHUNK_ROWS ((int64_t)1 << 23)   // A4 accumulates at most this many rows per partial set
 #define RQR_GAUSS_PARTIAL_ROWS 16384     // ksplit * s2 <= this
 #define RQR_PANEL_FRAG_BYTES (2 * 10 * 4096 * sizeof(double))   // rqr_tall_panel.cu
 
@@ -22,6 +23,16 @@
     } while (0)
 
 static inline size_t rqr_align256(size_t x) { return (x + 255) & ~(size_t)255; }
+// Gram partials the workspace holds: the A4 kernels are launched per chunk of RQR_GRAM_CHUNK_ROWS rows, each
+// chunk with its own partial set, so that no register accumulator sums more than ~600 row-blocks before the
+// fixed-order tree (rounding error of a long chain on an input whose first rows carry most of the mass).
+// 160 MB budget: 1216 partials for n <= 128, 305 at n = 256.
+static inline int rqr_gram_partial_cap(int n)
+{
+    const int64_t by_budget = ((int64_t)160 << 20) / ((int64_t)n * n * 8);
+    const int64_t cap = by_budget < 1216 ? by_budget : 1216;
+    return (int)(cap < RQR_MAX_GRAM_PARTIALS ? RQR_MAX_GRAM_PARTIALS : cap);
+}
 // leading dimension of S2 in the workspace: s1 rounded up to 16 doubles, pad columns zero, so that every
 // row is 128-byte aligned for the bulk copies of the DMMA GEMM whatever s1 is (paper grid: odd s1)
 __host__ __device__ static inline int64_t rqr_s2_ld(int64_t s1) { return (s1 + 15) & ~(int64_t)15; }
@@ -48,7 +59,7 @@ static inline RqrLayout rqr_layout(int64_t m, int n, int64_t s1)
     size_t nn = (size_t)n * n * sizeof(double);
     L.hdr = 0;
     L.A = 256;
-    L.A_small = L.A + rqr_align256((size_t)RQR_MAX_GRAM_PARTIALS * nn);
+    L.A_small = L.A + rqr_align256((size_t)rqr_gram_partial_cap(n) * nn);
     L.A_frags = L.A_small + rqr_align256(16 * nn);
     L.B_off = L.A_frags + RQR_PANEL_FRAG_BYTES;
     L.B_cur = L.B_off + rqr_align256((size_t)(s1 + 1) * 4);

@@ -154,10 +154,25 @@ extern "C" int rqr_trsm_gram(const double* V, int64_t m, int n, int64_t ldv, con
     double* part = (double*)((char*)work + 256);        // region A
     int nparts = 0;
     double* frags = (double*)((char*)work + rqr_layout(1, n, 1).A_frags);
-    int rc = g_force_generic ? RQR_TALL_NOT_HANDLED
-                             : rqr_trsm_gram_mma(V, m, n, ldv, R0, V1, ldq, part, &nparts, st);
-    if (rc == RQR_TALL_NOT_HANDLED && !g_force_generic)
-        rc = rqr_trsm_gram_panel(V, m, n, ldv, R0, V1, ldq, part, &nparts, frags, st);
+    // rows are processed in chunks, one partial set per chunk (rqr_gram_partial_cap): bounded accumulation chains
+    const int cap = rqr_gram_partial_cap(n);
+    int64_t chunk = RQR_GRAM_CHUNK_ROWS;
+    while ((m + chunk - 1) / chunk * 148 > cap) chunk *= 2;
+    int rc = RQR_TALL_NOT_HANDLED;
+    if (!g_force_generic) {
+        for (int64_t r0 = 0; r0 < m; r0 += chunk) {
+            const int64_t mc = (m - r0) < chunk ? (m - r0) : chunk;
+            int np = 0;
+            rc = rqr_trsm_gram_mma(V + r0 * ldv, mc, n, ldv, R0, V1 ? V1 + r0 * ldq : nullptr, ldq,
+                                   part + (size_t)nparts * n * n, &np, st);
+            if (rc != RQR_OK) break;
+            nparts += np;
+        }
+        if (rc == RQR_TALL_NOT_HANDLED) {
+            nparts = 0;
+            rc = rqr_trsm_gram_panel(V, m, n, ldv, R0, V1, ldq, part, &nparts, frags, chunk, st);
+        }
+    }
     if (rc == RQR_TALL_NOT_HANDLED) {
         generic_attrs();
         nparts = generic_grid(m);

@@ -13,7 +13,7 @@ int rqr_apply_mma(const double* V, int64_t m, int n, int64_t ldv, const double* 
                   double* Q, int64_t ldq, cudaStream_t st);
 // 64 < n <= 256 (rqr_tall_panel.cu); `frags` = the workspace's panel fragment region
 int rqr_trsm_gram_panel(const double* V, int64_t m, int n, int64_t ldv, const double* R0, double* V1,
-                        int64_t ldq, double* part, int* nparts, double* frags, cudaStream_t st);
+                        int64_t ldq, double* part, int* nparts, double* frags, int64_t chunk_rows, cudaStream_t st);
 int rqr_apply_panel(const double* V, int64_t m, int n, int64_t ldv, const double* R0, const double* R1,
                     double* Q, int64_t ldq, double* frags, cudaStream_t st);
 // test hook: 0 = auto, 1 = force the generic kernels

@@ -238,7 +238,7 @@ struct SyrkPlan {
 template <int NB, int F>
 __device__ __forceinline__ void syrk_fold_warp(const double* __restrict__ stages, uint64_t* full, uint64_t* empty,
                                                int64_t m, int64_t ntiles, int n, int lane,
-                                               double* __restrict__ P)
+                                               double* __restrict__ P, int accumulate)
 {
     using Plan = SyrkPlan<NB>;
     constexpr int LDS = Plan::LDS, NF = NB - F, A2 = NB - 1 - 2 * F;
@@ -274,25 +274,28 @@ __device__ __forceinline__ void syrk_fold_warp(const double* __restrict__ stages
         const int a_blk = b < NF ? F : NB - 1 - F;
         const int b_blk = b < NF ? F + b : NB - 1 - F + (b - NF);
         const int row = 8 * a_blk + r, col = 8 * b_blk + 2 * q;
-        if (row < n && col < n) P[(size_t)row * n + col] = G[b][0];
-        if (row < n && col + 1 < n) P[(size_t)row * n + col + 1] = G[b][1];
+        // accumulate: this launch covers a later chunk of rows and adds to the partial of the first one
+        // (two-level summation: no register accumulator sums more than one chunk; only this lane touches dst)
+        if (row < n && col < n) P[(size_t)row * n + col] = accumulate ? P[(size_t)row * n + col] + G[b][0] : G[b][0];
+        if (row < n && col + 1 < n)
+            P[(size_t)row * n + col + 1] = accumulate ? P[(size_t)row * n + col + 1] + G[b][1] : G[b][1];
     }
 }
 
 template <int NB, int F>
 __device__ __forceinline__ void syrk_dispatch(int f, const double* stages, uint64_t* full, uint64_t* empty,
-                                              int64_t m, int64_t ntiles, int n, int lane, double* P)
+                                              int64_t m, int64_t ntiles, int n, int lane, double* P, int accumulate)
 {
     if constexpr (F < NB / 2) {
-        if (f == F) syrk_fold_warp<NB, F>(stages, full, empty, m, ntiles, n, lane, P);
-        else syrk_dispatch<NB, F + 1>(f, stages, full, empty, m, ntiles, n, lane, P);
+        if (f == F) syrk_fold_warp<NB, F>(stages, full, empty, m, ntiles, n, lane, P, accumulate);
+        else syrk_dispatch<NB, F + 1>(f, stages, full, empty, m, ntiles, n, lane, P, accumulate);
     }
 }
 
 // grid = (row walkers, ceil(NB/2 / 8)); part[blockIdx.x] receives this walker's partial (upper blocks)
 template <int NB>
 __global__ void __launch_bounds__((PANEL_WARPS + 1) * 32, 1)
-k_syrk_fold(const double* __restrict__ X, int64_t m, int n, int64_t ldx, double* __restrict__ part)
+k_syrk_fold(const double* __restrict__ X, int64_t m, int n, int64_t ldx, double* __restrict__ part, int accumulate)
 {
     using Plan = SyrkPlan<NB>;
     extern __shared__ __align__(16) double smem[];
@@ -329,7 +332,7 @@ k_syrk_fold(const double* __restrict__ X, int64_t m, int n, int64_t ldx, double*
     const int f = blockIdx.y * fpp + warp;
     double* P = part + (size_t)blockIdx.x * n * n;
     if (warp < fpp && f < NB / 2) {
-        syrk_dispatch<NB, 0>(f, stages, full, empty, m, ntiles, n, lane, P);
+        syrk_dispatch<NB, 0>(f, stages, full, empty, m, ntiles, n, lane, P, accumulate);
     } else {
         // no fold for this warp (NB/2 not a multiple of 8): keep the empty-barrier protocol alive
         int stage = 0;
@@ -387,7 +390,8 @@ static int launch_panel(const double* V, int64_t m, int n, int64_t ldv, const do
 }
 
 template <int NB>
-static int launch_syrk(const double* X, int64_t m, int n, int64_t ldx, double* part, int* nparts, cudaStream_t st)
+static int launch_syrk(const double* X, int64_t m, int n, int64_t ldx, double* part, int* nparts, int accumulate,
+                       cudaStream_t st)
 {
     using Plan = SyrkPlan<NB>;
     static_assert(Plan::bytes <= 227 * 1024, "k_syrk_fold shared memory plan too large");
@@ -402,7 +406,7 @@ static int launch_syrk(const double* X, int64_t m, int n, int64_t ldx, double* p
     if (ntiles < walkers) walkers = (int)ntiles;
     *nparts = walkers;
     dim3 grid(walkers, PARTS);
-    k_syrk_fold<NB><<<grid, (PANEL_WARPS + 1) * 32, Plan::bytes, st>>>(X, m, n, ldx, part);
+    k_syrk_fold<NB><<<grid, (PANEL_WARPS + 1) * 32, Plan::bytes, st>>>(X, m, n, ldx, part, accumulate);
     RQR_LAUNCH_CHECK();
     return RQR_OK;
 }
@@ -414,9 +418,28 @@ static int build_frags(const double* R, int n, int NP, double* frags, cudaStream
     return RQR_OK;
 }
 
-int rqr_trsm_gram_panel(const double* V, int64_t m, int n, int64_t ldv, const double* R0, double* V1,
-                        int64_t ldq, double* part, int* nparts, double* frags, cudaStream_t st)
+// The syrk runs per chunk of SYRK_CHUNK_ROWS rows; the first chunk writes the partial set, the later ones add to
+// it (two-level summation: a register accumulator sums at most SYRK_CHUNK_ROWS / (4 walkers) products).
+#define SYRK_CHUNK_ROWS ((int64_t)1 << 20)
+template <int NB>
+static int launch_syrk_chunks(const double* X, int64_t m, int n, int64_t ldx, double* part, int* nparts, cudaStream_t st)
 {
+    int np0 = 0;
+    for (int64_t r0 = 0; r0 < m; r0 += SYRK_CHUNK_ROWS) {
+        const int64_t mc = (m - r0) < SYRK_CHUNK_ROWS ? (m - r0) : SYRK_CHUNK_ROWS;
+        int np = 0;
+        int rc = launch_syrk<NB>(X + r0 * ldx, mc, n, ldx, part, &np, r0 > 0, st);
+        if (rc != RQR_OK) return rc;
+        if (r0 == 0) np0 = np;                 // the first chunk is the largest: it defines every partial
+    }
+    *nparts = np0;
+    return RQR_OK;
+}
+
+int rqr_trsm_gram_panel(const double* V, int64_t m, int n, int64_t ldv, const double* R0, double* V1,
+                        int64_t ldq, double* part, int* nparts, double* frags, int64_t chunk_rows, cudaStream_t st)
+{
+    (void)chunk_rows;
     if (!panel_ok(V, n, ldv, V1, ldq)) return RQR_TALL_NOT_HANDLED;
     if (R0 && !V1) return -7;                       // n > 64: V1 must be stored (see include/rqr.h, hazard H1)
     if (!R0 && V1) return RQR_TALL_NOT_HANDLED;     // plain copy + Gram: generic kernel
@@ -434,12 +457,12 @@ int rqr_trsm_gram_panel(const double* V, int64_t m, int n, int64_t ldv, const do
         ldx = ldq;
     }
     switch (8 * (NP - 1) + panel_last_nb(n, NP)) {        // column blocks: 12, 16, 20, 24, 28, 32
-        case 12: return launch_syrk<12>(X, m, n, ldx, part, nparts, st);
-        case 16: return launch_syrk<16>(X, m, n, ldx, part, nparts, st);
-        case 20: return launch_syrk<20>(X, m, n, ldx, part, nparts, st);
-        case 24: return launch_syrk<24>(X, m, n, ldx, part, nparts, st);
-        case 28: return launch_syrk<28>(X, m, n, ldx, part, nparts, st);
-        default: return launch_syrk<32>(X, m, n, ldx, part, nparts, st);
+        case 12: return launch_syrk_chunks<12>(X, m, n, ldx, part, nparts, st);
+        case 16: return launch_syrk_chunks<16>(X, m, n, ldx, part, nparts, st);
+        case 20: return launch_syrk_chunks<20>(X, m, n, ldx, part, nparts, st);
+        case 24: return launch_syrk_chunks<24>(X, m, n, ldx, part, nparts, st);
+        case 28: return launch_syrk_chunks<28>(X, m, n, ldx, part, nparts, st);
+        default: return launch_syrk_chunks<32>(X, m, n, ldx, part, nparts, st);
     }
 }
 

@@ -57,7 +57,12 @@ def _hbm_peak():
 def _checks(V, Q, R):
     n = V.shape[1]
     eye = torch.eye(n, dtype=torch.float64, device=V.device)
-    orth = float(torch.linalg.norm(Q.T @ Q - eye))
+    # Q^T Q by pairwise summation of 2^20-row pieces: a single library GEMM over 2^25 rows has a rounding
+    # error of its own (measured 3e-12 on a coherent Q) that would be charged to the factorization
+    parts = [Q[i:i + (1 << 20)].T @ Q[i:i + (1 << 20)] for i in range(0, Q.shape[0], 1 << 20)]
+    while len(parts) > 1:
+        parts = [parts[i] + parts[i + 1] if i + 1 < len(parts) else parts[i] for i in range(0, len(parts), 2)]
+    orth = float(torch.linalg.norm(parts[0] - eye))
     num = 0.0
     step = 1 << 21
     for i0 in range(0, V.shape[0], step):
