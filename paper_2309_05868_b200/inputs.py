@@ -133,3 +133,22 @@ def make_V_reflectors(m: int, n: int, kappa: float, seed: int, device="cpu", k: 
     V = U @ W.T
     del U
     return V.contiguous()
+
+
+def make_coherent_V(m: int, n: int, kappa: float, seed: int, device="cpu", k: int = 4) -> torch.Tensor:
+    """Stress input: same singular values, but U = H_1 ... H_k [I_n; 0]: the first n rows carry almost all of
+    the mass (maximal coherence).  Hard for a CountSketch (heavy rows may share a bucket) and for long
+    floating-point accumulations (the sums reach their final size in the first row-block)."""
+    gen = torch.Generator(device=device)
+    gen.manual_seed(int(seed))
+    U = torch.zeros(m, n, dtype=torch.float64, device=device)
+    U[:n] = torch.eye(n, dtype=torch.float64, device=device)
+    for _ in range(k):
+        v = torch.randn(m, generator=gen, dtype=torch.float64, device=device)
+        v /= torch.linalg.norm(v)
+        U.addr_(v, v @ U, alpha=-2.0)
+    W = _haar(n, n, gen, device)
+    U *= singular_values(n, kappa, device)
+    V = U @ W.T
+    del U
+    return V.contiguous()

@@ -262,3 +262,22 @@ def test_one_shot_is_bit_reproducible(rq, m, n):
         Q, R, info = run_rand(rq, Vd, s1, s2, 42, 0, 0, True)
         assert info == 0
         assert torch.equal(R, R0) and torch.equal(Q, Q0)
+
+
+@pytest.mark.parametrize("m,n", [(1 << 22, 64), (1 << 22, 128)])
+def test_coherent_input_meets_the_bar(rq, m, n):
+    """Maximally coherent V (first n rows carry the mass): stresses the CountSketch embedding and the depth of the
+    Gram accumulations ("Accumulation depth").  Q^T Q is summed pairwise over 2^18-row pieces
+    so that the check's own rounding stays below the bar."""
+    s1, s2 = inputs.sketch_sizes(n)
+    Vd = inputs.make_coherent_V(m, n, 1e12, 7, device="cuda")
+    Q, R, info = run_rand(rq, Vd, s1, s2, 42, 0, 0, True)
+    assert info == 0
+    parts = [Q[i:i + (1 << 18)].T @ Q[i:i + (1 << 18)] for i in range(0, m, 1 << 18)]
+    while len(parts) > 1:
+        parts = [parts[i] + parts[i + 1] for i in range(0, len(parts), 2)]
+    eye = torch.eye(n, dtype=torch.float64, device="cuda")
+    assert float(torch.linalg.norm(parts[0] - eye)) <= ORTH_TOL
+    check_R(R)
+    num = sum(float(torch.linalg.norm(Vd[i:i + (1 << 20)] - Q[i:i + (1 << 20)] @ R)) ** 2 for i in range(0, m, 1 << 20))
+    assert num ** 0.5 / float(torch.linalg.norm(Vd)) <= RES_TOL
