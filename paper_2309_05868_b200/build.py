@@ -24,17 +24,21 @@ def _stale() -> bool:
 def build_lib(force: bool = False, verbose: bool = False) -> str:
     if not force and not _stale():
         return LIB
-    objs = []
     os.makedirs(os.path.join(HERE, "build"), exist_ok=True)
-    log = []
-    for src in SOURCES:
+
+    def compile_one(src):
         obj = os.path.join(HERE, "build", src.replace(".cu", ".o"))
         cmd = ["nvcc", *NVCC_FLAGS, "-c", os.path.join(CSRC, src), "-o", obj]
         r = subprocess.run(cmd, capture_output=True, text=True)
-        log.append(r.stderr)
         if r.returncode != 0:
             raise RuntimeError("nvcc failed for %s:\n%s" % (src, r.stderr))
-        objs.append(obj)
+        return obj, r.stderr
+
+    from concurrent.futures import ThreadPoolExecutor
+    with ThreadPoolExecutor(max_workers=min(len(SOURCES), os.cpu_count() or 1)) as ex:
+        done = list(ex.map(compile_one, SOURCES))
+    objs = [o for o, _ in done]
+    log = [e for _, e in done]
     cmd = ["nvcc", "-shared", "-o", LIB, *objs, "-gencode", "arch=compute_100a,code=sm_100a"]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
