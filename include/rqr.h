@@ -136,6 +136,13 @@ int rqr_scholqr3(const double* V, int64_t m, int n, double* Q, double* R, void* 
  * generated on the fly).                                             */
 int rqr_gauss_randcholqr(const double* V, int64_t m, int n, int s, uint64_t seed, double* Q,
                          double* R, void* work, int* d_info, void* stream);
+/* rand_cholQR with ONE CountSketch (the paper's "Sparse" rows): R0 = R factor of the
+ * Householder QR of the s1 x n sketch W1 = S1 V itself, computed by a TSQR tree.  n <= 64 in this version.   */
+int rqr_count_randcholqr(const double* V, int64_t m, int n, int64_t s1, uint64_t seed, double* Q,
+                         double* R, void* work, int* d_info, int variant, int flags, void* stream);
+/* R factor (n x n upper, diag > 0) of the Householder QR of a tall A (rows x n row-major, ld n, n <= 64,
+ * rows >= n) by a TSQR tree of 128-row blocks; A is not modified; `work` as for the other calls.            */
+int rqr_tsqr_r(const double* A, int64_t rows, int n, double* R, void* work, int* d_info, void* stream);
 /* The dense sketch step alone: W (s x n) = S V for rows [row0, row0+m) of m_total.           */
 int rqr_dense_gauss_sketch(const double* V, int64_t m, int n, int64_t ldv, int64_t row0,
                            int64_t m_total, int s, uint64_t seed, double* W, void* work,

@@ -42,6 +42,8 @@ SIGNATURES = {
     "rqr_cholqr2": (_int, [_vp, _i64, _int, _vp, _vp, _vp, _vp, _vp]),
     "rqr_scholqr3": (_int, [_vp, _i64, _int, _vp, _vp, _vp, _vp, _vp]),
     "rqr_gauss_randcholqr": (_int, [_vp, _i64, _int, _int, _u64, _vp, _vp, _vp, _vp, _vp]),
+    "rqr_count_randcholqr": (_int, [_vp, _i64, _int, _i64, _u64, _vp, _vp, _vp, _vp, _int, _int, _vp]),
+    "rqr_tsqr_r": (_int, [_vp, _i64, _int, _vp, _vp, _vp, _vp]),
     "rqr_dense_gauss_sketch": (_int, [_vp, _i64, _int, _i64, _i64, _i64, _int, _u64, _vp, _vp, _vp]),
     "rqr_debug_hash_sign": (_int, [_u64, _i64, _i64, _i64, _vp, _vp, _vp]),
     "rqr_debug_gauss": (_int, [_u64, _u32, _u64, _i64, _vp, _vp]),
@@ -188,6 +190,19 @@ def gauss_randcholqr(V, s, seed, Q, R, work, info):
     assert V.is_contiguous() and Q.is_contiguous()
     _chk(lib().rqr_gauss_randcholqr(_ptr(_f64(V, "V")), m, n, s, seed, _ptr(Q), _ptr(R), _ptr(work), _ptr(info),
                                     _stream()), "rqr_gauss_randcholqr")
+
+
+def count_randcholqr(V, s1, seed, Q, R, work, info, variant=VARIANT_SORTED, flags=0):
+    m, n = V.shape
+    assert V.is_contiguous() and Q.is_contiguous()
+    _chk(lib().rqr_count_randcholqr(_ptr(_f64(V, "V")), m, n, s1, seed, _ptr(Q), _ptr(R), _ptr(work), _ptr(info),
+                                    variant, flags, _stream()), "rqr_count_randcholqr")
+
+
+def tsqr_r(A, R, work, info=None):
+    rows, n = A.shape
+    assert A.is_contiguous()
+    _chk(lib().rqr_tsqr_r(_ptr(_f64(A, "A")), rows, n, _ptr(R), _ptr(work), _ptr(info), _stream()), "rqr_tsqr_r")
 
 
 def dense_gauss_sketch(V, s, seed, W, work, row0=0, m_total=None):

@@ -6,6 +6,7 @@
 int rqr_chol_dev(const double* G, int n, double shift, const double* d_shift, double* R1,
                  int* d_info, cudaStream_t st, const double* Rprev, double* Rprod);
 int rqr_scholqr3_shift(const double* G, int n, int64_t m, double* d_out, cudaStream_t st);
+int rqr_tsqr_r_dev(const double* A, int64_t rows, int n, double* R, double* scratch, int* d_info, cudaStream_t st);
 
 extern "C" const char* rqr_version(void) { return "rqr 0.1 (sm_100a)"; }
 
@@ -99,6 +100,44 @@ extern "C" int rqr_gauss_randcholqr(const double* V, int64_t m, int n, int s, ui
     RQR_TRY(rqr_dense_gauss_sketch(V, m, n, n, 0, m, s, seed, W, work, st));
     RQR_TRY(rqr_small_geqrf(W, s, n, R0, d_info, st));
     RQR_TRY(tail_cholqr(V, m, n, R0, Q, R1, G, work, d_info, 0, st, R));
+    return RQR_OK;
+}
+
+// rows the TSQR scratch (region A of the workspace) can take
+static int64_t tsqr_max_rows(int n) { return (int64_t)128 * rqr_gram_partial_cap(n) * 2 / 3; }
+
+extern "C" int rqr_tsqr_r(const double* A, int64_t rows, int n, double* R, void* work, int* d_info, void* stream)
+{
+    if (!A) return -1;
+    if (n < 2 || n > 64) return -3;
+    if (rows < n || rows > tsqr_max_rows(n)) return -2;
+    if (!R) return -4;
+    if (!work) return -5;
+    return rqr_tsqr_r_dev(A, rows, n, R, (double*)((char*)work + 256), d_info, (cudaStream_t)stream);
+}
+
+// rand_cholQR with ONE CountSketch (the paper's "Sparse" rows, Tables 1-3): R0 is the R
+// factor of the Householder QR of the s1 x n sketch W1 itself -- the O(n^2)-row factorization that the second,
+// Gaussian, sketch of the multisketch avoids.  Here it is a TSQR tree (n <= 64).
+extern "C" int rqr_count_randcholqr(const double* V, int64_t m, int n, int64_t s1, uint64_t seed, double* Q,
+                                    double* R, void* work, int* d_info, int variant, int flags, void* stream)
+{
+    int rc = check_common(V, m, n, Q, R, work);
+    if (rc == -100) return !Q ? -6 : (!R ? -7 : -8);
+    if (rc != RQR_OK) return rc;
+    if (n > 64) return -3;
+    if (s1 < n || s1 >= ((int64_t)1 << 31) || s1 > m || s1 > tsqr_max_rows(n)) return -4;
+    if (variant != RQR_VARIANT_SORTED && variant != RQR_VARIANT_SCATTER) return -10;
+    cudaStream_t st = (cudaStream_t)stream;
+    RqrLayout L = rqr_layout(m, n, s1);
+    double* R0 = small_mat(work, L, n, RQR_SM_R0);
+    double* R1 = small_mat(work, L, n, RQR_SM_R1);
+    double* G = small_mat(work, L, n, RQR_SM_G);
+    double* W1 = (double*)((char*)work + L.F_W1);
+    if (d_info && cudaMemsetAsync(d_info, 0, sizeof(int), st) != cudaSuccess) return RQR_ERR_LAUNCH;
+    RQR_TRY(rqr_countsketch(V, m, n, n, 0, s1, seed, W1, work, variant, flags & RQR_FLAG_PREPARED, st));
+    RQR_TRY(rqr_tsqr_r_dev(W1, s1, n, R0, (double*)((char*)work + 256), d_info, st));
+    RQR_TRY(tail_cholqr(V, m, n, R0, Q, R1, G, work, d_info, flags & RQR_FLAG_RECOMPUTE_V1, st, R));
     return RQR_OK;
 }
 

@@ -47,7 +47,8 @@ __host__ __device__ static inline int64_t rqr_s2_ld(int64_t s1) { return (s1 + 1
 //   C  S2 slot         f(s1)     sized for s2 = RQR_MAX_S2
 //   D  gauss partials  f(n)
 //   E  sorted rows     f(m)      m u32 (row | sign<<31)
-//   F  one-shot        W1 (s1 x n), W (s2max x n)
+//   W  one-shot W      (s2max x n), in the n-only part (before B)
+//   F  one-shot W1     (s1 x n)
 // ---------------------------------------------------------------------------------------
 struct RqrLayout {
     size_t hdr, A, A_small, A_frags, B_off, B_cur, C, D, E, F_W1, F_W, total;
@@ -61,14 +62,16 @@ static inline RqrLayout rqr_layout(int64_t m, int n, int64_t s1)
     L.A = 256;
     L.A_small = L.A + rqr_align256((size_t)rqr_gram_partial_cap(n) * nn);
     L.A_frags = L.A_small + rqr_align256(16 * nn);
-    L.B_off = L.A_frags + RQR_PANEL_FRAG_BYTES;
+    // W (s2 x n) of the one-shot drivers sits in the n-only part: rqr_gauss_randcholqr and rqr_cholqr2 do not
+    // know s1, and nothing they write may land on the prepared sketch state (regions B, C, E)
+    L.F_W = L.A_frags + RQR_PANEL_FRAG_BYTES;
+    L.B_off = L.F_W + rqr_align256((size_t)RQR_MAX_S2 * n * sizeof(double));
     L.B_cur = L.B_off + rqr_align256((size_t)(s1 + 1) * 4);
     L.C = L.B_cur + rqr_align256((size_t)s1 * 4);
     L.D = L.C + rqr_align256((size_t)RQR_MAX_S2 * (size_t)rqr_s2_ld(s1) * sizeof(double));
     L.E = L.D + rqr_align256((size_t)RQR_GAUSS_PARTIAL_ROWS * n * sizeof(double));
     L.F_W1 = L.E + rqr_align256((size_t)m * 4);
-    L.F_W = L.F_W1 + rqr_align256((size_t)s1 * n * sizeof(double));
-    L.total = L.F_W + rqr_align256((size_t)RQR_MAX_S2 * n * sizeof(double));
+    L.total = L.F_W1 + rqr_align256((size_t)s1 * n * sizeof(double));
     return L;
 }
 

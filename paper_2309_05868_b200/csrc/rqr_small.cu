@@ -213,8 +213,8 @@ __device__ __forceinline__ void geqrf_g8_steps(double (&a)[2][16], int n, int w,
     }
 }
 
-__global__ void __launch_bounds__(256, 1)
-k_geqrf_g8(const double* __restrict__ W, int s2, int n, double* __restrict__ R0, int* d_info)
+__device__ __forceinline__ void geqrf_g8_body(const double* __restrict__ W, int s2, int n, double* __restrict__ R0,
+                                              int* d_info)
 {
     __shared__ double vbuf[2][128];
     __shared__ double den_s[2], sgn_s[2];
@@ -233,6 +233,47 @@ k_geqrf_g8(const double* __restrict__ W, int s2, int n, double* __restrict__ R0,
         if (c < i) R0[e] = 0.0;
     }
     geqrf_g8_steps<0>(a, n, w, lane, vbuf, den_s, sgn_s, R0, d_info);
+}
+
+__global__ void __launch_bounds__(256, 1)
+k_geqrf_g8(const double* __restrict__ W, int s2, int n, double* __restrict__ R0, int* d_info)
+{
+    geqrf_g8_body(W, s2, n, R0, d_info);
+}
+
+// One level of a TSQR tree: block b = rows [b rows/nb, (b+1) rows/nb) of A (at most 128 each), its R
+// factor goes to Rout + b n^2.  A rank-deficient BLOCK is not an error of the tree: d_info is NULL
+// except at the root.
+__global__ void __launch_bounds__(256, 1)
+k_geqrf_g8_batched(const double* __restrict__ A, int64_t rows, int nb, int n, double* __restrict__ Rout)
+{
+    const int64_t r0 = (int64_t)blockIdx.x * rows / nb, r1 = (int64_t)(blockIdx.x + 1) * rows / nb;
+    geqrf_g8_body(A + r0 * n, (int)(r1 - r0), n, Rout + (int64_t)blockIdx.x * n * n, nullptr);
+}
+
+// R factor of the Householder QR of a TALL matrix A (rows x n, n <= 64, any rows >= n) by a TSQR tree of
+// k_geqrf_g8 blocks: level by level, blocks of at most 128 rows are reduced to their n x n R factors, which are
+// stacked and reduced again.  R (diag > 0) is unique, so the tree gives the R of plain Householder QR to rounding.
+// `scratch` holds the stacked R factors of two consecutive levels: 1.5 * ceil(rows / 128) * n * n doubles.
+int rqr_tsqr_r_dev(const double* A, int64_t rows, int n, double* R, double* scratch, int* d_info, cudaStream_t st)
+{
+    const double* in = A;
+    int64_t rows_in = rows;
+    double* out = scratch;
+    double* other = scratch + ((rows + 127) / 128) * (int64_t)n * n;
+    for (;;) {
+        const int64_t nb = (rows_in + 127) / 128;
+        if (nb <= 1) {
+            k_geqrf_g8<<<1, 256, 0, st>>>(in, (int)rows_in, n, R, d_info);
+            RQR_LAUNCH_CHECK();
+            return RQR_OK;
+        }
+        k_geqrf_g8_batched<<<(unsigned)nb, 256, 0, st>>>(in, rows_in, (int)nb, n, out);
+        RQR_LAUNCH_CHECK();
+        in = out;
+        rows_in = nb * n;
+        double* t = out; out = other; other = t;
+    }
 }
 
 // Generic fallback, any 2 <= n <= 256, s2 <= 512: W stays in global memory (L2-resident) and is

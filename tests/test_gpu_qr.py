@@ -281,3 +281,54 @@ def test_coherent_input_meets_the_bar(rq, m, n):
     check_R(R)
     num = sum(float(torch.linalg.norm(Vd[i:i + (1 << 20)] - Q[i:i + (1 << 20)] @ R)) ** 2 for i in range(0, m, 1 << 20))
     assert num ** 0.5 / float(torch.linalg.norm(Vd)) <= RES_TOL
+
+
+@pytest.mark.parametrize("m,n,kappa", [(65536, 64, 1e12), (40000, 32, 1e14), (20000, 16, 1e10), (100000, 50, 1e8)])
+def test_single_countsketch_rand_cholqr(rq, orc, m, n, kappa):
+    """SURVEY.md 8(f) N3, the paper's "Sparse" rows: rand_cholQR with ONE CountSketch, R0 from
+    the Householder QR of the s1 x n sketch (a TSQR tree on the GPU).  Oracle: the same steps composed from the
+    oracle's functions (CountSketch, plain Householder R, substitution, Gram, Cholesky, substitution, product)."""
+    s1 = 2 * n * n
+    V = inputs.make_V(m, n, kappa, 606)
+    Vd = V.cuda()
+    Q = torch.empty_like(Vd)
+    R = torch.empty(n, n, dtype=torch.float64, device="cuda")
+    work = rq.alloc_workspace(m, n, s1, 2 * n)
+    info = rq.new_info()
+    rq.count_randcholqr(Vd, s1, 42, Q, R, work, info)
+    torch.cuda.synchronize()
+    assert int(info.item()) == 0
+    assert orth_err(Q) <= ORTH_TOL and resid(Vd, Q, R) <= RES_TOL
+    check_R(R)
+    Vh = V.numpy()
+    R0, i0 = orc.hhqr_r(orc.countsketch(Vh, s1, 42))
+    V1 = orc.trsm(Vh, R0)
+    R1, i1 = orc.chol(orc.gram(V1))
+    Ro = orc.triu_mul(R1, R0)
+    assert i0 == 0 and i1 == 0
+    assert np.linalg.norm(R.cpu().numpy() - Ro) <= R_TOL * np.linalg.norm(Ro)
+    assert np.linalg.cond(R1) < 100                      # kappa(V1) = O(1) with one sketch too (Cor. 5.2, PAPER.md:837-839)
+
+
+def test_prepared_sketch_survives_the_comparators(rq):
+    """The comparators share the workspace with a prepared Count-Gauss sketch (bench.py and the sweep call them
+    back to back): nothing they write may land on the sketch state.  (Regression: the single-Gaussian driver's W
+    used to be placed by a layout computed without s1 and overwrote the bucket offsets.)"""
+    m, n = 200000, 32
+    s1, s2 = inputs.sketch_sizes(n)
+    Vd = inputs.make_V(m, n, 1e6, 11, device="cuda")
+    Q = torch.empty_like(Vd); R = torch.empty(n, n, dtype=torch.float64, device="cuda")
+    Q2 = torch.empty_like(Vd); R2 = torch.empty_like(R)
+    work = rq.alloc_workspace(m, n, s1, s2)
+    info = rq.new_info()
+    rq.sketch_prepare(m, n, s1, s2, 42, work)
+    rq.rand_cholqr(Vd, s1, s2, 42, Q, R, work, info, 0, rq.FLAG_PREPARED)
+    rq.gauss_randcholqr(Vd, s2, 42, Q2, R2, work, info)
+    rq.cholqr2(Vd, Q2, R2, work, info)
+    rq.scholqr3(Vd, Q2, R2, work, info)
+    rq.count_randcholqr(Vd, s1, 42, Q2, R2, work, info, 0, rq.FLAG_PREPARED)
+    assert int(info.item()) == 0 and orth_err(Q2) <= ORTH_TOL
+    rq.rand_cholqr(Vd, s1, s2, 42, Q2, R2, work, info, 0, rq.FLAG_PREPARED)
+    torch.cuda.synchronize()
+    assert int(info.item()) == 0
+    assert torch.equal(R, R2) and torch.equal(Q, Q2)

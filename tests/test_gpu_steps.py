@@ -253,3 +253,24 @@ def test_triu_mul_parity(rq, orc, n):
     Ro = orc.triu_mul(R1.numpy(), R0.numpy())
     assert np.abs(host(R) - Ro).max() <= 1e-15 * n * np.abs(Ro).max()
     assert np.array_equal(np.tril(host(R), -1), np.zeros((n, n)))
+
+
+@pytest.mark.parametrize("rows,n", [(8192, 64), (2048, 32), (5000, 64), (129, 64), (128, 64), (1000, 16), (34277, 64),
+                                    (77, 8)])
+def test_tsqr_r_matches_householder(rq, orc, rows, n):
+    """TSQR tree of 128-row Householder blocks vs the oracle's plain Householder QR of the whole matrix: R with a
+    positive diagonal is unique, so the two agree norm-wise to rounding (graded columns: kappa ~ 1e10)."""
+    rng = np.random.default_rng(rows + n)
+    A = rng.standard_normal((rows, n)) * np.logspace(0, -10, n)
+    R = torch.full((n, n), np.nan, dtype=torch.float64, device="cuda")
+    work = rq.alloc_workspace(max(rows, 2 * n * n), n, max(rows, n), 2 * n)
+    info = rq.new_info()
+    Ad = dev(A)
+    rq.tsqr_r(Ad, R, work, info)
+    Ro, io = orc.hhqr_r(A)
+    assert int(info.item()) == 0 and io == 0
+    Rh = host(R)
+    assert np.array_equal(host(Ad), A)                      # A is not modified
+    assert np.array_equal(np.tril(Rh, -1), np.zeros_like(Rh)) and (np.diag(Rh) > 0).all()
+    assert np.linalg.norm(Rh - Ro) <= 1e-13 * np.linalg.norm(Ro)
+    assert np.all(np.linalg.norm(Rh - Ro, axis=1) <= 1e-11 * np.linalg.norm(Ro, axis=1) + 1e-300)
