@@ -99,12 +99,14 @@ class ClockSampler(threading.Thread):
         return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons)}
 
 
-def launches_per_step(n):
+def launches_per_step(n, m=0):
     """Kernels of ours launched by one rqr_rand_cholqr with a prepared sketch (sorted variant, stored V1):
     countsketch 1, Gaussian GEMM + reduce 2, Householder 1, A4 2 (n <= 64: fused kernel + partial reduce) or
     4 (n > 64: fragment build, panel substitution, syrk, reduce), Cholesky 1 (the product R = R1 R0 is fused into
     it for n <= 128; a separate launch above), A6 1 (n > 64: + fragment build)."""
-    return 8 if n <= 64 else (11 if n <= 128 else 12)
+    if n <= 64:
+        return 8 + max(0, -(-m // (1 << 23)) - 1)          # one more A4 launch per further 2^23-row chunk
+    return (11 if n <= 128 else 12) + max(0, -(-m // (1 << 20)) - 1)   # the syrk runs per 2^20-row chunk
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
@@ -391,7 +393,7 @@ def main():
             "cholqr2_ms": main_out["cholqr2_ms"], "cholqr2_info": main_out["cholqr2_info"],
             "sketch_gen_ms": main_out["sketch_gen_ms"], "breakdown_ms": bd,
             "fp64_peak_tflops": p64s, "e2e": main_out.get("e2e"),
-            "gpu_launches": launches_per_step(n) * args.steps, "roofline": roof, "cpu_baseline": cpu,
+            "gpu_launches": launches_per_step(n, m) * args.steps, "roofline": roof, "cpu_baseline": cpu,
             "clocks": sampler.summary(), "extra": extra}
     print(json.dumps(line))
 
@@ -435,7 +437,7 @@ def run_sharded(torch, rq, args, world, rank):
                 "config": {"workload": args.workload, "m_per_gpu": m, "m_total": m_total, "n": n, "s1": s1, "s2": s2,
                            "parallelism": "row-sharded, 2 all-reduces (W, G) per step",
                            "l2": "inputs_exceed_L2"},
-                "gpu_launches": (launches_per_step(n) + 1) * args.steps,      # step entry points: A7 is its own launch
+                "gpu_launches": (launches_per_step(n, m) + 1) * args.steps,      # step entry points: A7 is its own launch
                 "info": int(bufs["info"].item()), "orth_err": orth}
         print(json.dumps(line))
 
