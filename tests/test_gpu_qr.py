@@ -332,3 +332,56 @@ def test_prepared_sketch_survives_the_comparators(rq):
     torch.cuda.synchronize()
     assert int(info.item()) == 0
     assert torch.equal(R, R2) and torch.equal(Q, Q2)
+
+
+def _fuzz_cases(count, seed):
+    rng = np.random.default_rng(seed)
+    cases = []
+    while len(cases) < count:
+        kind = rng.integers(0, 4)
+        if kind == 0:
+            n = int(rng.integers(1, 33)) * 2                      # even, <= 64: fused kernels
+        elif kind == 1:
+            n = int(rng.integers(33, 129)) * 2                    # even, 66..256: panel kernels
+        elif kind == 2:
+            n = int(rng.integers(2, 40)) | 1                      # odd: generic kernels
+        else:
+            n = int(rng.choice([8, 16, 24, 32, 48, 64, 96, 128, 160, 192, 224, 256]))
+        # sketch sizes in the regime of the paper: s2 = O(n), s1 = O(n^2)
+        s2 = int(rng.integers((3 * n + 1) // 2, min(1024, 4 * n) + 1))
+        s1 = int(rng.integers(max(s2, n * n // 2), 4 * n * n + 1))
+        m_hi = 40000 if (n & 1) else (300000 if n <= 128 else 120000)
+        if s1 >= m_hi:
+            continue
+        m = int(rng.integers(max(s1, n), m_hi + 1))
+        kappa = float(10.0 ** rng.uniform(0, 12))
+        cases.append((m, n, s1, s2, kappa, int(rng.integers(0, 2)), int(rng.integers(0, 2)), int(rng.integers(1, 1 << 30))))
+    return cases
+
+
+@pytest.mark.parametrize("case", _fuzz_cases(36, 20260101), ids=lambda c: "m%d-n%d-s1_%d-s2_%d" % c[:4])
+def test_random_shapes_meet_the_invariants(rq, case):
+    """Seeded random shapes, sketch sizes, variants and flags: every one must satisfy Thm 5.3's bounds
+    and the structure of R.  Catches what the hand-picked shapes miss (ragged tiles, odd n, s1 not a multiple of
+    anything, tall sketches, the narrow last panel, workspace layout mistakes)."""
+    m, n, s1, s2, kappa, variant, recompute, seed = case
+    Vd = inputs.make_V(m, n, kappa, seed % 9973, device="cuda")
+    flags = rq.FLAG_RECOMPUTE_V1 if recompute else 0
+    Q, R, info = run_rand(rq, Vd, s1, s2, seed, variant, flags, bool(seed & 1))
+    assert info == 0
+    assert orth_err(Q) <= ORTH_TOL
+    assert resid(Vd, Q, R) <= RES_TOL
+    check_R(R)
+    # in place, same workspace reused after a comparator ran on it
+    work = rq.alloc_workspace(m, n, s1, s2)
+    info_t = rq.new_info()
+    Q2 = torch.empty_like(Vd); R2 = torch.empty_like(R)
+    rq.cholqr2(Vd, Q2, R2, work, info_t)
+    Vc = Vd.clone()
+    rq.rand_cholqr(Vc, s1, s2, seed, Vc, R2, work, info_t, variant, flags)
+    torch.cuda.synchronize()
+    assert int(info_t.item()) == 0
+    if variant == 0:
+        assert torch.equal(Vc, Q) and torch.equal(R2, R)
+    else:
+        assert orth_err(Vc) <= ORTH_TOL
