@@ -21,7 +21,10 @@
 // (blockIdx.y) to hold all folds: they walk the same row tiles, the second read hits L2.
 #include "rqr_mma.cuh"
 
-#define PANEL_WARPS 8        // consumer warps; warp PANEL_WARPS is the producer
+#define PANEL_WARPS 8        // consumer warps of k_syrk_fold; warp PANEL_WARPS is the producer
+#ifndef PANEL_CW_WIDE
+#define PANEL_CW_WIDE 11     // consumer warps of k_trsm_panel for NP = 2 (PanelPlan)
+#endif
 #define PANEL_SLOT 4096      // doubles per fragment slot (32 KB)
 #define PANEL_DIAG 2304      // doubles used by a diagonal slot: Tf (8*64) + nRf (28*64)
 #define SYRK_TR 32           // rows per tile of k_syrk_fold
@@ -64,21 +67,25 @@ k_build_panel_frags(const double* __restrict__ R, int n, double* __restrict__ fr
 
 template <int NP>
 struct PanelPlan {
+    // consumer warps of k_trsm_panel: 11 (+ the producer = 3 per SM sub-partition, 170 registers each) at NP = 2
+    // (measured at 2^21 rows: n = 128 A6 1.196 -> 1.157 ms, n = 96 0.755 -> 0.706 ms), 8 above (NP = 3: 2.46 vs
+    // 2.49 ms with 11; NP = 4: one 8 x 264-double landing block per warp is 17 KB)
+    static constexpr int CW = (NP == 2) ? PANEL_CW_WIDE : 8;
     static constexpr int N8 = 64 * NP;
     static constexpr int LDL = N8 + LDL_PAD;
     static constexpr int STEPS = NP * (NP + 1) / 2;
-    static constexpr int LSTAGES = (NP <= 2) ? 2 : 1;
-    static constexpr int NBARS = 4 + PANEL_WARPS * LSTAGES;       // full[2], empty[2], landing
+    static constexpr int LSTAGES = (NP <= 2 && CW <= 8) ? 2 : 1;
+    static constexpr int NBARS = 4 + CW * LSTAGES;       // full[2], empty[2], landing
     static constexpr size_t bars = 2 * PANEL_SLOT;                // doubles
     static constexpr size_t ring = bars + ((NBARS + 1) & ~1);
-    static constexpr size_t ring_doubles = (size_t)PANEL_WARPS * LSTAGES * 8 * LDL;
+    static constexpr size_t ring_doubles = (size_t)CW * LSTAGES * 8 * LDL;
     static constexpr size_t bytes = (ring + ring_doubles) * sizeof(double);
 };
 
 // X = V R^-1 (npass = 1) or (V Ra^-1) Rb^-1 (npass = 2; fragment sets Ra then Rb), X -> Q.
 // LASTNB = 4: the last panel has 4 column blocks (n <= 64 (NP-1) + 32): its DMMAs for J >= 4 are skipped.
 template <int NP, bool FULL, int LASTNB>
-__global__ void __launch_bounds__((PANEL_WARPS + 1) * 32, 1)
+__global__ void __launch_bounds__((PanelPlan<NP>::CW + 1) * 32, 1)
 k_trsm_panel(const double* V, int64_t m, int n, int64_t ldv, const double* __restrict__ frags,
              int npass, double* Q, int64_t ldq)
 {
@@ -95,16 +102,16 @@ k_trsm_panel(const double* V, int64_t m, int n, int64_t ldv, const double* __res
 
     for (int i = threadIdx.x; i < (int)Plan::ring_doubles; i += blockDim.x) ring[i] = 0.0;
     if (threadIdx.x < 2) mbar_init(full + threadIdx.x, 1);
-    else if (threadIdx.x < 4) mbar_init(empty + (threadIdx.x - 2), PANEL_WARPS);
+    else if (threadIdx.x < 4) mbar_init(empty + (threadIdx.x - 2), Plan::CW);
     else if (threadIdx.x < Plan::NBARS) mbar_init(bars + threadIdx.x, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     fence_proxy_async();
     __syncthreads();
 
     const int64_t nrb = (m + 7) / 8;
-    const int64_t ntiles = (nrb + PANEL_WARPS - 1) / PANEL_WARPS;
+    const int64_t ntiles = (nrb + Plan::CW - 1) / Plan::CW;
 
-    if (warp == PANEL_WARPS) {
+    if (warp == Plan::CW) {
         // producer: streams the fragment slots, in consumption order, for every tile of this CTA
         if (lane == 0) {
             int buf = 0;
@@ -135,7 +142,7 @@ k_trsm_panel(const double* V, int64_t m, int n, int64_t ldv, const double* __res
 #pragma unroll
     for (int s = 0; s < LST; ++s) {
         const int64_t t = blockIdx.x + (int64_t)s * gridDim.x;
-        if (t < ntiles && t * PANEL_WARPS + warp < nrb) wr.issue(s, t * PANEL_WARPS + warp, lane);
+        if (t < ntiles && t * Plan::CW + warp < nrb) wr.issue(s, t * Plan::CW + warp, lane);
     }
 
     double x[NP][8][2];
@@ -145,7 +152,7 @@ k_trsm_panel(const double* V, int64_t m, int n, int64_t ldv, const double* __res
     uint32_t lphase = 0, fph = 0;
     auto nohook = []() {};
     for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-        const int64_t rblk = tile * PANEL_WARPS + warp;
+        const int64_t rblk = tile * Plan::CW + warp;
         const bool active = rblk < nrb;
         int valid = 0;
         if (active) {
@@ -165,10 +172,10 @@ k_trsm_panel(const double* V, int64_t m, int n, int64_t ldv, const double* __res
                 }
             // the whole row-block is in registers: refill the stage for the tile LST rounds ahead
             const int64_t nt = tile + (int64_t)LST * gridDim.x;
-            if (nt < ntiles && nt * PANEL_WARPS + warp < nrb) {
+            if (nt < ntiles && nt * Plan::CW + warp < nrb) {
                 fence_proxy_async();
                 __syncwarp();
-                wr.issue(lstage, nt * PANEL_WARPS + warp, lane);
+                wr.issue(lstage, nt * Plan::CW + warp, lane);
             }
         } else {
 #pragma unroll
@@ -368,9 +375,9 @@ static int launch_panel_w(const double* V, int64_t m, int n, int64_t ldv, const 
         cudaFuncSetAttribute(k_trsm_panel<NP, false, LASTNB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
         attr = true;
     }
-    const int64_t ntiles = ((m + 7) / 8 + PANEL_WARPS - 1) / PANEL_WARPS;
+    const int64_t ntiles = ((m + 7) / 8 + Plan::CW - 1) / Plan::CW;
     const int grid = (int)(ntiles < 148 ? ntiles : 148);
-    const int threads = (PANEL_WARPS + 1) * 32;
+    const int threads = (Plan::CW + 1) * 32;
     if (n == 64 * (NP - 1) + 8 * LASTNB)
         k_trsm_panel<NP, true, LASTNB><<<grid, threads, Plan::bytes, st>>>(V, m, n, ldv, frags, npass, Q, ldq);
     else
