@@ -106,7 +106,7 @@ def launches_per_step(n, m=0):
     it for n <= 128; a separate launch above), A6 1 (n > 64: + fragment build)."""
     if n <= 64:
         return 8 + max(0, -(-m // (1 << 23)) - 1)          # one more A4 launch per further 2^23-row chunk
-    return (11 if n <= 128 else 12) + max(0, -(-m // (1 << 20)) - 1)   # the syrk runs per 2^20-row chunk
+    return (11 if n <= 128 else 12) + max(0, -(-m // (1 << 21)) - 1)   # the syrk runs per 2^21-row chunk
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed

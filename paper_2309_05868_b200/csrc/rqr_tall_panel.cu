@@ -427,7 +427,7 @@ static int build_frags(const double* R, int n, int NP, double* frags, cudaStream
 
 // The syrk runs per chunk of SYRK_CHUNK_ROWS rows; the first chunk writes the partial set, the later ones add to
 // it (two-level summation: a register accumulator sums at most SYRK_CHUNK_ROWS / (4 walkers) products).
-#define SYRK_CHUNK_ROWS ((int64_t)1 << 20)
+#define SYRK_CHUNK_ROWS ((int64_t)1 << 21)
 template <int NB>
 static int launch_syrk_chunks(const double* X, int64_t m, int n, int64_t ldx, double* part, int* nparts, cudaStream_t st)
 {
