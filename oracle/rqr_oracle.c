@@ -28,6 +28,9 @@
  *   gaussian          worked example, moments, Kolmogorov-Smirnov against N(0,1)
  *   countsketch       dense S1 @ V through numpy; exact integer case; column-sum identity
  *   gauss_sketch      numpy S2 @ W1
+ *   rademacher        sign bits against the Philox words spelled out, +-1/sqrt(s2) exactly, balance and
+ *                     pairwise independence of rows, E||S x||^2 = ||x||^2, embedding of a random subspace,
+ *                     numpy S2 @ W1; rand_cholqr with it: the Thm 5.3 invariants
  *   hhqr_r/hhqr_full  LAPACK QR through numpy; R^T R = W^T W
  *   trsm, chol, gram, triu_mul   scipy/numpy library routines; exact integer cases
  *   rand_cholqr       Thm 5.3 invariants over kappa = 1 .. 1e15,
@@ -213,6 +216,48 @@ void orc_gauss_sketch(const double *W1, int64_t s1, int n, int s2, uint64_t seed
     orc_gauss_matrix(seed, s2, s1, S2);
     /* loop nest r, c, j: every entry W[r,j] still receives its terms in ascending c (the
      * stated order); only the memory walk is contiguous */
+#pragma omp parallel for schedule(static)
+    for (int r = 0; r < s2; ++r) {
+        double *w = W + (int64_t)r * n;
+        for (int j = 0; j < n; ++j) w[j] = 0.0;
+        for (int64_t c = 0; c < s1; ++c) {
+            const double a = S2[(int64_t)r * s1 + c];
+            const double *b = W1 + c * n;
+            for (int j = 0; j < n; ++j) w[j] += a * b[j];
+        }
+    }
+    free(S2);
+}
+
+/* ------------------------------------------------------------------------------------
+ * N4  Dense Rademacher S2 in place of the Gaussian one (future work: "dense
+ * Rademacher sketch matrices in place of dense Gaussian sketches ... far lower storage
+ * requirements ... can be generated much more efficiently"; the analysis "is amenable to any
+ * multisketching strategy", same paragraph).  Reading S21 in DESIGN.md:
+ *   S2[r, c] = sigma(r, c) / sqrt(s2),  sigma = -1 if bit (c mod 128) of the 128-bit Philox output
+ *   o = philox(idx = r * ceil(s1 / 128) + (c div 128), stream 4) is set, else +1;  bit b of the
+ *   output is bit (b mod 32) of word o[b div 32].
+ * W = S2 W1 as in O3: W[r, j] = sum_{c ascending} S2[r, c] * W1[c, j].
+ * ---------------------------------------------------------------------------------- */
+void orc_rademacher_matrix(uint64_t seed, int s2, int64_t s1, double *S2 /* s2 x s1 */)
+{
+    const uint64_t ng = (uint64_t)((s1 + 127) / 128);
+    const double d = sqrt((double)s2);
+    for (int r = 0; r < s2; ++r)
+        for (int64_t c = 0; c < s1; ++c) {
+            uint32_t o[4];
+            philox_stream(seed, (uint64_t)r * ng + (uint64_t)(c / 128), 4u, o);
+            const int b = (int)(c % 128);
+            const int set = (int)((o[b / 32] >> (b % 32)) & 1u);
+            S2[(int64_t)r * s1 + c] = (set ? -1.0 : 1.0) / d;
+        }
+}
+
+void orc_rademacher_sketch(const double *W1, int64_t s1, int n, int s2, uint64_t seed,
+                           double *W /* s2 x n */)
+{
+    double *S2 = (double *)malloc(sizeof(double) * (size_t)s2 * (size_t)s1);
+    orc_rademacher_matrix(seed, s2, s1, S2);
 #pragma omp parallel for schedule(static)
     for (int r = 0; r < s2; ++r) {
         double *w = W + (int64_t)r * n;
@@ -431,9 +476,9 @@ static int cholqr_step(const double *A, int64_t m, int n, double shift, double *
  *   R = R1 R0.
  * Optional outputs (may be NULL): R0out, R1out (n x n), V1out (m x n), W1out, Wout.
  * ---------------------------------------------------------------------------------- */
-int orc_rand_cholqr(const double *V, int64_t m, int n, int64_t s1, int s2, uint64_t seed,
-                    double *Q, double *R, double *R0out, double *R1out, double *V1out,
-                    double *W1out, double *Wout)
+static int rand_cholqr_impl(const double *V, int64_t m, int n, int64_t s1, int s2, uint64_t seed,
+                           double *Q, double *R, double *R0out, double *R1out, double *V1out,
+                           double *W1out, double *Wout, int rademacher)
 {
     double *W1 = (double *)malloc(sizeof(double) * (size_t)s1 * (size_t)n);
     double *W = (double *)malloc(sizeof(double) * (size_t)s2 * (size_t)n);
@@ -442,7 +487,8 @@ int orc_rand_cholqr(const double *V, int64_t m, int n, int64_t s1, int s2, uint6
     double *G = (double *)malloc(sizeof(double) * (size_t)n * (size_t)n);
     int info;
     orc_countsketch(V, m, n, n, s1, seed, 0, W1);
-    orc_gauss_sketch(W1, s1, n, s2, seed, W);
+    if (rademacher) orc_rademacher_sketch(W1, s1, n, s2, seed, W);
+    else orc_gauss_sketch(W1, s1, n, s2, seed, W);
     if (W1out) memcpy(W1out, W1, sizeof(double) * (size_t)s1 * (size_t)n);
     if (Wout) memcpy(Wout, W, sizeof(double) * (size_t)s2 * (size_t)n);
     info = orc_hhqr(W, s2, n, R0, NULL);
@@ -456,6 +502,21 @@ int orc_rand_cholqr(const double *V, int64_t m, int n, int64_t s1, int s2, uint6
     }
     free(W1); free(W); free(R0); free(R1); free(G);
     return info;
+}
+
+int orc_rand_cholqr(const double *V, int64_t m, int n, int64_t s1, int s2, uint64_t seed,
+                    double *Q, double *R, double *R0out, double *R1out, double *V1out,
+                    double *W1out, double *Wout)
+{
+    return rand_cholqr_impl(V, m, n, s1, s2, seed, Q, R, R0out, R1out, V1out, W1out, Wout, 0);
+}
+
+/* the same with the Rademacher S2 of N4 (Count-Rademacher multisketch) */
+int orc_rand_cholqr_rademacher(const double *V, int64_t m, int n, int64_t s1, int s2, uint64_t seed,
+                               double *Q, double *R, double *R0out, double *R1out, double *V1out,
+                               double *W1out, double *Wout)
+{
+    return rand_cholqr_impl(V, m, n, s1, s2, seed, Q, R, R0out, R1out, V1out, W1out, Wout, 1);
 }
 
 /* rand_cholQR with one dense Gaussian sketch S (s x m) in place of S2 S1

@@ -115,6 +115,21 @@ def gauss_sketch(W1, s2, seed):
     return W
 
 
+def rademacher_matrix(seed, s2, s1):
+    """N4: dense Rademacher S2, entries +-1/sqrt(s2) from Philox stream 4."""
+    S2 = np.empty((s2, s1), dtype=np.float64)
+    lib().orc_rademacher_matrix(_u64(seed), _int(s2), _i64(s1), _p(S2))
+    return S2
+
+
+def rademacher_sketch(W1, s2, seed):
+    W1 = _f64(W1)
+    s1, n = W1.shape
+    W = np.empty((s2, n), dtype=np.float64)
+    lib().orc_rademacher_sketch(_p(W1), _i64(s1), _int(n), _int(s2), _u64(seed), _p(W))
+    return W
+
+
 def dense_gauss_sketch(V, s, seed, row0=0, m_total=None):
     V = _f64(V)
     m, n = V.shape
@@ -177,22 +192,22 @@ def triu_mul(R1, R0):
     return R
 
 
-def rand_cholqr(V, s1, s2, seed, want_parts=False):
-    """Alg. 3 with Count-Gauss.  Returns (Q, R, info) or, with want_parts, a dict that also
-    holds R0, R1, V1, W1, W."""
+def rand_cholqr(V, s1, s2, seed, want_parts=False, rademacher=False):
+    """Alg. 3 with Count-Gauss (rademacher=True: Count-Rademacher, N4).  Returns (Q, R, info) or, with
+    want_parts, a dict that also holds R0, R1, V1, W1, W."""
     V = _f64(V)
+    fn = lib().orc_rand_cholqr_rademacher if rademacher else lib().orc_rand_cholqr
     m, n = V.shape
     Q = np.empty_like(V)
     R = np.zeros((n, n), dtype=np.float64)
     if not want_parts:
         z = ctypes.c_void_p(0)
-        info = lib().orc_rand_cholqr(_p(V), _i64(m), _int(n), _i64(s1), _int(s2), _u64(seed),
-                                     _p(Q), _p(R), z, z, z, z, z)
+        info = fn(_p(V), _i64(m), _int(n), _i64(s1), _int(s2), _u64(seed), _p(Q), _p(R), z, z, z, z, z)
         return Q, R, int(info)
     R0 = np.zeros((n, n)); R1 = np.zeros((n, n)); V1 = np.empty_like(V)
     W1 = np.empty((s1, n)); W = np.empty((s2, n))
-    info = lib().orc_rand_cholqr(_p(V), _i64(m), _int(n), _i64(s1), _int(s2), _u64(seed),
-                                 _p(Q), _p(R), _p(R0), _p(R1), _p(V1), _p(W1), _p(W))
+    info = fn(_p(V), _i64(m), _int(n), _i64(s1), _int(s2), _u64(seed),
+              _p(Q), _p(R), _p(R0), _p(R1), _p(V1), _p(W1), _p(W))
     return dict(Q=Q, R=R, R0=R0, R1=R1, V1=V1, W1=W1, W=W, info=int(info))
 
 

@@ -677,7 +677,7 @@ k_chol_blocked(const double* __restrict__ G, int n, double shift_h, const double
     }
 }
 
-// Column-distributed right-looking Cholesky, ONE barrier per step.  Column c -> CTA c % ncta,
+// n > 128: column-distributed right-looking Cholesky, ONE barrier per step.  Column c -> CTA c % ncta,
 // warp (c / ncta) % NW, slot (c / ncta) / NW; lane l owns rows l + 32 p (rows <= c are used).
 // Step j: every column's warp publishes its row-j entry A[j][c] into a double-buffered row buffer;
 // the lane that owns the pivot A[j][j] also publishes d = A[j][j], r = sqrt(d) and 1/r.  After the
@@ -688,105 +688,6 @@ k_chol_blocked(const double* __restrict__ G, int n, double shift_h, const double
 // CL = false: one CTA, row buffer in shared memory; CL = true: a cluster, row buffer in the (not
 // yet written) output R1, cluster barrier.
 #define CHOL_ROW_LD (RQR_MAX_N + 4)      // row entries, then d, r, 1/r
-
-// Single-CTA version (n <= 128), written like k_geqrf_g8 for few instructions per step: row j of R
-// goes straight to global memory when it is formed (no select keeps it in the tile), and
-// r = d rsqrt(d), 1/r = rsqrt(d) come from one MUFU-based sequence on the critical path.
-template <int RPL, int CPW, int NW>
-__global__ void __launch_bounds__(NW * 32, 1)
-k_chol_small(const double* __restrict__ G, int n, double shift_h, const double* __restrict__ d_shift,
-             double* R1, int* d_info, const double* __restrict__ Rprev, double* __restrict__ Rprod, int staged)
-{
-    __shared__ double srow[2][CHOL_ROW_LD];
-    const double shift = shift_h + (d_shift ? *d_shift : 0.0);
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    double a[CPW][RPL];
-#pragma unroll
-    for (int q = 0; q < CPW; ++q)
-#pragma unroll
-        for (int p = 0; p < RPL; ++p) {
-            const int c = w + NW * q, i = lane + 32 * p;
-            a[q][p] = (c < n && i <= c) ? G[(int64_t)i * n + c] + ((i == c) ? shift : 0.0) : 0.0;
-        }
-    for (int e = threadIdx.x; e < 2 * CHOL_ROW_LD; e += NW * 32) (&srow[0][0])[e] = 0.0;
-    for (int e = threadIdx.x; e < n * n; e += NW * 32) {          // exact zeros below the diagonal
-        const int i = e / n, c = e - i * n;
-        if (c < i) R1[e] = 0.0;
-    }
-    __syncthreads();
-    int fail = 0;
-    for (int j = 0; j < n; ++j) {
-        const int lj = j & 31, pj = j >> 5;
-        double* rb = srow[j & 1];
-        if (lane == lj) {                                  // publish row j of the trailing matrix
-#pragma unroll
-            for (int p = 0; p < RPL; ++p) if (p == pj) {   // warp-uniform
-#pragma unroll
-                for (int q = 0; q < CPW; ++q) rb[w + NW * q] = a[q][p];
-            }
-            if (w == j % NW) {                             // this lane holds the pivot A[j][j]
-                const int qj = j / NW;
-                double d = 0.0;
-#pragma unroll
-                for (int q = 0; q < CPW; ++q)
-#pragma unroll
-                    for (int p = 0; p < RPL; ++p) d = (q == qj && p == pj) ? a[q][p] : d;
-                const double ri = rsqrt(d);
-                rb[RQR_MAX_N] = d;
-                rb[RQR_MAX_N + 1] = d * ri;
-                rb[RQR_MAX_N + 2] = ri;
-            }
-        }
-        __syncthreads();
-        const double d = rb[RQR_MAX_N], rjj = rb[RQR_MAX_N + 1], rinv = rb[RQR_MAX_N + 2];
-        if (!(d > 0.0) || !(d < 1.0e308)) { fail = j + 1; break; }      // uniform: same d everywhere
-        double rja[RPL];                                   // R[j][a] for this lane's rows; 0 for a <= j
-#pragma unroll
-        for (int p = 0; p < RPL; ++p) {
-            const int i = lane + 32 * p;
-            rja[p] = (i > j) ? rb[i] * rinv : 0.0;
-        }
-#pragma unroll
-        for (int q = 0; q < CPW; ++q) {
-            const int c = w + NW * q;
-            const double rjc = (c > j) ? rb[c] * rinv : 0.0;            // 0 freezes finished columns
-            if (lane == lj && c >= j && c < n) R1[(int64_t)j * n + c] = (c == j) ? rjj : rjc;
-#pragma unroll
-            for (int p = 0; p < RPL; ++p) a[q][p] = fma(-rja[p], rjc, a[q][p]);   // rows > c: never read
-        }
-    }
-    if (fail && threadIdx.x == 0) rqr_set_info(d_info, RQR_INFO_NOT_SPD + fail);
-    if (Rprod != nullptr) {
-        // fused A7 of the one-shot drivers: Rprod = R1 Rprev (upper x upper, Alg. 3 step 3 PAPER.md:206).
-        // R1 was written by this CTA: visible after the barrier.  Both factors are staged in shared
-        // memory when the launch provided room for them (n <= 64), rows of Rprev padded against conflicts.
-        extern __shared__ double stage[];
-        __syncthreads();
-        if (staged) {
-            double* s1_ = stage;                         // R1, row-major, ld n
-            double* s0_ = stage + n * n;                 // Rprev, row-major, ld n + 1
-            for (int e = threadIdx.x; e < n * n; e += NW * 32) {
-                const int a_ = e / n, c = e - a_ * n;
-                s1_[e] = R1[e];
-                s0_[a_ * (n + 1) + c] = __ldg(Rprev + e);
-            }
-            __syncthreads();
-            for (int e = threadIdx.x; e < n * n; e += NW * 32) {
-                const int a_ = e / n, c = e - a_ * n;
-                double acc = 0.0;
-                for (int k = a_; k <= c; ++k) acc = fma(s1_[a_ * n + k], s0_[k * (n + 1) + c], acc);
-                Rprod[e] = (c >= a_) ? acc : 0.0;
-            }
-        } else {
-            for (int e = threadIdx.x; e < n * n; e += NW * 32) {
-                const int a_ = e / n, c = e - a_ * n;
-                double acc = 0.0;
-                for (int k = a_; k <= c; ++k) acc = fma(__ldcg(R1 + a_ * n + k), __ldg(Rprev + k * n + c), acc);
-                Rprod[e] = (c >= a_) ? acc : 0.0;
-            }
-        }
-    }
-}
 
 template <int RPL, int CPW, int NW, bool CL>
 __global__ void __launch_bounds__(NW * 32, 1)
@@ -896,7 +797,7 @@ int rqr_scholqr3_shift(const double* G, int n, int64_t m, double* d_out, cudaStr
     return RQR_OK;
 }
 
-// Rprod != NULL: also Rprod = R1 Rprev (the one-shot drivers' A7), fused into the single-CTA kernel
+// Rprod != NULL: also Rprod = R1 Rprev (the one-shot drivers' A7), fused into the single-CTA blocked kernel
 // for n <= 128, a separate k_triu_mul launch above that.
 int rqr_chol_dev(const double* G, int n, double shift, const double* d_shift, double* R1,
                  int* d_info, cudaStream_t st, const double* Rprev, double* Rprod)
