@@ -69,6 +69,16 @@ extern "C" {
                                  traffic instead of 40mn, 4mn^2 flops instead of 3mn^2).
                                  Honoured for n <= 64; for n > 64 V1 is always stored.       */
 
+#define RQR_S2_RADEMACHER 16  /* SURVEY.md 8(f) N4, PAPER.md:947 ("dense Rademacher sketch matrices in
+                                 place of dense Gaussian sketches"): S2 has entries +-1/sqrt(s2)
+                                 (reading S21; sign bits from Philox stream 4) and is
+                                 generated on the fly inside the A2 product -- no S2 in memory
+                                 (8 s2 s1 bytes: 512 MiB at n = 256), nothing to generate in A0.
+                                 OR it into `variant` of rqr_workspace_bytes, rqr_sketch_prepare,
+                                 rqr_countsketch (it only moves a workspace region there) and
+                                 rqr_rand_cholqr, and into `flags` of rqr_gauss_sketch; a workspace
+                                 must be used with the setting it was sized and prepared for.      */
+
 /* Size in bytes of the workspace every call below accepts for this problem shape. */
 size_t rqr_workspace_bytes(int64_t m, int n, int64_t s1, int s2, int variant);
 
@@ -157,6 +167,9 @@ int rqr_debug_gauss(uint64_t seed, uint32_t stream_id, uint64_t first, int64_t c
 /* Pointer to S2 (s2 x s1) inside a workspace prepared for (n, s1).  Row r starts at r * ld with
  * ld = s1 rounded up to a multiple of 16; the pad columns hold zeros.                         */
 const double* rqr_workspace_S2(void* work, int n, int64_t s1);
+/* test hook: the signs (+1 / -1) of the Rademacher S2 entries (row, c0 .. c0 + count) for sketch width s1 */
+int rqr_debug_rademacher(uint64_t seed, int64_t s1, int row, int64_t c0, int64_t count, int8_t* sign,
+                         void* stream);
 
 /* Test hook: on != 0 forces the generic (non-DMMA) kernels in rqr_trsm_gram / rqr_apply.       */
 void rqr_debug_force_generic(int on);

@@ -21,6 +21,7 @@ VARIANT_SORTED = 0
 VARIANT_SCATTER = 1
 FLAG_PREPARED = 1
 FLAG_RECOMPUTE_V1 = 2
+S2_RADEMACHER = 16          # OR into `variant` (workspace, prepare, countsketch, rand_cholqr) / `flags` (gauss_sketch)
 PROBE_DFMA = 0
 PROBE_DMMA = 1
 
@@ -48,6 +49,7 @@ SIGNATURES = {
     "rqr_debug_hash_sign": (_int, [_u64, _i64, _i64, _i64, _vp, _vp, _vp]),
     "rqr_debug_gauss": (_int, [_u64, _u32, _u64, _i64, _vp, _vp]),
     "rqr_workspace_S2": (_vp, [_vp, _int, _i64]),
+    "rqr_debug_rademacher": (_int, [_u64, _i64, _int, _i64, _i64, _vp, _vp]),
     "rqr_debug_force_generic": (None, [_int]),
     "rqr_version": (ctypes.c_char_p, []),
     "rqr_probe_fp64": (_int, [_int, _int, _int, _vp, _vp, _vp]),
@@ -222,6 +224,12 @@ def debug_gauss(seed, stream_id, first, count, device="cuda"):
     z = torch.empty(count, dtype=torch.float64, device=device)
     _chk(lib().rqr_debug_gauss(seed, stream_id, first, count, _ptr(z), _stream()), "rqr_debug_gauss")
     return z
+
+
+def debug_rademacher(seed, s1, row, c0, count, device="cuda"):
+    sg = torch.empty(count, dtype=torch.int8, device=device)
+    _chk(lib().rqr_debug_rademacher(seed, s1, row, c0, count, _ptr(sg), _stream()), "rqr_debug_rademacher")
+    return sg
 
 
 def workspace_S2(work, n, s1, s2):

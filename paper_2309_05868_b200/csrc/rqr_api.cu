@@ -12,9 +12,8 @@ extern "C" const char* rqr_version(void) { return "rqr 0.1 (sm_100a)"; }
 
 extern "C" size_t rqr_workspace_bytes(int64_t m, int n, int64_t s1, int s2, int variant)
 {
-    (void)variant;
     if (m < 1 || n < 2 || n > RQR_MAX_N || s1 < 1 || s2 < 1 || s2 > RQR_MAX_S2) return 0;
-    return rqr_layout(m, n, s1).total;
+    return rqr_layout(m, n, s1, (variant & RQR_S2_RADEMACHER) != 0).total;
 }
 
 #define RQR_TRY(call)                 \
@@ -63,9 +62,11 @@ extern "C" int rqr_rand_cholqr(const double* V, int64_t m, int n, int64_t s1, in
     if (rc != RQR_OK) return rc;
     if (s1 < 1 || s1 >= ((int64_t)1 << 31) || s1 > m) return -4;
     if (s2 < n || s2 > s1 || s2 > RQR_MAX_S2) return -5;      // eq. (20)
-    if (variant != RQR_VARIANT_SORTED && variant != RQR_VARIANT_SCATTER) return -11;
+    const int rad = variant & RQR_S2_RADEMACHER;                 // N4: Count-Rademacher multisketch
+    if ((variant & ~RQR_S2_RADEMACHER) != RQR_VARIANT_SORTED && (variant & ~RQR_S2_RADEMACHER) != RQR_VARIANT_SCATTER)
+        return -11;
     cudaStream_t st = (cudaStream_t)stream;
-    RqrLayout L = rqr_layout(m, n, s1);
+    RqrLayout L = rqr_layout(m, n, s1, rad != 0);
     double* R0 = small_mat(work, L, n, RQR_SM_R0);
     double* R1 = small_mat(work, L, n, RQR_SM_R1);
     double* G = small_mat(work, L, n, RQR_SM_G);
@@ -76,7 +77,7 @@ extern "C" int rqr_rand_cholqr(const double* V, int64_t m, int n, int64_t s1, in
         RQR_TRY(rqr_sketch_prepare(m, n, 0, s1, s2, seed, variant, work, st));
     // Alg. 1 randQR: W = S2 S1 V; R0 = hhqr(W).R; V1 = V R0^-1
     RQR_TRY(rqr_countsketch(V, m, n, n, 0, s1, seed, W1, work, variant, RQR_FLAG_PREPARED, st));
-    RQR_TRY(rqr_gauss_sketch(W1, s1, n, s2, seed, W, work, RQR_FLAG_PREPARED, st));
+    RQR_TRY(rqr_gauss_sketch(W1, s1, n, s2, seed, W, work, RQR_FLAG_PREPARED | rad, st));
     RQR_TRY(rqr_small_geqrf(W, s2, n, R0, d_info, st));
     // Alg. 2 cholQR of V1; Alg. 3 step 3
     RQR_TRY(tail_cholqr(V, m, n, R0, Q, R1, G, work, d_info, flags & RQR_FLAG_RECOMPUTE_V1, st, R));

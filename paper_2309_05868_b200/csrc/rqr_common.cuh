@@ -16,6 +16,7 @@
 #define RQR_PHILOX_STREAM_COUNT 0u
 #define RQR_PHILOX_STREAM_S2 1u
 #define RQR_PHILOX_STREAM_DENSE 3u
+#define RQR_PHILOX_STREAM_RADEMACHER 4u
 
 #define RQR_LAUNCH_CHECK()                                   \
     do {                                                     \
@@ -44,7 +45,7 @@ __host__ __device__ static inline int64_t rqr_s2_ld(int64_t s1) { return (s1 + 1
 //   A  tall scratch    f(n)      Gram partials, small matrices of the one-shot drivers, panel
 //                                fragment slots of the n > 64 kernels (2 sets x 10 x 32 KB)
 //   B  bucket offsets  f(s1)     (s1+1) u32 offsets, s1 u32 cursors
-//   C  S2 slot         f(s1)     sized for s2 = RQR_MAX_S2
+//   C  S2 slot         f(s1)     sized for s2 = RQR_MAX_S2; empty with RQR_S2_RADEMACHER
 //   D  gauss partials  f(n)
 //   E  sorted rows     f(m)      m u32 (row | sign<<31)
 //   W  one-shot W      (s2max x n), in the n-only part (before B)
@@ -54,7 +55,8 @@ struct RqrLayout {
     size_t hdr, A, A_small, A_frags, B_off, B_cur, C, D, E, F_W1, F_W, total;
 };
 
-static inline RqrLayout rqr_layout(int64_t m, int n, int64_t s1)
+// no_S2: the Rademacher S2 of N4 is generated on the fly, region C is empty
+static inline RqrLayout rqr_layout(int64_t m, int n, int64_t s1, bool no_S2 = false)
 {
     RqrLayout L;
     size_t nn = (size_t)n * n * sizeof(double);
@@ -68,7 +70,7 @@ static inline RqrLayout rqr_layout(int64_t m, int n, int64_t s1)
     L.B_off = L.F_W + rqr_align256((size_t)RQR_MAX_S2 * n * sizeof(double));
     L.B_cur = L.B_off + rqr_align256((size_t)(s1 + 1) * 4);
     L.C = L.B_cur + rqr_align256((size_t)s1 * 4);
-    L.D = L.C + rqr_align256((size_t)RQR_MAX_S2 * (size_t)rqr_s2_ld(s1) * sizeof(double));
+    L.D = L.C + (no_S2 ? 0 : rqr_align256((size_t)RQR_MAX_S2 * (size_t)rqr_s2_ld(s1) * sizeof(double)));
     L.E = L.D + rqr_align256((size_t)RQR_GAUSS_PARTIAL_ROWS * n * sizeof(double));
     L.F_W1 = L.E + rqr_align256((size_t)m * 4);
     L.total = L.F_W1 + rqr_align256((size_t)s1 * n * sizeof(double));
@@ -102,6 +104,12 @@ __host__ __device__ __forceinline__ void rqr_philox(uint64_t seed, uint64_t idx,
         k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
     }
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// Rademacher S2 (N4; reading S21): the 128 sign bits of row r, columns [128 g, 128 g + 128)
+__device__ __forceinline__ void rqr_rademacher_bits(uint64_t seed, uint32_t r, uint64_t ng, uint64_t g, uint32_t out[4])
+{
+    rqr_philox(seed, (uint64_t)r * ng + g, RQR_PHILOX_STREAM_RADEMACHER, out);
 }
 
 // CountSketch bucket and sign of GLOBAL row index i (reading S1/S2).

@@ -5,6 +5,8 @@
 // tile (64 x 16) and of W1 (16 x n) with per-row bulk async copies into padded rows (strides 20 and
 // n+4 doubles: the A- and B-fragment reads are bank-conflict free); 4 stages, full/empty mbarriers.
 // Partials go to the caller's buffer and are reduced in fixed order by k_reduce_partials.
+// RAD (N4): S2 is the dense Rademacher matrix of reading S21; nothing of S2 is staged, every lane
+// forms its A-fragment entries +-1/sqrt(s2) from the Philox words of its row (one call per 128 columns).
 #include "rqr_mma.cuh"
 
 #define GM_KB 16
@@ -25,10 +27,10 @@ struct GaussPlan {
     static constexpr size_t bytes = (bars + 2 * GM_STAGES) * sizeof(double);
 };
 
-template <int NBN>
+template <int NBN, bool RAD>
 __global__ void __launch_bounds__((GM_WARPS + 1) * 32, 1)
 k_gauss_gemm_mma(const double* __restrict__ S2, const double* __restrict__ W1, int64_t s1, int n, int s2,
-                 int64_t kchunk, double* __restrict__ part)
+                 int64_t kchunk, double* __restrict__ part, uint64_t seed)
 {
     using Plan = GaussPlan<NBN>;
     constexpr int LDA = Plan::LDA, LDB = Plan::LDB;
@@ -61,10 +63,11 @@ k_gauss_gemm_mma(const double* __restrict__ S2, const double* __restrict__ W1, i
             // the last slice may run past s1: S2's pad columns are zero, the matching rows of the B stage
             // keep finite data of an earlier slice (0 x finite = 0), so only the existing rows of W1 are copied
             const int rows_b = (int)((s1 - k) < GM_KB ? (s1 - k) : GM_KB);
-            if (lane == 0) mbar_expect_tx(full + stage, (uint32_t)(rows_a * GM_KB * 8 + rows_b * n * 8));
+            if (lane == 0) mbar_expect_tx(full + stage, (uint32_t)((RAD ? 0 : rows_a * GM_KB * 8) + rows_b * n * 8));
             __syncwarp();
-            for (int r = lane; r < rows_a; r += 32)
-                bulk_g2s(A + r * LDA, S2 + (int64_t)(m0 + r) * lds2 + k, GM_KB * 8, full + stage);
+            if (!RAD)
+                for (int r = lane; r < rows_a; r += 32)
+                    bulk_g2s(A + r * LDA, S2 + (int64_t)(m0 + r) * lds2 + k, GM_KB * 8, full + stage);
             if (lane < rows_b) bulk_g2s(B + lane * LDB, W1 + (k + lane) * n, (uint32_t)(n * 8), full + stage);
             if (++stage == GM_STAGES) { stage = 0; ph ^= 1u; }
         }
@@ -76,13 +79,31 @@ k_gauss_gemm_mma(const double* __restrict__ S2, const double* __restrict__ W1, i
     for (int b = 0; b < NBN; ++b) { acc[b][0] = 0.0; acc[b][1] = 0.0; }
     int stage = 0;
     uint32_t ph = 0;
+    const uint64_t ng = (uint64_t)((s1 + 127) >> 7);
+    const double inv = 1.0 / sqrt((double)s2);
+    uint32_t o[4] = {0u, 0u, 0u, 0u};
+    int64_t gcur = -1;
     for (int s = 0; s < nsteps; ++s) {
         const double* A = smem + (size_t)stage * Plan::stage + (8 * warp + r) * LDA + q;
         const double* B = smem + (size_t)stage * Plan::stage + Plan::a_doubles + q * LDB + r;
+        uint32_t bits = 0;
+        const int64_t kcol = k0 + (int64_t)s * GM_KB;
+        if (RAD) {
+            const int64_t g = kcol >> 7;
+            if (g != gcur) {
+                rqr_rademacher_bits(seed, (uint32_t)(m0 + 8 * warp + r), ng, (uint64_t)g, o);
+                gcur = g;
+            }
+            const int b0 = (int)(kcol & 127);
+            const uint32_t word = b0 < 64 ? (b0 < 32 ? o[0] : o[1]) : (b0 < 96 ? o[2] : o[3]);
+            bits = word >> ((b0 & 31) + q);                    // bit 4 j: column kcol + 4 j + q
+        }
         mbar_wait(full + stage, ph);
 #pragma unroll
         for (int kk = 0; kk < GM_KB; kk += 4) {
-            const double a = A[kk];
+            double a;
+            if (RAD) a = (kcol + kk + q < s1) ? (((bits >> kk) & 1u) ? -inv : inv) : 0.0;
+            else a = A[kk];
 #pragma unroll
             for (int b = 0; b < NBN; ++b) dmma(acc[b][0], acc[b][1], a, B[kk * LDB + 8 * b]);
         }
@@ -102,15 +123,15 @@ k_gauss_gemm_mma(const double* __restrict__ S2, const double* __restrict__ W1, i
     }
 }
 
-template <int NBN>
+template <int NBN, bool RAD>
 static int launch_gauss_mma(const double* S2, const double* W1, int64_t s1, int n, int s2, double* part,
-                            int64_t ks_cap, int* ks_out, cudaStream_t st)
+                            int64_t ks_cap, int* ks_out, cudaStream_t st, uint64_t seed)
 {
     using Plan = GaussPlan<NBN>;
     static_assert(Plan::bytes <= 227 * 1024, "k_gauss_gemm_mma shared memory plan too large");
     static bool attr = false;
     if (!attr) {
-        cudaFuncSetAttribute(k_gauss_gemm_mma<NBN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
+        cudaFuncSetAttribute(k_gauss_gemm_mma<NBN, RAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
         attr = true;
     }
     const int tiles_m = (s2 + 63) / 64;
@@ -122,19 +143,24 @@ static int launch_gauss_mma(const double* S2, const double* W1, int64_t s1, int 
     const int64_t kchunk = ((kblocks + ks - 1) / ks) * GM_KB;
     ks = (s1 + kchunk - 1) / kchunk;
     dim3 grid(1, tiles_m, (unsigned)ks);
-    k_gauss_gemm_mma<NBN><<<grid, (GM_WARPS + 1) * 32, Plan::bytes, st>>>(S2, W1, s1, n, s2, kchunk, part);
+    k_gauss_gemm_mma<NBN, RAD><<<grid, (GM_WARPS + 1) * 32, Plan::bytes, st>>>(S2, W1, s1, n, s2, kchunk, part, seed);
     RQR_LAUNCH_CHECK();
     *ks_out = (int)ks;
     return RQR_OK;
 }
 
-// returns RQR_TALL_NOT_HANDLED when the shape is left to the DFMA kernel
+// returns RQR_TALL_NOT_HANDLED when the shape is left to the DFMA kernel; S2 == NULL: Rademacher S2 from `seed`
 int rqr_gauss_gemm_mma(const double* S2, const double* W1, int64_t s1, int n, int s2, double* part,
-                       int64_t ks_cap, int* ks_out, cudaStream_t st)
+                       int64_t ks_cap, int* ks_out, cudaStream_t st, uint64_t seed)
 {
     if (n < 96 || n > 256 || (n & 1)) return RQR_TALL_NOT_HANDLED;
     if ((((uintptr_t)S2 | (uintptr_t)W1) & 15) != 0) return RQR_TALL_NOT_HANDLED;
-    if (n <= 128) return launch_gauss_mma<16>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st);
-    if (n <= 192) return launch_gauss_mma<24>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st);
-    return launch_gauss_mma<32>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st);
+    if (S2) {
+        if (n <= 128) return launch_gauss_mma<16, false>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st, seed);
+        if (n <= 192) return launch_gauss_mma<24, false>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st, seed);
+        return launch_gauss_mma<32, false>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st, seed);
+    }
+    if (n <= 128) return launch_gauss_mma<16, true>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st, seed);
+    if (n <= 192) return launch_gauss_mma<24, true>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st, seed);
+    return launch_gauss_mma<32, true>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st, seed);
 }

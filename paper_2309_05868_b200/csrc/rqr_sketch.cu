@@ -5,7 +5,7 @@
 #include "rqr_tall.cuh"
 
 int rqr_gauss_gemm_mma(const double* S2, const double* W1, int64_t s1, int n, int s2, double* part,
-                       int64_t ks_cap, int* ks_out, cudaStream_t st);
+                       int64_t ks_cap, int* ks_out, cudaStream_t st, uint64_t seed);
 
 // =========================================================================================
 // A0: sketch generation (off the paper's clock)
@@ -174,12 +174,14 @@ extern "C" int rqr_sketch_prepare(int64_t m, int n, int64_t row0, int64_t s1, in
     if (row0 < 0) return -3;
     if (s1 < 1 || s1 >= ((int64_t)1 << 31)) return -4;
     if (s2 < 1 || s2 > RQR_MAX_S2 || s2 > s1) return -5;
+    const bool rademacher = (variant & RQR_S2_RADEMACHER) != 0;
+    variant &= ~RQR_S2_RADEMACHER;
     if (variant != RQR_VARIANT_SORTED && variant != RQR_VARIANT_SCATTER) return -7;
     if (!work) return -8;
     cudaStream_t st = (cudaStream_t)stream;
-    RqrLayout L = rqr_layout(m, n, s1);
+    RqrLayout L = rqr_layout(m, n, s1, rademacher);
     char* w = (char*)work;
-    int rc = launch_prepare_S2(s1, s2, seed, (double*)(w + L.C), st);
+    int rc = rademacher ? RQR_OK : launch_prepare_S2(s1, s2, seed, (double*)(w + L.C), st);
     if (rc != RQR_OK) return rc;
     if (variant == RQR_VARIANT_SORTED)
         rc = launch_prepare_sorted(m, row0, s1, seed, (uint32_t*)(w + L.B_off),
@@ -292,6 +294,8 @@ extern "C" int rqr_countsketch(const double* V, int64_t m, int n, int64_t ldv, i
     if (row0 < 0) return -5;
     if (s1 < 1 || s1 >= ((int64_t)1 << 31)) return -6;
     if (!W1) return -8;
+    const bool rademacher = (variant & RQR_S2_RADEMACHER) != 0;      // only moves region E of the workspace
+    variant &= ~RQR_S2_RADEMACHER;
     if (variant != RQR_VARIANT_SORTED && variant != RQR_VARIANT_SCATTER) return -10;
     cudaStream_t st = (cudaStream_t)stream;
     if (variant == RQR_VARIANT_SCATTER) {
@@ -305,7 +309,7 @@ extern "C" int rqr_countsketch(const double* V, int64_t m, int n, int64_t ldv, i
         return RQR_OK;
     }
     if (!work) return -9;
-    RqrLayout L = rqr_layout(m, n, s1);
+    RqrLayout L = rqr_layout(m, n, s1, rademacher);
     char* w = (char*)work;
     uint32_t* off = (uint32_t*)(w + L.B_off);
     uint32_t* cur = (uint32_t*)(w + L.B_cur);
@@ -395,6 +399,80 @@ k_gauss_gemm_splitk(const double* __restrict__ S2, const double* __restrict__ W1
     }
 }
 
+// N4: the same split-K product with S2 a dense Rademacher matrix generated on the fly (entries +-1/sqrt(s2),
+// PAPER.md:947; reading S21): no S2 in memory, the A tile comes from 16 bits of the row's Philox words.
+__global__ void __launch_bounds__(256)
+k_rademacher_gemm_splitk(uint64_t seed, const double* __restrict__ W1, int64_t s1, int n, int s2,
+                         int64_t kchunk, double* __restrict__ part)
+{
+    __shared__ double As[GS_BK][GS_BM + 1];
+    __shared__ double Bs[GS_BK][GS_BN];
+    const int tid = threadIdx.x;
+    const int tx = tid & 15, ty = tid >> 4;
+    const int row_base = blockIdx.y * GS_BM, col_base = blockIdx.x * GS_BN;
+    const int64_t k0 = (int64_t)blockIdx.z * kchunk;              // a multiple of GS_BK = 16
+    const int64_t k1 = k0 + kchunk < s1 ? k0 + kchunk : s1;
+    const uint64_t ng = (uint64_t)((s1 + 127) >> 7);
+    const double inv = 1.0 / sqrt((double)s2);
+    uint32_t o0 = 0, o1 = 0, o2 = 0, o3 = 0;
+    int64_t gcur = -1;
+    double acc[4][4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j] = 0.0;
+    for (int64_t kk = k0; kk < k1; kk += GS_BK) {
+        if (tid < GS_BM) {                                        // one thread per row of the tile
+            const int gr = row_base + tid;
+            const int64_t g = kk >> 7;
+            if (g != gcur) {
+                uint32_t o[4];
+                rqr_rademacher_bits(seed, (uint32_t)gr, ng, (uint64_t)g, o);
+                o0 = o[0]; o1 = o[1]; o2 = o[2]; o3 = o[3];
+                gcur = g;
+            }
+            const int b0 = (int)(kk & 127);
+            const uint32_t word = b0 < 64 ? (b0 < 32 ? o0 : o1) : (b0 < 96 ? o2 : o3);
+            const uint32_t bits = word >> (b0 & 31);
+#pragma unroll
+            for (int k = 0; k < GS_BK; ++k)
+                As[k][tid] = (gr < s2 && kk + k < k1) ? (((bits >> k) & 1u) ? -inv : inv) : 0.0;
+        }
+#pragma unroll
+        for (int t = 0; t < 4; ++t) {
+            int idx = tid + t * 256;
+            int k = idx >> 6, c = idx & 63;
+            int gc = col_base + c; int64_t gk = kk + k;
+            Bs[k][c] = (gc < n && gk < k1) ? W1[gk * n + gc] : 0.0;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < GS_BK; ++k) {
+            double a[4], b[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) a[i] = As[k][ty + 16 * i];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) b[j] = Bs[k][tx + 16 * j];
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) acc[i][j] = fma(a[i], b[j], acc[i][j]);
+        }
+        __syncthreads();
+    }
+    double* P = part + (int64_t)blockIdx.z * s2 * n;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        int gr = row_base + ty + 16 * i;
+        if (gr >= s2) continue;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            int gc = col_base + tx + 16 * j;
+            if (gc < n) P[(int64_t)gr * n + gc] = acc[i][j];
+        }
+    }
+}
+
 // out[e] = sum_p part[p][e].  Fixed order: 4 interleaved groups of partials (p = g, g+4, ...; 8
 // loads in flight per thread), then the groups in order 0..3 through shared memory.
 __global__ void __launch_bounds__(256)
@@ -440,19 +518,20 @@ extern "C" int rqr_gauss_sketch(const double* W1, int64_t s1, int n, int s2, uin
     if (!W) return -6;
     if (!work) return -7;
     cudaStream_t st = (cudaStream_t)stream;
-    RqrLayout L = rqr_layout(1, n, s1);
+    const bool rademacher = (flags & RQR_S2_RADEMACHER) != 0;
+    RqrLayout L = rqr_layout(1, n, s1, rademacher);
     char* w = (char*)work;
     double* S2 = (double*)(w + L.C);
     double* part = (double*)(w + L.D);
-    if (!(flags & RQR_FLAG_PREPARED)) {
+    if (!rademacher && !(flags & RQR_FLAG_PREPARED)) {
         int rc = launch_prepare_S2(s1, s2, seed, S2, st);
         if (rc != RQR_OK) return rc;
     }
     int64_t ks_cap = RQR_GAUSS_PARTIAL_ROWS / s2;
     int64_t elems = (int64_t)s2 * n;
     {
-        int ks_mma = 0;                           // n >= 128: FP64 DMMA GEMM (rqr_gauss_mma.cu)
-        int rc = rqr_gauss_gemm_mma(S2, W1, s1, n, s2, part, ks_cap, &ks_mma, st);
+        int ks_mma = 0;                           // n >= 96: FP64 DMMA GEMM (rqr_gauss_mma.cu)
+        int rc = rqr_gauss_gemm_mma(rademacher ? nullptr : S2, W1, s1, n, s2, part, ks_cap, &ks_mma, st, seed);
         if (rc == RQR_OK) {
             k_reduce_partials<<<(int)((elems + 63) / 64), 256, 0, st>>>(part, ks_mma, elems, W);
             RQR_LAUNCH_CHECK();
@@ -469,7 +548,8 @@ extern "C" int rqr_gauss_sketch(const double* W1, int64_t s1, int n, int s2, uin
     int64_t kchunk = ((kblocks + ks - 1) / ks) * GS_BK;
     ks = (s1 + kchunk - 1) / kchunk;
     dim3 grid(tiles_n, tiles_m, (unsigned)ks);
-    k_gauss_gemm_splitk<<<grid, 256, 0, st>>>(S2, W1, s1, n, s2, kchunk, part);
+    if (rademacher) k_rademacher_gemm_splitk<<<grid, 256, 0, st>>>(seed, W1, s1, n, s2, kchunk, part);
+    else k_gauss_gemm_splitk<<<grid, 256, 0, st>>>(S2, W1, s1, n, s2, kchunk, part);
     RQR_LAUNCH_CHECK();
     k_reduce_partials<<<(int)((elems + 63) / 64), 256, 0, st>>>(part, (int)ks, elems, W);
     RQR_LAUNCH_CHECK();
@@ -602,6 +682,32 @@ extern "C" int rqr_debug_hash_sign(uint64_t seed, int64_t row0, int64_t count, i
     if (!sign) return -6;
     int blocks = (int)((count + 255) / 256 < 4096 ? (count + 255) / 256 : 4096);
     k_debug_hash_sign<<<blocks, 256, 0, (cudaStream_t)stream>>>(seed, row0, count, (uint32_t)s1, bucket, sign);
+    RQR_LAUNCH_CHECK();
+    return RQR_OK;
+}
+
+__global__ void k_debug_rademacher(uint64_t seed, int64_t s1, int row, int64_t c0, int64_t count, int8_t* sign)
+{
+    const uint64_t ng = (uint64_t)((s1 + 127) >> 7);
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < count; i += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t c = c0 + i;
+        uint32_t o[4];
+        rqr_rademacher_bits(seed, (uint32_t)row, ng, (uint64_t)(c >> 7), o);
+        const int b = (int)(c & 127);
+        const uint32_t word = b < 64 ? (b < 32 ? o[0] : o[1]) : (b < 96 ? o[2] : o[3]);
+        sign[i] = ((word >> (b & 31)) & 1u) ? (int8_t)-1 : (int8_t)1;
+    }
+}
+
+extern "C" int rqr_debug_rademacher(uint64_t seed, int64_t s1, int row, int64_t c0, int64_t count, int8_t* sign,
+                                    void* stream)
+{
+    if (s1 < 1 || s1 >= ((int64_t)1 << 31)) return -2;
+    if (row < 0 || row >= RQR_MAX_S2) return -3;
+    if (c0 < 0 || count < 1 || c0 + count > s1) return -4;
+    if (!sign) return -6;
+    int blocks = (int)((count + 255) / 256 < 4096 ? (count + 255) / 256 : 4096);
+    k_debug_rademacher<<<blocks, 256, 0, (cudaStream_t)stream>>>(seed, s1, row, c0, count, sign);
     RQR_LAUNCH_CHECK();
     return RQR_OK;
 }

@@ -3,7 +3,8 @@
   python -m paper_2309_05868_b200.stepbench --m 8388608 --n 64 [--reps 10]
 
 Prints one JSON line: CUDA-event time of every step called on its own (A0 sketch generation, A1 in both
-CountSketch variants, A2, A3, A4 with and without R0, A5, A6 stored / recomputed, A7), with the achieved
+CountSketch variants, A2 with the Gaussian and with the on-the-fly Rademacher S2 (N4), A3, A4 with and without R0,
+A5, A6 stored / recomputed, A7, the one-shot with either S2), with the achieved
 GB/s or TFLOP/s of the m-sized passes against their algorithmic work.  The input is a
 plain Gaussian matrix: timings do not depend on the values.
 """
@@ -79,6 +80,15 @@ def main(argv=None):
     if n <= 64:
         t["A6_apply_recompute_V1"] = _time(lambda: rq.apply(V, R0, R1, Q, work), reps)
     t["A7_triu_mul"] = _time(lambda: rq.triu_mul(R1, R0, R), reps)
+    # N4: Rademacher S2 generated on the fly (no S2 in the workspace), and the one-shot with either S2
+    RAD = rq.S2_RADEMACHER
+    t["one_shot_gauss_S2"] = _time(lambda: rq.rand_cholqr(V, s1, s2, 42, Q, R, work, info, 0, P), reps)
+    del work
+    workr = rq.alloc_workspace(m, n, s1, s2, RAD)
+    t["A0_sketch_prepare_rademacher"] = _time(lambda: rq.sketch_prepare(m, n, s1, s2, 42, workr, RAD), max(2, reps // 3))
+    t["A2_rademacher_sketch"] = _time(lambda: rq.gauss_sketch(W1, s2, 42, W, workr, P | RAD), reps)
+    t["one_shot_rademacher_S2"] = _time(lambda: rq.rand_cholqr(V, s1, s2, 42, Q, R, workr, info, RAD, P), reps)
+    out["workspace_bytes"] = {"gauss_S2": rq.workspace_bytes(m, n, s1, s2, 0), "rademacher_S2": rq.workspace_bytes(m, n, s1, s2, RAD)}
     mn = float(m) * n
     out["achieved"] = {
         "A1_sorted_GBs": 8.0 * mn / t["A1_countsketch_sorted"] / 1e6,

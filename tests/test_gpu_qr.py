@@ -385,3 +385,35 @@ def test_random_shapes_meet_the_invariants(rq, case):
         assert torch.equal(Vc, Q) and torch.equal(R2, R)
     else:
         assert orth_err(Vc) <= ORTH_TOL
+
+
+# ---- N4: Count-Rademacher multisketch (S2 dense Rademacher, generated on the fly) ----
+@pytest.mark.parametrize("name,m,n,kappa", [("C1", 20000, 16, 1e10), ("n64", 65536, 64, 1e12), ("n70", 100000, 70, 1e8),
+                                            ("n128", 40000, 128, 1e12), ("n256", 140000, 256, 1e14),
+                                            ("ragged", 4099, 24, 1e6)])
+def test_rand_cholqr_rademacher_matches_oracle(rq, orc, name, m, n, kappa):
+    s1, s2 = inputs.sketch_sizes(n)
+    V = inputs.make_V(m, n, kappa, 1234)
+    Vd = V.cuda()
+    Qo, Ro, io = orc.rand_cholqr(V.numpy(), s1, s2, 42, rademacher=True)
+    assert io == 0
+    for variant, flags, prepared in [(rq.S2_RADEMACHER, 0, False), (rq.S2_RADEMACHER, rq.FLAG_RECOMPUTE_V1, True),
+                                     (rq.S2_RADEMACHER | 1, 0, True)]:
+        Q, R, info = run_rand(rq, Vd, s1, s2, 42, variant, flags, prepared)
+        assert info == 0
+        assert orth_err(Q) <= ORTH_TOL
+        assert resid(Vd, Q, R) <= RES_TOL
+        check_R(R)
+        assert np.linalg.norm(R.cpu().numpy() - Ro) <= R_TOL * np.linalg.norm(Ro)
+    Qot = torch.from_numpy(Qo)
+    assert orth_err(Qot) <= ORTH_TOL and resid(V, Qot, torch.from_numpy(Ro)) <= RES_TOL
+
+
+def test_rademacher_full_size_C2(rq):
+    """BASELINE configs[1] shape with the Rademacher S2: the north_star bars at full size."""
+    m, n = 1 << 20, 64
+    s1, s2 = inputs.sketch_sizes(n)
+    Vd = inputs.make_V(m, n, 1e12, 42, device="cuda")
+    Q, R, info = run_rand(rq, Vd, s1, s2, 42, rq.S2_RADEMACHER, 0, True)
+    assert info == 0 and orth_err(Q) <= ORTH_TOL and resid(Vd, Q, R) <= RES_TOL
+    check_R(R)

@@ -274,3 +274,47 @@ def test_tsqr_r_matches_householder(rq, orc, rows, n):
     assert np.array_equal(np.tril(Rh, -1), np.zeros_like(Rh)) and (np.diag(Rh) > 0).all()
     assert np.linalg.norm(Rh - Ro) <= 1e-13 * np.linalg.norm(Ro)
     assert np.all(np.linalg.norm(Rh - Ro, axis=1) <= 1e-11 * np.linalg.norm(Ro, axis=1) + 1e-300)
+
+
+# ---- N4: dense Rademacher S2 generated on the fly (reading S21) ----
+@pytest.mark.parametrize("s1,s2", [(300, 5), (8192, 128), (129, 7), (40953, 789)])
+def test_rademacher_signs_bit_exact(rq, orc, s1, s2):
+    So = orc.rademacher_matrix(42, s2, s1)
+    for row in sorted({0, 1, s2 // 2, s2 - 1}):
+        sg = host(rq.debug_rademacher(42, s1, row, 0, s1))
+        assert np.array_equal(sg, np.where(So[row] < 0, -1, 1).astype(np.int8))
+    c0 = s1 // 3
+    sg = host(rq.debug_rademacher(42, s1, s2 - 1, c0, s1 - c0))        # ragged start inside a 128-bit group
+    assert np.array_equal(sg, np.where(So[s2 - 1, c0:] < 0, -1, 1).astype(np.int8))
+
+
+@pytest.mark.parametrize("s1,n,s2", [(512, 16, 32), (8192, 64, 128), (9940, 70, 140), (300, 5, 7),
+                                     (32768, 128, 256), (9984, 200, 401), (40953, 70, 789), (131072, 256, 512)])
+def test_rademacher_sketch_parity(rq, orc, s1, n, s2):
+    rng = np.random.default_rng(s1 + n)
+    W1 = rng.standard_normal((s1, n))
+    W = torch.empty(s2, n, dtype=torch.float64, device="cuda")
+    work = rq.alloc_workspace(s1, n, s1, s2, rq.S2_RADEMACHER)
+    rq.gauss_sketch(dev(W1), s2, 42, W, work, rq.S2_RADEMACHER)
+    Wo = orc.rademacher_sketch(W1, s2, 42)
+    assert np.abs(host(W) - Wo).max() <= 1e-13 * np.abs(Wo).max()
+
+
+@pytest.mark.parametrize("s1,n,s2", [(5000, 24, 64), (9000, 70, 256), (700, 9, 16)])
+def test_rademacher_sketch_exact_on_integers(rq, orc, s1, n, s2):
+    """s2 a power of 4: 1/sqrt(s2) is a power of two, so on integer data every +- sum is exact in any order and
+    the split-K kernel must agree with the oracle to the last bit (a wrong sign or a dropped column cannot hide)."""
+    rng = np.random.default_rng(s1)
+    Wi = np.rint(rng.standard_normal((s1, n)) * 16)
+    W = torch.empty(s2, n, dtype=torch.float64, device="cuda")
+    work = rq.alloc_workspace(s1, n, s1, s2, rq.S2_RADEMACHER)
+    rq.gauss_sketch(dev(Wi), s2, 42, W, work, rq.S2_RADEMACHER)
+    assert np.array_equal(host(W), orc.rademacher_sketch(Wi, s2, 42))
+
+
+def test_rademacher_workspace_has_no_S2(rq):
+    n, m = 256, 1 << 21
+    s1, s2 = 2 * n * n, 2 * n
+    full = rq.workspace_bytes(m, n, s1, s2, 0)
+    lean = rq.workspace_bytes(m, n, s1, s2, rq.S2_RADEMACHER)
+    assert full - lean >= 8 * s2 * s1                                  # the 512 MiB of S2 at n = 256
