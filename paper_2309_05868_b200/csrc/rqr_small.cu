@@ -523,10 +523,23 @@ __device__ __forceinline__ void cholb_dmma(double& c0, double& c1, double a, dou
                  : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
-__global__ void __launch_bounds__(256, 1)
-k_chol_blocked(const double* __restrict__ G, int n, double shift_h, const double* __restrict__ d_shift,
-               double* __restrict__ R1, int* d_info, const double* __restrict__ Rprev, double* __restrict__ Rprod)
+// Where the two-level driver parks inv(R_KK) of the first half (16 blocks of 8 x 8): in the strictly lower
+// triangle of R1's leading 128 x 128 block, which is zero in the result and re-zeroed by k_chol2_syrk:
+// block (K + 1, K) for K < 15, block (15, 0) for K = 15.
+__device__ __forceinline__ double* chol2_tslot(double* base, int ld, int K)
 {
+    return (K < 15) ? base + (int64_t)(8 * (K + 1)) * ld + 8 * K : base + (int64_t)(8 * 15) * ld;
+}
+
+__global__ void __launch_bounds__(256, 1)
+k_chol_blocked(const double* G, int ldg, int n, double shift_h, const double* __restrict__ d_shift,
+               double* R1, int ldr, int* d_info, int info_off, const double* __restrict__ Rprev,
+               double* __restrict__ Rprod, double* Tsave, int ldt, double* zero_src, int zero_cols)
+{
+    // G, R1: n x n with leading dimensions ldg, ldr (the two-level driver for n > 128 factors sub-blocks in place).
+    // Tsave != NULL: inv(R_KK) of block K is also stored (8 x 8, leading dimension ldt) at Tsave + T-slot(K), see
+    // chol2_tslot.  zero_src != NULL: the scratch area that held the input (== G; n rows x zero_cols columns, leading
+    // dimension ldg) is zeroed once the input is in shared memory.
     extern __shared__ double dyn[];
     const int NB = (n + 7) >> 3, np = 8 * NB;
     const int LD = np + 8 + (np & 8);         // row stride = 8 mod 16 doubles: the 128-bit C-fragment accesses are conflict free
@@ -538,12 +551,19 @@ k_chol_blocked(const double* __restrict__ G, int n, double shift_h, const double
     for (int e = tid; e < np * np; e += 256) {
         const int i = e / np, c = e - i * np;
         double v = (i == c) ? 1.0 : 0.0;
-        if (i < n && c < n) v = G[(int64_t)i * n + c] + ((i == c) ? shift : 0.0);
+        if (i < n && c < n) v = G[(int64_t)i * ldg + c] + ((i == c) ? shift : 0.0);
         A[i * LD + c] = v;
+    }
+    if (zero_src != nullptr) {
+        __syncthreads();                                  // every thread has read its part of the scratch input
+        for (int e = tid; e < n * zero_cols; e += 256) {
+            const int i = e / zero_cols, c = e - i * zero_cols;
+            zero_src[(int64_t)i * ldg + c] = 0.0;
+        }
     }
     for (int e = tid; e < n * n; e += 256) {              // exact zeros below the diagonal
         const int i = e / n, c = e - i * n;
-        if (c < i) R1[e] = 0.0;
+        if (c < i) R1[(int64_t)i * ldr + c] = 0.0;
     }
     if (tid == 0) fail_s = 0;
     if (tid < 64) Ts[tid >> 3][tid & 7] = 0.0;            // the strict lower triangle of T stays zero
@@ -603,7 +623,8 @@ k_chol_blocked(const double* __restrict__ G, int n, double shift_h, const double
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
                 const int i = (lane + 32 * h) >> 3, c = (lane + 32 * h) & 7;
-                if (c >= i && 8 * K + c < n) R1[(int64_t)(8 * K + i) * n + 8 * K + c] = A[(8 * K + i) * LD + 8 * K + c];
+                if (c >= i && 8 * K + c < n) R1[(int64_t)(8 * K + i) * ldr + 8 * K + c] = A[(8 * K + i) * LD + 8 * K + c];
+                if (Tsave != nullptr) chol2_tslot(Tsave, ldt, K)[i * ldt + c] = Ts[i][c];
             }
         }
         // (2) row panel: R[K,J] = T^T A[K,J], J > K
@@ -618,8 +639,8 @@ k_chol_blocked(const double* __restrict__ G, int n, double shift_h, const double
             __syncwarp();
             *reinterpret_cast<double2*>(A + (8 * K + r) * LD + 8 * J + 2 * q) = make_double2(c0, c1);
             const int row = 8 * K + r, col = 8 * J + 2 * q;
-            if (row < n && col < n) R1[(int64_t)row * n + col] = c0;
-            if (row < n && col + 1 < n) R1[(int64_t)row * n + col + 1] = c1;
+            if (row < n && col < n) R1[(int64_t)row * ldr + col] = c0;
+            if (row < n && col + 1 < n) R1[(int64_t)row * ldr + col + 1] = c1;
         }
         __syncthreads();
         // (3) trailing update: A[I,J] -= R[K,I]^T R[K,J], K < I <= J
@@ -641,7 +662,7 @@ k_chol_blocked(const double* __restrict__ G, int n, double shift_h, const double
         __syncthreads();
     }
     if (fail_s) {
-        if (tid == 0) rqr_set_info(d_info, RQR_INFO_NOT_SPD + fail_s);
+        if (tid == 0) rqr_set_info(d_info, RQR_INFO_NOT_SPD + info_off + fail_s);
         return;
     }
     if (Rprod != nullptr) {
@@ -677,99 +698,83 @@ k_chol_blocked(const double* __restrict__ G, int n, double shift_h, const double
     }
 }
 
-// n > 128: column-distributed right-looking Cholesky, ONE barrier per step.  Column c -> CTA c % ncta,
-// warp (c / ncta) % NW, slot (c / ncta) / NW; lane l owns rows l + 32 p (rows <= c are used).
-// Step j: every column's warp publishes its row-j entry A[j][c] into a double-buffered row buffer;
-// the lane that owns the pivot A[j][j] also publishes d = A[j][j], r = sqrt(d) and 1/r.  After the
-// barrier every thread forms the entries R[j][a] = A[j][a] (1/r) it needs (same inputs, same
-// operations: identical in every thread) and updates A[a][c] -= R[j][a] R[j][c], j < a <= c.
-// Few warps on purpose: the step is latency-bound and FP64 issue is half rate, so redundant
-// scalar work in 32 warps costs more than the parallelism gains.
-// CL = false: one CTA, row buffer in shared memory; CL = true: a cluster, row buffer in the (not
-// yet written) output R1, cluster barrier.
-#define CHOL_ROW_LD (RQR_MAX_N + 4)      // row entries, then d, r, 1/r
-
-template <int RPL, int CPW, int NW, bool CL>
-__global__ void __launch_bounds__(NW * 32, 1)
-k_chol_cols(const double* __restrict__ G, int n, double shift_h, const double* __restrict__ d_shift,
-            double* R1, int* d_info)
+// ---- two-level Cholesky for 128 < n <= 256 on the blocked kernel: with h = 128 and G = [G11 G12; G12^T G22]
+//   R11 = chol(G11)                     k_chol_blocked, keeps inv(R_KK) of its 16 diagonal blocks
+//   R12 = R11^-T G12                    k_chol2_trsm: one warp per 8 columns, block forward substitution
+//   S   = G22 - R12^T R12               k_chol2_syrk: one warp per 8 x 8 block of the upper triangle
+//   R22 = chol(S)                       k_chol_blocked again (pivot indices offset by h)
+// Scratch is the part of R1 that is zero in the result: the T blocks in the strict lower triangle of the
+// leading block (chol2_tslot), S in the lower-left block R1[h:n, 0:h]; both are zeroed again on the way.
+// k_chol2_trsm computes the TRANSPOSED slice X^T = (B^T[K] - sum_{I<K} X^T[I] R11[I,K]) inv(R_KK): the C fragment
+// of X^T[I] is the A operand of the later products with the k-permuted B fragments (k slot q <-> row 2q + s),
+// so the 16-step chain never leaves the registers.
+__global__ void __launch_bounds__(32)
+k_chol2_trsm(const double* __restrict__ G, int n, double* R1)
 {
-    __shared__ double srow[2][CHOL_ROW_LD];
-    const double shift = shift_h + (d_shift ? *d_shift : 0.0);
-    const int ncta = CL ? (int)cluster_size() : 1, rank = CL ? (int)cluster_rank() : 0;
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    double* rowbuf = CL ? R1 : &srow[0][0];
-    double a[CPW][RPL];
+    constexpr int H = 128, NBH = 16;
+    const int lane = threadIdx.x, r = lane >> 2, q = lane & 3;
+    const int col = H + 8 * blockIdx.x + r;                   // my column of G12 / R12 (row r of the slice^T)
+    const bool colok = col < n;
+    double xs[NBH][2];
 #pragma unroll
-    for (int q = 0; q < CPW; ++q)
+    for (int K = 0; K < NBH; ++K) {
+        // acc = B^T[K]: C fragment (row r, columns 2q, 2q+1) = G[8K + 2q + s][col]
+        double a0 = colok ? G[(int64_t)(8 * K + 2 * q) * n + col] : 0.0;
+        double a1 = colok ? G[(int64_t)(8 * K + 2 * q + 1) * n + col] : 0.0;
+        double b0 = 0.0, b1 = 0.0;                            // second accumulator: two independent chains
 #pragma unroll
-        for (int p = 0; p < RPL; ++p) {
-            const int c = (w + NW * q) * ncta + rank, i = lane + 32 * p;
-            a[q][p] = (c < n && i <= c) ? G[(int64_t)i * n + c] + ((i == c) ? shift : 0.0) : 0.0;
+        for (int I = 0; I < K; ++I) {
+            const double* Rb = R1 + (int64_t)(8 * I + 2 * q) * n + 8 * K + r;     // R11[I,K][2q + s][r]
+            cholb_dmma(a0, a1, -xs[I][0], Rb[0]);
+            cholb_dmma(b0, b1, -xs[I][1], Rb[n]);
         }
-    int fail = 0;
-    // column ids of this thread's slots (c >= n: a padding column, never stored)
-    int col[CPW];
-#pragma unroll
-    for (int q = 0; q < CPW; ++q) col[q] = (w + NW * q) * ncta + rank;
-    for (int j = 0; j < n; ++j) {
-        const int lj = j & 31, pj = j >> 5;
-        double* rb = rowbuf + (j & 1) * CHOL_ROW_LD;
-        // publish row j (branch-free selects; finished columns publish a value nobody reads)
-        double val[CPW];
-#pragma unroll
-        for (int q = 0; q < CPW; ++q) {
-            val[q] = a[q][0];
-#pragma unroll
-            for (int p = 1; p < RPL; ++p) val[q] = (p == pj) ? a[q][p] : val[q];
-        }
-        if (lane == lj) {
-#pragma unroll
-            for (int q = 0; q < CPW; ++q) {
-                if (col[q] < RQR_MAX_N) rb[col[q]] = val[q];
-                if (col[q] == j) {
-                    const double rjj = sqrt(val[q]);
-                    rb[RQR_MAX_N] = val[q];
-                    rb[RQR_MAX_N + 1] = rjj;
-                    rb[RQR_MAX_N + 2] = 1.0 / rjj;
-                }
-            }
-        }
-        if (CL) cluster_sync_all(); else __syncthreads();
-        const double d = CL ? __ldcg(rb + RQR_MAX_N) : rb[RQR_MAX_N];
-        const double rjj = CL ? __ldcg(rb + RQR_MAX_N + 1) : rb[RQR_MAX_N + 1];
-        const double rinv = CL ? __ldcg(rb + RQR_MAX_N + 2) : rb[RQR_MAX_N + 2];
-        double rja[RPL];                                  // R[j][a] for this lane's rows; 0 for a <= j
-#pragma unroll
-        for (int p = 0; p < RPL; ++p) {
-            const int i = lane + 32 * p;
-            const double x = CL ? __ldcg(rb + (i < RQR_MAX_N ? i : 0)) : rb[i < RQR_MAX_N ? i : 0];
-            rja[p] = (i > j && i < n) ? x * rinv : 0.0;
-        }
-        if (!(d > 0.0) || !(d < 1.0e308)) { fail = j + 1; break; }      // uniform: same d everywhere
-#pragma unroll
-        for (int q = 0; q < CPW; ++q) {
-            const int c = col[q];
-            const double x = CL ? __ldcg(rb + (c < RQR_MAX_N ? c : 0)) : rb[c < RQR_MAX_N ? c : 0];
-            // R[j][c]; 0 for finished (c < j) and padding columns so that their entries stay frozen
-            const double rjc = (c == j) ? rjj : ((c > j && c < n) ? x * rinv : 0.0);
-#pragma unroll
-            for (int p = 0; p < RPL; ++p) {
-                const int i = lane + 32 * p;
-                const double upd = fma(-rja[p], rjc, a[q][p]);       // entries with i > c are never read
-                a[q][p] = (i == j && c >= j) ? rjc : upd;
-            }
+        a0 += b0; a1 += b1;
+        const double* T = chol2_tslot(R1, n, K);
+        double y0 = 0.0, y1 = 0.0;
+        cholb_dmma(y0, y1, a0, T[(2 * q) * n + r]);
+        cholb_dmma(y0, y1, a1, T[(2 * q + 1) * n + r]);
+        xs[K][0] = y0; xs[K][1] = y1;
+        if (colok) {
+            R1[(int64_t)(8 * K + 2 * q) * n + col] = y0;
+            R1[(int64_t)(8 * K + 2 * q + 1) * n + col] = y1;
         }
     }
-    if (fail && threadIdx.x == 0 && rank == 0) rqr_set_info(d_info, RQR_INFO_NOT_SPD + fail);
-    if (CL) cluster_sync_all();            // the row buffer lives in R1: all reads done before it is overwritten
-#pragma unroll
-    for (int q = 0; q < CPW; ++q)
-#pragma unroll
-        for (int p = 0; p < RPL; ++p) {
-            const int c = (w + NW * q) * ncta + rank, i = lane + 32 * p;
-            if (c < n && i < n) R1[(int64_t)i * n + c] = (i <= c) ? a[q][p] : 0.0;
+}
+
+__global__ void __launch_bounds__(256)
+k_chol2_syrk(const double* __restrict__ G, int n, double shift_h, const double* __restrict__ d_shift, double* R1)
+{
+    constexpr int H = 128, NBH = 16;
+    const double shift = shift_h + (d_shift ? *d_shift : 0.0);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, r = lane >> 2, q = lane & 3;
+    const int n2 = n - H, NB2 = (n2 + 7) >> 3;
+    if (blockIdx.x == 0) {                                    // the T blocks are not needed any more
+        for (int e = threadIdx.x; e < NBH * 64; e += 256) {
+            const int K = e >> 6, i = (e >> 3) & 7, c = e & 7;
+            chol2_tslot(R1, n, K)[i * n + c] = 0.0;
         }
+    }
+    const int blk = blockIdx.x * 8 + warp;
+    if (blk >= NB2 * (NB2 + 1) / 2) return;
+    int I = 0, rem = blk;
+    while (rem >= NB2 - I) { rem -= NB2 - I; ++I; }
+    const int J = I + rem;
+    const int row = 8 * I + r, c0 = 8 * J + 2 * q;            // inside the trailing block
+    double s0 = 0.0, s1 = 0.0, t0 = 0.0, t1 = 0.0;
+    if (row < n2 && c0 < n2) s0 = G[(int64_t)(H + row) * n + H + c0] + ((row == c0) ? shift : 0.0);
+    if (row < n2 && c0 + 1 < n2) s1 = G[(int64_t)(H + row) * n + H + c0 + 1] + ((row == c0 + 1) ? shift : 0.0);
+    const bool aok = H + 8 * I + r < n, bok = H + 8 * J + r < n;
+#pragma unroll 4
+    for (int k = 0; k < H; k += 8) {
+        const double* Ra = R1 + (int64_t)(k + q) * n + H;     // R12[k + q][.]
+        const double a0 = aok ? -Ra[8 * I + r] : 0.0, a1 = aok ? -Ra[4 * n + 8 * I + r] : 0.0;
+        const double b0 = bok ? Ra[8 * J + r] : 0.0, b1 = bok ? Ra[4 * n + 8 * J + r] : 0.0;
+        cholb_dmma(s0, s1, a0, b0);
+        cholb_dmma(t0, t1, a1, b1);
+    }
+    double* S = R1 + (int64_t)H * n;                          // scratch: R1[h:n, 0:h], leading dimension n
+    if (row < n2 && c0 < n2) S[(int64_t)row * n + c0] = s0 + t0;
+    if (row < n2 && c0 + 1 < n2) S[(int64_t)row * n + c0 + 1] = s1 + t1;
 }
 
 int rqr_chol_dev(const double* G, int n, double shift, const double* d_shift, double* R1,
@@ -798,7 +803,7 @@ int rqr_scholqr3_shift(const double* G, int n, int64_t m, double* d_out, cudaStr
 }
 
 // Rprod != NULL: also Rprod = R1 Rprev (the one-shot drivers' A7), fused into the single-CTA blocked kernel
-// for n <= 128, a separate k_triu_mul launch above that.
+// for n <= 128, a separate k_triu_mul launch above that (two-level factorization, see k_chol2_trsm).
 int rqr_chol_dev(const double* G, int n, double shift, const double* d_shift, double* R1,
                  int* d_info, cudaStream_t st, const double* Rprev, double* Rprod)
 {
@@ -806,18 +811,30 @@ int rqr_chol_dev(const double* G, int n, double shift, const double* d_shift, do
     if (n < 2 || n > RQR_MAX_N) return -2;
     if (!R1) return -4;
     if (G == R1) return -4;
+    static bool attr = false;
+    if (!attr) {
+        cudaFuncSetAttribute(k_chol_blocked, cudaFuncAttributeMaxDynamicSharedMemorySize, 144 * 1024);
+        attr = true;
+    }
+    auto smem_of = [](int nn) { const int np = (nn + 7) & ~7; return (size_t)np * (np + 8 + (np & 8)) * sizeof(double); };
     if (n <= 128) {
-        const int np = (n + 7) & ~7;
-        const size_t sm = (size_t)np * (np + 8 + (np & 8)) * sizeof(double);                         // <= 140 KB
-        static bool attr = false;
-        if (!attr) {
-            cudaFuncSetAttribute(k_chol_blocked, cudaFuncAttributeMaxDynamicSharedMemorySize, 144 * 1024);
-            attr = true;
-        }
-        k_chol_blocked<<<1, 256, sm, st>>>(G, n, shift, d_shift, R1, d_info, Rprev, Rprod);
+        k_chol_blocked<<<1, 256, smem_of(n), st>>>(G, n, n, shift, d_shift, R1, n, d_info, 0, Rprev, Rprod,
+                                                   nullptr, 0, nullptr, 0);
     } else {
-        int rc = launch_cluster(k_chol_cols<8, 4, 8, true>, 8, 256, st, G, n, shift, d_shift, R1, d_info);
-        if (rc != RQR_OK || !Rprod) return rc;
+        // two-level (see k_chol2_trsm): 0.51 ms -> 0.12 ms at n = 256
+        const int h = 128, n2 = n - h, nb2 = (n2 + 7) / 8;
+        double* S = R1 + (int64_t)h * n;
+        k_chol_blocked<<<1, 256, smem_of(h), st>>>(G, n, h, shift, d_shift, R1, n, d_info, 0, nullptr, nullptr,
+                                                   R1, n, nullptr, 0);
+        RQR_LAUNCH_CHECK();
+        k_chol2_trsm<<<nb2, 32, 0, st>>>(G, n, R1);
+        RQR_LAUNCH_CHECK();
+        k_chol2_syrk<<<(nb2 * (nb2 + 1) / 2 + 7) / 8, 256, 0, st>>>(G, n, shift, d_shift, R1);
+        RQR_LAUNCH_CHECK();
+        k_chol_blocked<<<1, 256, smem_of(n2), st>>>(S, n, n2, 0.0, nullptr, R1 + (int64_t)h * n + h, n, d_info, h,
+                                                    nullptr, nullptr, nullptr, 0, S, h);
+        RQR_LAUNCH_CHECK();
+        if (!Rprod) return RQR_OK;
         return rqr_triu_mul(R1, Rprev, n, Rprod, st);
     }
     RQR_LAUNCH_CHECK();

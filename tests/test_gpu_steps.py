@@ -220,7 +220,7 @@ def test_trsm_rowwise_backward_error_with_graded_R(rq):
             rq.force_generic(False)
 
 
-@pytest.mark.parametrize("n", [2, 16, 64, 70, 128, 256])
+@pytest.mark.parametrize("n", [2, 16, 64, 70, 128, 129, 136, 200, 250, 256])
 def test_chol_parity_and_failure(rq, orc, n):
     A = inputs.make_V(4 * n + 3, n, 30.0, n).numpy()
     Gm = A.T @ A
