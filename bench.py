@@ -7,7 +7,8 @@ A "step" is one whole factorization (all SURVEY.md 8(a) rows A1..A7) of one synt
 V = U diag(sigma) W^T of the named workload.  Sketch generation A0 is OFF the clock, the
 paper's convention; `with_sketch_gen` reports the time including it.
 `value` = algorithmic GFLOP/s (paper_2309_05868_b200/flops.py) with V resident in HBM;
-`e2e` = the same through host buffers (H2D of V, D2H of Q and R inside the timed region).
+`e2e` = the same through host buffers (every step uploads its V from pinned host memory and reads Q and R back
+inside the timed region; steps double-buffered over three streams, the one-stream serial figure beside it).
 N > 1: the rows are sharded over ranks (PAPER.md:228 footnote 3), weak scaling.
 """
 from __future__ import annotations
@@ -291,23 +292,70 @@ def run_config(torch, rq, name, args, peaks, p64, want_e2e=True, want_breakdown=
         out["breakdown_ms"] = breakdown(torch, rq, Vd, c, seed, Q, R, bufs, max(3, args.steps // 3),
                                         args.recompute_v1)
     if want_e2e:
+        # End to end through host buffers.  Every step copies its V from pinned host memory and reads its Q and R
+        # back; the steps are pipelined the way a caller streaming panels would run them: double-buffered device
+        # arrays, H2D / factorization / D2H on three streams, so step i's read-back overlaps step i+1's upload
+        # (PCIe is full duplex; the factorization itself is ~30x shorter than either copy).  The serial figure
+        # (one step start to finish on one stream) is reported beside it.
         Vh = torch.empty(Vd.shape, dtype=torch.float64, pin_memory=True)
         Vh.copy_(Vd)
-        Qh = torch.empty(Vd.shape, dtype=torch.float64, pin_memory=True)
-        Rh = torch.empty(n, n, dtype=torch.float64, pin_memory=True)
-        Vin = torch.empty_like(Vd)
+        Qh = [torch.empty(Vd.shape, dtype=torch.float64, pin_memory=True) for _ in range(2)]
+        Rh = [torch.empty(n, n, dtype=torch.float64, pin_memory=True) for _ in range(2)]
+        Vin = [torch.empty_like(Vd), Vd]            # Vd is not needed any more: second input buffer
+        Qd = [Q, torch.empty_like(Vd)]
+        Rd = [R, torch.empty_like(R)]
 
-        def step_e2e():
-            Vin.copy_(Vh, non_blocking=True)
-            rq.rand_cholqr(Vin, s1, s2, seed, Q, R, work, info, 0, flags)
-            Qh.copy_(Q, non_blocking=True)
-            Rh.copy_(R, non_blocking=True)
-        step_e2e()
+        def step_serial():
+            Vin[0].copy_(Vh, non_blocking=True)
+            rq.rand_cholqr(Vin[0], s1, s2, seed, Qd[0], Rd[0], work, info, 0, flags)
+            Qh[0].copy_(Qd[0], non_blocking=True)
+            Rh[0].copy_(Rd[0], non_blocking=True)
+        step_serial()
         k = max(2, min(args.steps, 5))
-        ms_e = time_region(torch, step_e2e, k) / k
-        out["e2e"] = {"value": F / ms_e / 1e6, "unit": "GFLOP/s", "ms_per_step": ms_e,
-                      "h2d_bytes_per_step": int(8 * m * n), "d2h_bytes_per_step": int(8 * m * n + 8 * n * n)}
-        del Vh, Qh, Vin
+        ms_serial = time_region(torch, step_serial, k) / k
+
+        s_in, s_cmp, s_out = torch.cuda.Stream(), torch.cuda.Stream(), torch.cuda.Stream()
+
+        def run_pipeline(steps):
+            ev_in = [None, None]; ev_cmp = [None, None]; ev_out = [None, None]
+            torch.cuda.synchronize()
+            e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+            with torch.cuda.stream(s_in):
+                e0.record()
+            for i in range(steps):
+                b = i & 1
+                with torch.cuda.stream(s_in):
+                    if ev_cmp[b] is not None:
+                        s_in.wait_event(ev_cmp[b])              # the factorization that read Vin[b] is done
+                    Vin[b].copy_(Vh, non_blocking=True)
+                    ev_in[b] = torch.cuda.Event(); ev_in[b].record()
+                with torch.cuda.stream(s_cmp):
+                    s_cmp.wait_event(ev_in[b])
+                    if ev_out[b] is not None:
+                        s_cmp.wait_event(ev_out[b])             # Qd[b], Rd[b] have been read back
+                    rq.rand_cholqr(Vin[b], s1, s2, seed, Qd[b], Rd[b], work, info, 0, flags)
+                    ev_cmp[b] = torch.cuda.Event(); ev_cmp[b].record()
+                with torch.cuda.stream(s_out):
+                    s_out.wait_event(ev_cmp[b])
+                    Qh[b].copy_(Qd[b], non_blocking=True)
+                    Rh[b].copy_(Rd[b], non_blocking=True)
+                    ev_out[b] = torch.cuda.Event(); ev_out[b].record()
+            with torch.cuda.stream(s_out):
+                s_out.wait_stream(s_in); s_out.wait_stream(s_cmp)
+                e1.record()
+            torch.cuda.synchronize()
+            return e0.elapsed_time(e1)
+        run_pipeline(3)
+        ke = max(4, args.steps)
+        ms_e = run_pipeline(ke) / ke
+        ok = bool(int(info.item()) == 0 and torch.equal(Qh[0], Qh[1]) and torch.equal(Rh[0], Rh[1]))
+        out["e2e"] = {"value": F / ms_e / 1e6, "unit": "GFLOP/s", "ms_per_step": ms_e, "steps": ke,
+                      "h2d_bytes_per_step": int(8 * m * n), "d2h_bytes_per_step": int(8 * m * n + 8 * n * n),
+                      "pipeline": "double-buffered; H2D, factorization, D2H on three streams; whole region timed "
+                                  "from the first upload to the last read-back",
+                      "serial_ms_per_step": ms_serial, "serial_value": F / ms_serial / 1e6,
+                      "results_identical_across_buffers": ok}
+        del Vh, Qh, Vin, Qd
     out["_V_host_sample"] = Vd[: min(m, ORACLE_SAMPLE_ROWS)].cpu().numpy() if not args.no_cpu_baseline else None
     del Vd, Q, bufs
     torch.cuda.empty_cache()
