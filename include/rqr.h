@@ -135,6 +135,15 @@ int rqr_rand_cholqr(const double* V, int64_t m, int n, int64_t s1, int s2, uint6
                     double* Q, double* R, void* work, int* d_info, int variant, int flags,
                     void* stream);
 
+/* Batched / strided form for block-Krylov use ("Krylov subspace methods that
+ * require tall-and-skinny QR factorizations, particularly block ..."): `batch` problems of the same shape,
+ * problem b at V + b strideV (m x n, ld n), Q + b strideQ, R + b n^2, d_info + b.  The sketch operator is the
+ * same for every problem (one seed), so the sketch state in `work` is generated once (or not at all with
+ * RQR_FLAG_PREPARED) and the problems run back to back on the stream; each is bit-identical to the single call. */
+int rqr_rand_cholqr_batched(const double* V, int64_t m, int n, int batch, int64_t strideV, int64_t s1, int s2,
+                            uint64_t seed, double* Q, int64_t strideQ, double* R, void* work, int* d_info,
+                            int variant, int flags, void* stream);
+
 /* Comparators on the same kernels.  Alg. 4 CholeskyQR2.                   */
 int rqr_cholqr2(const double* V, int64_t m, int n, double* Q, double* R, void* work, int* d_info,
                 void* stream);

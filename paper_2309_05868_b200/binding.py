@@ -40,6 +40,8 @@ SIGNATURES = {
     "rqr_apply": (_int, [_vp, _i64, _int, _i64, _vp, _vp, _vp, _i64, _vp, _vp]),
     "rqr_triu_mul": (_int, [_vp, _vp, _int, _vp, _vp]),
     "rqr_rand_cholqr": (_int, [_vp, _i64, _int, _i64, _int, _u64, _vp, _vp, _vp, _vp, _int, _int, _vp]),
+    "rqr_rand_cholqr_batched": (_int, [_vp, _i64, _int, _int, _i64, _i64, _int, _u64, _vp, _i64, _vp, _vp, _vp, _int, _int,
+                                       _vp]),
     "rqr_cholqr2": (_int, [_vp, _i64, _int, _vp, _vp, _vp, _vp, _vp]),
     "rqr_scholqr3": (_int, [_vp, _i64, _int, _vp, _vp, _vp, _vp, _vp]),
     "rqr_gauss_randcholqr": (_int, [_vp, _i64, _int, _int, _u64, _vp, _vp, _vp, _vp, _vp]),
@@ -173,6 +175,15 @@ def rand_cholqr(V, s1, s2, seed, Q, R, work, info, variant=VARIANT_SORTED, flags
     assert V.is_contiguous() and Q.is_contiguous()
     _chk(lib().rqr_rand_cholqr(_ptr(V), m, n, s1, s2, seed, _ptr(Q), _ptr(R), _ptr(work), _ptr(info), variant, flags,
                                _stream()), "rqr_rand_cholqr")
+
+
+def rand_cholqr_batched(V, s1, s2, seed, Q, R, work, info, variant=VARIANT_SORTED, flags=0):
+    """V, Q: (batch, m, n) contiguous; R: (batch, n, n); info: (batch,) int32."""
+    _f64(V, "V"); _f64(Q, "Q"); _f64(R, "R")
+    batch, m, n = V.shape
+    assert V.is_contiguous() and Q.is_contiguous() and R.is_contiguous() and info.numel() >= batch
+    _chk(lib().rqr_rand_cholqr_batched(_ptr(V), m, n, batch, m * n, s1, s2, seed, _ptr(Q), m * n, _ptr(R), _ptr(work),
+                                       _ptr(info), variant, flags, _stream()), "rqr_rand_cholqr_batched")
 
 
 def cholqr2(V, Q, R, work, info):

@@ -84,6 +84,24 @@ extern "C" int rqr_rand_cholqr(const double* V, int64_t m, int n, int64_t s1, in
     return RQR_OK;
 }
 
+extern "C" int rqr_rand_cholqr_batched(const double* V, int64_t m, int n, int batch, int64_t strideV, int64_t s1,
+                                       int s2, uint64_t seed, double* Q, int64_t strideQ, double* R, void* work,
+                                       int* d_info, int variant, int flags, void* stream)
+{
+    if (batch < 1) return -4;
+    if (strideV < m * n || strideQ < m * n) return -5;
+    if (!V || !Q || !R) return !V ? -1 : (!Q ? -9 : -11);
+    if (!(flags & RQR_FLAG_PREPARED)) {
+        if (m < 1 || n < 2 || n > RQR_MAX_N || !work) return -2;
+        RQR_TRY(rqr_sketch_prepare(m, n, 0, s1, s2, seed, variant, work, (cudaStream_t)stream));
+    }
+    for (int b = 0; b < batch; ++b)
+        RQR_TRY(rqr_rand_cholqr(V + (int64_t)b * strideV, m, n, s1, s2, seed, Q + (int64_t)b * strideQ,
+                                R + (int64_t)b * n * n, work, d_info ? d_info + b : nullptr, variant,
+                                flags | RQR_FLAG_PREPARED, stream));
+    return RQR_OK;
+}
+
 extern "C" int rqr_gauss_randcholqr(const double* V, int64_t m, int n, int s, uint64_t seed,
                                     double* Q, double* R, void* work, int* d_info, void* stream)
 {

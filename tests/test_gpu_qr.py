@@ -417,3 +417,23 @@ def test_rademacher_full_size_C2(rq):
     Q, R, info = run_rand(rq, Vd, s1, s2, 42, rq.S2_RADEMACHER, 0, True)
     assert info == 0 and orth_err(Q) <= ORTH_TOL and resid(Vd, Q, R) <= RES_TOL
     check_R(R)
+
+
+def test_batched_is_bit_identical_to_single_calls(rq):
+    """N4, batched / strided interface: one sketch state, the problems back to back; every problem must equal its
+    own single call bit for bit, and a failing problem must not disturb its neighbours' info."""
+    batch, m, n = 4, 30000, 48
+    s1, s2 = inputs.sketch_sizes(n)
+    V = torch.stack([inputs.make_V(m, n, 10.0 ** (3 * b), 100 + b) for b in range(batch)]).cuda().contiguous()
+    V[2, :, 5] = 0.0                                      # problem 2 is rank deficient
+    Q = torch.empty_like(V); R = torch.empty(batch, n, n, dtype=torch.float64, device="cuda")
+    info = torch.zeros(batch, dtype=torch.int32, device="cuda")
+    work = rq.alloc_workspace(m, n, s1, s2)
+    rq.rand_cholqr_batched(V, s1, s2, 42, Q, R, work, info)
+    torch.cuda.synchronize()
+    infos = info.cpu().tolist()
+    assert infos[0] == 0 and infos[1] == 0 and infos[3] == 0 and infos[2] != 0
+    for b in (0, 1, 3):
+        Qs, Rs, i1 = run_rand(rq, V[b].contiguous(), s1, s2, 42)
+        assert i1 == 0 and torch.equal(Qs, Q[b]) and torch.equal(Rs, R[b])
+        assert orth_err(Q[b]) <= ORTH_TOL and resid(V[b], Q[b], R[b]) <= RES_TOL
