@@ -116,8 +116,10 @@ int rqr_trsm_gram(const double* V, int64_t m, int n, int64_t ldv, const double* 
                   double* V1, int64_t ldq, void* work, void* stream);
 
 /* A5 -- upper Cholesky factor, G + shift I = R1^T R1 (Alg. 2 step 2).  R1 is n x n
- * upper triangular with diag > 0 and exact zeros below; it must not alias G (its storage is the
- * exchange buffer of the cluster kernel for n > 128).                                        */
+ * upper triangular with diag > 0 and exact zeros below; it must not alias G (for n > 128 the part
+ * of R1 that ends up zero is scratch during the call: inverse diagonal blocks and the Schur
+ * complement of the two-level factorization live there).  First failing pivot j (0-based):
+ * *d_info = RQR_INFO_NOT_SPD + j + 1.                                                         */
 int rqr_chol(const double* G, int n, double shift, double* R1, int* d_info, void* stream);
 
 /* A6 -- Q = (V R0^-1) R1^-1 (Alg. 2 step 3), never V (R0^-1 R1^-1).
