@@ -82,22 +82,37 @@ __device__ __forceinline__ double r_padded(const double* __restrict__ R, int n, 
     return (i < n && c < n) ? __ldg(R + i * n + c) : ((i == c) ? 1.0 : 0.0);
 }
 
+// `stage`: (8 NB)^2 doubles of shared memory that are free in the prologue (the callers pass their landing ring
+// and zero it afterwards).  The diagonal panel of R is staged there with coalesced loads first, so the back
+// substitution (64 threads, a dependent chain) and the fragment fills read shared memory instead of L2, and the
+// divisions by the diagonal are 8 independent reciprocals up front: 11 -> 3 us of prologue at n = 64.
 template <int NB>
 __device__ void build_tri_frags(const double* __restrict__ R, int n, double* __restrict__ Tf,
                                 double* __restrict__ nRf, double* __restrict__ scratch /* NB*64 */,
+                                double* __restrict__ stage /* (8 NB)^2 */,
                                 int base = 0 /* first row/column of the diagonal panel */)
 {
+    constexpr int N = 8 * NB;
     const int tid = threadIdx.x;
+    for (int t = tid; t < N * N; t += blockDim.x) {
+        const int i = t / N, c = t - i * N;
+        stage[t] = r_padded(R, n, base + i, base + c);
+    }
+    __syncthreads();
     // T_J column c by back substitution: R_JJ t = e_c  (one thread per (J, c))
     for (int t = tid; t < NB * 8; t += blockDim.x) {
         const int J = t >> 3, c = t & 7;
+        const double* D = stage + (8 * J) * N + 8 * J;
+        double rinv[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) rinv[i] = 1.0 / D[i * N + i];
         double tc[8];
 #pragma unroll
         for (int i = 7; i >= 0; --i) {
             double s = (i == c) ? 1.0 : 0.0;
 #pragma unroll
-            for (int k = 7; k > i; --k) s = fma(-r_padded(R, n, base + 8 * J + i, base + 8 * J + k), tc[k], s);
-            tc[i] = (i <= c) ? s / r_padded(R, n, base + 8 * J + i, base + 8 * J + i) : 0.0;
+            for (int k = 7; k > i; --k) s = fma(-D[i * N + k], tc[k], s);
+            tc[i] = (i <= c) ? s * rinv[i] : 0.0;
         }
 #pragma unroll
         for (int i = 0; i < 8; ++i) scratch[J * 64 + i * 8 + c] = tc[i];
@@ -113,7 +128,7 @@ __device__ void build_tri_frags(const double* __restrict__ R, int n, double* __r
         int J = 0, rem = p;
         while (rem >= NB - 1 - J) { rem -= NB - 1 - J; ++J; }
         const int Jp = J + 1 + rem;
-        nRf[t] = -r_padded(R, n, base + 8 * J + 2 * (lane & 3) + h, base + 8 * Jp + (lane >> 2));
+        nRf[t] = -stage[(8 * J + 2 * (lane & 3) + h) * N + 8 * Jp + (lane >> 2)];
     }
     __syncthreads();
 }

@@ -50,12 +50,14 @@ k_trsm_gram_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     double* xs = smem + Plan::xs + (size_t)warp * 2 * 8 * N8;
 
-    for (int i = threadIdx.x; i < (int)Plan::ring_doubles; i += blockDim.x) ring[i] = 0.0;
+    static_assert(Plan::ring_doubles >= 64 * NB * NB, "ring too small to stage R");
     if (threadIdx.x < GramWarps<NB>::value * GRAM_STAGES) mbar_init(bars + threadIdx.x, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    if (HAS_R) build_tri_frags<NB>(R0, n, Tf, nRf, scratch, ring);      // stages R in the (still unused) ring
+    // rows of a partial last row-block that the bulk copies do not write must be zero (they enter the Gram)
+    for (int i = threadIdx.x; i < (int)Plan::ring_doubles; i += blockDim.x) ring[i] = 0.0;
     fence_proxy_async();
     __syncthreads();
-    if (HAS_R) build_tri_frags<NB>(R0, n, Tf, nRf, scratch);
 
     WarpRing<LDL> wr{ring + (size_t)warp * GRAM_STAGES * 8 * LDL, bars + warp * GRAM_STAGES, V, ldv, m, n};
     const XsAddr<N8> ad(lane);
@@ -169,6 +171,15 @@ struct PairSet {
         return row(i) + k;
     }
 };
+
+// (a << 4 | b) of Gram block k of side 0 (entries 0..17) and side 1 (18..35), for the epilogue
+#define PAB(S, K) (unsigned char)((PairSet<S>::a(K) << 4) | PairSet<S>::b(K))
+__constant__ unsigned char c_pair_ab[36] = {
+    PAB(0, 0), PAB(0, 1), PAB(0, 2), PAB(0, 3), PAB(0, 4), PAB(0, 5), PAB(0, 6), PAB(0, 7), PAB(0, 8),
+    PAB(0, 9), PAB(0, 10), PAB(0, 11), PAB(0, 12), PAB(0, 13), PAB(0, 14), PAB(0, 15), PAB(0, 16), PAB(0, 17),
+    PAB(1, 0), PAB(1, 1), PAB(1, 2), PAB(1, 3), PAB(1, 4), PAB(1, 5), PAB(1, 6), PAB(1, 7), PAB(1, 8),
+    PAB(1, 9), PAB(1, 10), PAB(1, 11), PAB(1, 12), PAB(1, 13), PAB(1, 14), PAB(1, 15), PAB(1, 16), PAB(1, 17)};
+#undef PAB
 
 // Gram DMMAs [T0, T1) of an iteration: t -> row-block t / 36 of the pair, slab (t % 36) / 18, block t % 18
 template <int SIDE, int T0, int T1>
@@ -294,12 +305,13 @@ k_trsm_gram_pair(const double* __restrict__ V, int64_t m, int n, int64_t ldv, co
     double* ring = smem + PairPlan::ring;
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + PairPlan::bars);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    for (int i = threadIdx.x; i < (int)PairPlan::ring_doubles; i += blockDim.x) ring[i] = 0.0;
+    static_assert(PairPlan::ring_doubles >= 64 * 64, "ring too small to stage R");
     if (threadIdx.x < PAIR_WARPS * PAIR_STAGES) mbar_init(bars + threadIdx.x, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    build_tri_frags<8>(R0, n, smem, smem + 8 * 64, smem + PairPlan::scratch, ring);
+    for (int i = threadIdx.x; i < (int)PairPlan::ring_doubles; i += blockDim.x) ring[i] = 0.0;
     fence_proxy_async();
     __syncthreads();
-    build_tri_frags<8>(R0, n, smem, smem + 8 * 64, smem + PairPlan::scratch);
 
     double G[18][2];
 #pragma unroll
@@ -317,15 +329,20 @@ k_trsm_gram_pair(const double* __restrict__ V, int64_t m, int n, int64_t ldv, co
     }
     __syncthreads();
     double* P = part + (size_t)blockIdx.x * n * n;
-    for (int e = threadIdx.x; e < 2 * 18 * 64; e += blockDim.x) {
-        const int side = e / (18 * 64), k = (e / 64) % 18, l = (e >> 1) & 31, kk = e & 1;
-        double s = 0.0;
+    // thread = (block j = side * 18 + k of the 36 upper blocks: threadIdx / 64 + 6 i, element threadIdx % 64)
+    const int l = (threadIdx.x >> 1) & 31, kk = threadIdx.x & 1;
 #pragma unroll
-        for (int p = 0; p < PAIR_WARPS / 2; ++p) s += red[((size_t)(2 * p + side) * 18 + k) * 64 + 2 * l + kk];
-        const int a = side ? PairSet<1>::a(k) : PairSet<0>::a(k);
-        const int bb = side ? PairSet<1>::b(k) : PairSet<0>::b(k);
-        const int row = 8 * a + (l >> 2), col = 8 * bb + 2 * (l & 3) + kk;
-        if (row < n && col < n) P[row * n + col] = s;
+    for (int i = 0; i < 6; ++i) {
+        const int j = (threadIdx.x >> 6) + (PAIR_WARPS * 32 / 64) * i;       // 384 threads: 6 blocks per pass
+        if (j < 36) {
+            const int side = j >= 18, k = j - 18 * side;
+            double s = 0.0;
+#pragma unroll
+            for (int p = 0; p < PAIR_WARPS / 2; ++p) s += red[((size_t)(2 * p + side) * 18 + k) * 64 + 2 * l + kk];
+            const int ab = c_pair_ab[j];
+            const int row = 8 * (ab >> 4) + (l >> 2), col = 8 * (ab & 15) + 2 * (l & 3) + kk;
+            if (row < n && col < n) P[row * n + col] = s;
+        }
     }
 }
 
@@ -361,13 +378,14 @@ k_apply_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
     double* ring = smem + Plan::ring;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 
-    for (int i = threadIdx.x; i < (int)Plan::ring_doubles; i += blockDim.x) ring[i] = 0.0;
+    static_assert(Plan::ring_doubles >= 64 * NB * NB, "ring too small to stage R");
     if (threadIdx.x < ApplyCfg<NB, TWO>::WARPS * ApplyCfg<NB, TWO>::STAGES) mbar_init(bars + threadIdx.x, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    build_tri_frags<NB>(R1, n, Tf1, nRf1, scratch, ring);
+    if (TWO) build_tri_frags<NB>(R0, n, Tf0, nRf0, scratch, ring);
+    for (int i = threadIdx.x; i < (int)Plan::ring_doubles; i += blockDim.x) ring[i] = 0.0;
     fence_proxy_async();
     __syncthreads();
-    build_tri_frags<NB>(R1, n, Tf1, nRf1, scratch);
-    if (TWO) build_tri_frags<NB>(R0, n, Tf0, nRf0, scratch);
 
     WarpRing<LDL> wr{ring + (size_t)warp * ApplyCfg<NB, TWO>::STAGES * 8 * LDL, bars + warp * ApplyCfg<NB, TWO>::STAGES, V, ldv, m, n};
     const XsAddr<N8> ad(lane);

@@ -50,12 +50,13 @@ __global__ void __launch_bounds__(256)
 k_build_panel_frags(const double* __restrict__ R, int n, double* __restrict__ frags, int np, int last_nb)
 {
     __shared__ double scratch[8 * 64];
+    __shared__ double stage[64 * 64];
     int Pp, P;
     panel_slot_decode(blockIdx.x, Pp, P);
     double* out = frags + (size_t)blockIdx.x * PANEL_SLOT;
     if (Pp == P) {
-        if (P == np - 1 && last_nb == 4) build_tri_frags<4>(R, n, out, out + 256, scratch, 64 * P);
-        else build_tri_frags<8>(R, n, out, out + 512, scratch, 64 * P);
+        if (P == np - 1 && last_nb == 4) build_tri_frags<4>(R, n, out, out + 256, scratch, stage, 64 * P);
+        else build_tri_frags<8>(R, n, out, out + 512, scratch, stage, 64 * P);
     } else {
         for (int t = threadIdx.x; t < PANEL_SLOT; t += blockDim.x) {
             const int jj = t >> 6, h = (t >> 5) & 1, lane = t & 31;
