@@ -94,7 +94,8 @@ __device__ void build_tri_frags(const double* __restrict__ R, int n, double* __r
 {
     constexpr int N = 8 * NB;
     const int tid = threadIdx.x;
-    for (int t = tid; t < N * N; t += blockDim.x) {
+#pragma unroll 4
+    for (int t = tid; t < N * N; t += blockDim.x) {                 // unrolled: 4 loads of L2 latency in flight
         const int i = t / N, c = t - i * N;
         stage[t] = r_padded(R, n, base + i, base + c);
     }
