@@ -158,7 +158,8 @@ int rqr_scholqr3(const double* V, int64_t m, int n, double* Q, double* R, void* 
 int rqr_gauss_randcholqr(const double* V, int64_t m, int n, int s, uint64_t seed, double* Q,
                          double* R, void* work, int* d_info, void* stream);
 /* rand_cholQR with ONE CountSketch (the paper's "Sparse" rows): R0 = R factor of the
- * Householder QR of the s1 x n sketch W1 = S1 V itself, computed by a TSQR tree.  n <= 64 in this version.   */
+ * Householder QR of the s1 x n sketch W1 = S1 V itself, computed by a TSQR tree (n <= 64: 128-row blocks in the
+ * register-resident kernel; n > 64: 1024- / 512-row blocks, one thread-block cluster per block).              */
 int rqr_count_randcholqr(const double* V, int64_t m, int n, int64_t s1, uint64_t seed, double* Q,
                          double* R, void* work, int* d_info, int variant, int flags, void* stream);
 /* R factor (n x n upper, diag > 0) of the Householder QR of a tall A (rows x n row-major, ld n, n <= 64,

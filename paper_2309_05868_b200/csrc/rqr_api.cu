@@ -7,6 +7,7 @@ int rqr_chol_dev(const double* G, int n, double shift, const double* d_shift, do
                  int* d_info, cudaStream_t st, const double* Rprev, double* Rprod);
 int rqr_scholqr3_shift(const double* G, int n, int64_t m, double* d_out, cudaStream_t st);
 int rqr_tsqr_r_dev(const double* A, int64_t rows, int n, double* R, double* scratch, int* d_info, cudaStream_t st);
+int rqr_tsqr_r_wide_dev(double* A, int64_t rows, int n, double* R, double* scratch, int* d_info, cudaStream_t st);
 
 extern "C" const char* rqr_version(void) { return "rqr 0.1 (sm_100a)"; }
 
@@ -144,8 +145,9 @@ extern "C" int rqr_count_randcholqr(const double* V, int64_t m, int n, int64_t s
     int rc = check_common(V, m, n, Q, R, work);
     if (rc == -100) return !Q ? -6 : (!R ? -7 : -8);
     if (rc != RQR_OK) return rc;
-    if (n > 64) return -3;
-    if (s1 < n || s1 >= ((int64_t)1 << 31) || s1 > m || s1 > tsqr_max_rows(n)) return -4;
+    // n <= 64: tree of 128-row register-resident blocks; n > 64: blocks of 1024 / 512 rows in the cluster kernel
+    const int64_t max_rows = n <= 64 ? tsqr_max_rows(n) : (int64_t)(n <= 128 ? 1024 : 512) * rqr_gram_partial_cap(n);
+    if (s1 < n || s1 >= ((int64_t)1 << 31) || s1 > m || s1 > max_rows) return -4;
     if (variant != RQR_VARIANT_SORTED && variant != RQR_VARIANT_SCATTER) return -10;
     cudaStream_t st = (cudaStream_t)stream;
     RqrLayout L = rqr_layout(m, n, s1);
@@ -155,7 +157,8 @@ extern "C" int rqr_count_randcholqr(const double* V, int64_t m, int n, int64_t s
     double* W1 = (double*)((char*)work + L.F_W1);
     if (d_info && cudaMemsetAsync(d_info, 0, sizeof(int), st) != cudaSuccess) return RQR_ERR_LAUNCH;
     RQR_TRY(rqr_countsketch(V, m, n, n, 0, s1, seed, W1, work, variant, flags & RQR_FLAG_PREPARED, st));
-    RQR_TRY(rqr_tsqr_r_dev(W1, s1, n, R0, (double*)((char*)work + 256), d_info, st));
+    if (n <= 64) RQR_TRY(rqr_tsqr_r_dev(W1, s1, n, R0, (double*)((char*)work + 256), d_info, st));
+    else RQR_TRY(rqr_tsqr_r_wide_dev(W1, s1, n, R0, (double*)((char*)work + 256), d_info, st));
     RQR_TRY(tail_cholqr(V, m, n, R0, Q, R1, G, work, d_info, flags & RQR_FLAG_RECOMPUTE_V1, st, R));
     return RQR_OK;
 }

@@ -356,10 +356,21 @@ __device__ __forceinline__ void cluster_sync_all()
 // it (L2) with ONE cluster barrier per Householder step.
 template <int RPL, int CPW>
 __global__ void __launch_bounds__(512, 1)
-k_geqrf_cluster(double* W, int s2, int n, double* __restrict__ R0, int* d_info)
+k_geqrf_cluster(double* W, int s2, int n, double* R0, int* d_info, int64_t rows_total, int nb)
 {
     __shared__ double vs[32 * RPL];          // this step's reflector (registers hold the columns only)
     const int ncta = (int)cluster_size(), rank = (int)cluster_rank();
+    if (nb > 0) {
+        // one level of a TSQR tree (n > 64): cluster c factors rows [c rows_total / nb, (c+1) rows_total / nb) of W
+        // (at most 32 RPL each, destroyed) and writes its R factor to R0 + c n^2; a rank-deficient BLOCK is not an
+        // error of the tree
+        const int64_t cid = blockIdx.x / ncta;
+        const int64_t r0 = cid * rows_total / nb, r1 = (cid + 1) * rows_total / nb;
+        W += r0 * n;
+        s2 = (int)(r1 - r0);
+        R0 += cid * (int64_t)n * n;
+        d_info = nullptr;
+    }
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     double a[CPW][RPL];
 #pragma unroll
@@ -453,6 +464,25 @@ k_geqrf_cluster(double* W, int s2, int n, double* __restrict__ R0, int* d_info)
 }
 
 template <class K, class... Args>
+static int launch_cluster_grid(K kernel, int nclusters, int ncta, int threads, cudaStream_t st, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(nclusters * ncta);
+    cfg.blockDim = dim3(threads);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = ncta;
+    at[0].val.clusterDim.y = 1;
+    at[0].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    if (cudaLaunchKernelEx(&cfg, kernel, args...) != cudaSuccess) return RQR_ERR_LAUNCH;
+    return RQR_OK;
+}
+
+template <class K, class... Args>
 static int launch_cluster(K kernel, int ncta, int threads, cudaStream_t st, Args... args)
 {
     cudaLaunchConfig_t cfg = {};
@@ -497,15 +527,36 @@ extern "C" int rqr_small_geqrf(double* W, int s2, int n, double* R0, int* d_info
     if ((int64_t)s2 * n >= 2 * 32 * rpl + 2 + n) {
         if (rpl <= 16) {
             const int ncta = n <= 128 ? 4 : 8;                     // 16 warps x 2 columns per CTA
-            if (rpl <= 8) return launch_cluster(k_geqrf_cluster<8, 2>, ncta, 512, st, W, s2, n, R0, d_info);
-            return launch_cluster(k_geqrf_cluster<16, 2>, ncta, 512, st, W, s2, n, R0, d_info);
+            if (rpl <= 8) return launch_cluster(k_geqrf_cluster<8, 2>, ncta, 512, st, W, s2, n, R0, d_info, (int64_t)0, 0);
+            return launch_cluster(k_geqrf_cluster<16, 2>, ncta, 512, st, W, s2, n, R0, d_info, (int64_t)0, 0);
         }
         if (n <= 128)                                              // tall sketches of the paper's grid (s2 <= 1024)
-            return launch_cluster(k_geqrf_cluster<32, 1>, n <= 64 ? 4 : 8, 512, st, W, s2, n, R0, d_info);
+            return launch_cluster(k_geqrf_cluster<32, 1>, n <= 64 ? 4 : 8, 512, st, W, s2, n, R0, d_info, (int64_t)0, 0);
     }
     k_geqrf_gmem<<<1, 1024, 0, st>>>(W, s2, n, R0, d_info);
     RQR_LAUNCH_CHECK();
     return RQR_OK;
+}
+
+// TSQR tree for 64 < n <= 256 (the single-CountSketch variant N3 at the paper's larger widths): blocks of at most
+// 1024 (n <= 128) or 512 rows go through the cluster kernel, one cluster per block, level by level; the stacked R
+// factors ping-pong between `scratch` and A itself, which is DESTROYED.  scratch: ceil(rows / block rows) n^2 doubles.
+int rqr_tsqr_r_wide_dev(double* A, int64_t rows, int n, double* R, double* scratch, int* d_info, cudaStream_t st)
+{
+    const int BR = n <= 128 ? 1024 : 512;
+    double* in = A;
+    double* out = scratch;
+    int64_t rows_in = rows;
+    for (;;) {
+        const int64_t nb = (rows_in + BR - 1) / BR;
+        if (nb <= 1) return rqr_small_geqrf(in, (int)rows_in, n, R, d_info, st);
+        int rc;
+        if (n <= 128) rc = launch_cluster_grid(k_geqrf_cluster<32, 1>, (int)nb, 8, 512, st, in, 0, n, out, (int*)nullptr, rows_in, (int)nb);
+        else          rc = launch_cluster_grid(k_geqrf_cluster<16, 2>, (int)nb, 8, 512, st, in, 0, n, out, (int*)nullptr, rows_in, (int)nb);
+        if (rc != RQR_OK) return rc;
+        double* t = in; in = out; out = t;
+        rows_in = nb * n;
+    }
 }
 
 // =========================================================================================

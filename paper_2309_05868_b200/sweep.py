@@ -1,6 +1,6 @@
 """C5 sweep (BASELINE.json configs[4]): m in {2^17..2^25} x n in {32, 64, 128}, sigma log-spaced 1 -> 1e-12;
 rand_cholQR (Count-Gauss, s1 = 2n^2, s2 = 2n) vs single-Gaussian-sketch rand_cholQR vs CholeskyQR2 vs shifted
-CholeskyQR3 (and, for n <= 64, single-CountSketch rand_cholQR) on the same kernels, each reported as a fraction of its own FP64/HBM roofline.
+CholeskyQR3 and single-CountSketch rand_cholQR on the same kernels, each reported as a fraction of its own FP64/HBM roofline.
 
   python -m paper_2309_05868_b200.sweep [--n 32 64 128] [--logm 17 25] [--reps 10] [--out sweep.jsonl]
 
@@ -87,9 +87,8 @@ def run_point(m, n, reps, p64, hbm):
                               lambda: rq.gauss_randcholqr(V, s2, 42, Q, R, work, info)),
         "cholqr2": (flops.cholqr2_flops(m, n), 32.0 * m * n, lambda: rq.cholqr2(V, Q, R, work, info)),
         # one CountSketch, Householder QR of the s1 x n sketch itself (the paper's "Sparse" rows)
-        **({"count_rand_cholqr": (m * n + 2.0 * s1 * n * n - 2.0 * n ** 3 / 3.0 + 3.0 * m * n * n, 32.0 * m * n,
-                                  lambda: rq.count_randcholqr(V, s1, 42, Q, R, work, info, 0, rq.FLAG_PREPARED))}
-           if n <= 64 else {}),
+        "count_rand_cholqr": (m * n + 2.0 * s1 * n * n - 2.0 * n ** 3 / 3.0 + 3.0 * m * n * n, 32.0 * m * n,
+                              lambda: rq.count_randcholqr(V, s1, 42, Q, R, work, info, 0, rq.FLAG_PREPARED)),
         "scholqr3": (6.0 * m * n * n, 48.0 * m * n, lambda: rq.scholqr3(V, Q, R, work, info)),
     }
     for name, (F, B, fn) in models.items():

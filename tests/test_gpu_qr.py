@@ -283,10 +283,12 @@ def test_coherent_input_meets_the_bar(rq, m, n):
     assert num ** 0.5 / float(torch.linalg.norm(Vd)) <= RES_TOL
 
 
-@pytest.mark.parametrize("m,n,kappa", [(65536, 64, 1e12), (40000, 32, 1e14), (20000, 16, 1e10), (100000, 50, 1e8)])
+@pytest.mark.parametrize("m,n,kappa", [(65536, 64, 1e12), (40000, 32, 1e14), (20000, 16, 1e10), (100000, 50, 1e8),
+                                       (40000, 96, 1e10), (60000, 128, 1e12), (50000, 70, 1e8), (140000, 256, 1e12)])
 def test_single_countsketch_rand_cholqr(rq, orc, m, n, kappa):
     """SURVEY.md 8(f) N3, the paper's "Sparse" rows: rand_cholQR with ONE CountSketch, R0 from
-    the Householder QR of the s1 x n sketch (a TSQR tree on the GPU).  Oracle: the same steps composed from the
+    the Householder QR of the s1 x n sketch (a TSQR tree on the GPU: 128-row register blocks for n <= 64, 1024- / 512-row
+    cluster blocks above).  Oracle: the same steps composed from the
     oracle's functions (CountSketch, plain Householder R, substitution, Gram, Cholesky, substitution, product)."""
     s1 = 2 * n * n
     V = inputs.make_V(m, n, kappa, 606)
