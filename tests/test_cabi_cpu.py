@@ -69,6 +69,18 @@ def test_argument_validation_without_gpu(lib):
     assert lib.rqr_cholqr2(z, 100, 8, one, one, one, z, z) == -1
     assert lib.rqr_sketch_prepare(100, 8, 0, 64, 600, 1, 0, one, z) == -5
     assert lib.rqr_probe_fp64(5, 1, 1, one, z, z) == -1
+    # batched / strided one-shot and the Rademacher test hook
+    assert lib.rqr_rand_cholqr_batched(one, 100, 8, 0, 800, 64, 16, 1, one, 800, one, one, z, 0, 1, z) == -4     # batch < 1
+    assert lib.rqr_rand_cholqr_batched(one, 100, 8, 2, 799, 64, 16, 1, one, 800, one, one, z, 0, 1, z) == -5     # stride < m n
+    assert lib.rqr_rand_cholqr_batched(z, 100, 8, 2, 800, 64, 16, 1, one, 800, one, one, z, 0, 1, z) == -1
+    assert lib.rqr_debug_rademacher(1, 100, 2000, 0, 10, one, z) == -3                                          # row
+    assert lib.rqr_debug_rademacher(1, 100, 3, 95, 10, one, z) == -4                                            # past s1
+    # the Rademacher S2 needs no S2 slot: 8 * 1024 * ld bytes less
+    full = lib.rqr_workspace_bytes(1 << 20, 64, 8192, 128, 0)
+    lean = lib.rqr_workspace_bytes(1 << 20, 64, 8192, 128, 16)
+    assert full - lean == 8 * 1024 * 8192
+    assert lib.rqr_rand_cholqr(one, 100, 8, 64, 16, 1, one, one, one, z, 2, 0, z) == -11                         # variant
+    assert lib.rqr_rand_cholqr(one, 100, 8, 64, 16, 1, one, one, one, z, 32, 0, z) == -11
 
 
 def test_binding_refuses_cpu_tensors(lib):
