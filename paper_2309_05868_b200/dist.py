@@ -22,12 +22,18 @@ def shard_rows(m_total: int, world: int, rank: int) -> tuple[int, int]:
     return row0, rows
 
 
+S2_RADEMACHER = 16      # same value as RQR_S2_RADEMACHER in include/rqr.h
+
+
 def rand_cholqr_sharded(ops, V_local, row0, s1, s2, seed, Q_local, R, bufs, group=None, flags=0,
                         variant=0):
     """One factorization step on this rank's block rows.  bufs: dict with W1 (s1 x n), W (s2 x n),
-    R0, R1, G (n x n), work, info.  All ranks end with the same R; Q_local holds this rank's rows."""
+    R0, R1, G (n x n), work, info.  All ranks end with the same R; Q_local holds this rank's rows.
+    variant | S2_RADEMACHER: the replicated S2 is the on-the-fly Rademacher sketch (N4): no rank stores it
+    (bufs must come from alloc_bufs with the same variant)."""
+    rad = variant & S2_RADEMACHER
     ops.countsketch(V_local, s1, seed, bufs["W1"], bufs["work"], variant, flags, row0)
-    ops.gauss_sketch(bufs["W1"], s2, seed, bufs["W"], bufs["work"], flags)
+    ops.gauss_sketch(bufs["W1"], s2, seed, bufs["W"], bufs["work"], flags | rad)
     if dist.is_initialized() and dist.get_world_size(group) > 1:
         dist.all_reduce(bufs["W"], op=dist.ReduceOp.SUM, group=group)        # reduction 1
     ops.small_geqrf(bufs["W"], bufs["R0"], bufs["info"])
@@ -39,8 +45,8 @@ def rand_cholqr_sharded(ops, V_local, row0, s1, s2, seed, Q_local, R, bufs, grou
     ops.triu_mul(bufs["R1"], bufs["R0"], R)
 
 
-def alloc_bufs(ops, m_local, n, s1, s2, device):
+def alloc_bufs(ops, m_local, n, s1, s2, device, variant=0):
     f = dict(dtype=torch.float64, device=device)
     return {"W1": torch.empty(s1, n, **f), "W": torch.empty(s2, n, **f), "R0": torch.empty(n, n, **f),
             "R1": torch.empty(n, n, **f), "G": torch.empty(n, n, **f),
-            "work": ops.alloc_workspace(m_local, n, s1, s2), "info": ops.new_info()}
+            "work": ops.alloc_workspace(m_local, n, s1, s2, variant), "info": ops.new_info()}

@@ -23,17 +23,19 @@ class OracleOps:
         rqr_oracle.build()
         self.o = rqr_oracle
 
-    def alloc_workspace(self, m, n, s1, s2):
+    def alloc_workspace(self, m, n, s1, s2, variant=0):
         return torch.empty(1, dtype=torch.uint8)
 
     def new_info(self):
         return torch.zeros(1, dtype=torch.int32)
 
     def countsketch(self, V, s1, seed, W1, work, variant=0, flags=0, row0=0):
+        assert (variant & ~rdist.S2_RADEMACHER) in (0, 1)
         W1.copy_(torch.from_numpy(self.o.countsketch(V.numpy(), s1, seed, row0=row0)))
 
     def gauss_sketch(self, W1, s2, seed, W, work, flags=0):
-        W.copy_(torch.from_numpy(self.o.gauss_sketch(W1.numpy(), s2, seed)))
+        sk = self.o.rademacher_sketch if flags & rdist.S2_RADEMACHER else self.o.gauss_sketch
+        W.copy_(torch.from_numpy(sk(W1.numpy(), s2, seed)))
 
     def small_geqrf(self, W, R0, info=None):
         R, st = self.o.hhqr_r(W.numpy())
@@ -71,7 +73,7 @@ def _free_port():
     return p
 
 
-def _worker(rank, world, port, m, n, kappa, s1, s2, seed, out_dir):
+def _worker(rank, world, port, m, n, kappa, s1, s2, seed, out_dir, variant=0):
     os.environ["MASTER_ADDR"] = "127.0.0.1"
     os.environ["MASTER_PORT"] = str(port)
     dist.init_process_group("gloo", rank=rank, world_size=world)
@@ -82,8 +84,8 @@ def _worker(rank, world, port, m, n, kappa, s1, s2, seed, out_dir):
     Vl = V[row0:row0 + rows].contiguous()
     Q = torch.empty_like(Vl)
     R = torch.empty(n, n, dtype=torch.float64)
-    bufs = rdist.alloc_bufs(ops, rows, n, s1, s2, "cpu")
-    rdist.rand_cholqr_sharded(ops, Vl, row0, s1, s2, seed, Q, R, bufs)
+    bufs = rdist.alloc_bufs(ops, rows, n, s1, s2, "cpu", variant)
+    rdist.rand_cholqr_sharded(ops, Vl, row0, s1, s2, seed, Q, R, bufs, variant=variant)
     np.save(os.path.join(out_dir, "Q%d.npy" % rank), Q.numpy())
     np.save(os.path.join(out_dir, "R%d.npy" % rank), R.numpy())
     np.save(os.path.join(out_dir, "info%d.npy" % rank), bufs["info"].numpy())
@@ -101,11 +103,12 @@ def test_shard_rows_partition():
 
 
 @pytest.mark.timeout(300)
-def test_row_sharded_rand_cholqr_world2(tmp_path, orc):
+@pytest.mark.parametrize("variant", [0, rdist.S2_RADEMACHER])
+def test_row_sharded_rand_cholqr_world2(tmp_path, orc, variant):
     m, n, kappa, seed = 6001, 12, 1e9, 42           # odd m: unequal blocks
     s1, s2 = 2 * n * n, 2 * n
     port = _free_port()
-    mp.spawn(_worker, args=(2, port, m, n, kappa, s1, s2, seed, str(tmp_path)), nprocs=2, join=True)
+    mp.spawn(_worker, args=(2, port, m, n, kappa, s1, s2, seed, str(tmp_path), variant), nprocs=2, join=True)
     R0_, R1_ = np.load(tmp_path / "R0.npy"), np.load(tmp_path / "R1.npy")
     assert np.array_equal(R0_, R1_)                 # all-reduce gives every rank the same W and G
     assert int(np.load(tmp_path / "info0.npy")[0]) == 0
@@ -115,6 +118,6 @@ def test_row_sharded_rand_cholqr_world2(tmp_path, orc):
     assert np.linalg.norm(V - Q @ R0_) / np.linalg.norm(V) <= 1e-13
     assert np.all(np.diag(R0_) > 0) and np.array_equal(np.tril(R0_, -1), np.zeros((n, n)))
     # against the single-process oracle on the whole matrix: same hash (global row index), same S2
-    _, Rs, info = orc.rand_cholqr(V, s1, s2, seed)
+    _, Rs, info = orc.rand_cholqr(V, s1, s2, seed, rademacher=bool(variant))
     assert info == 0
     assert np.linalg.norm(R0_ - Rs) / np.linalg.norm(Rs) <= 1e-12
