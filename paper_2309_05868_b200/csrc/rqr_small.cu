@@ -463,6 +463,162 @@ k_geqrf_cluster(double* W, int s2, int n, double* R0, int* d_info, int64_t rows_
         }
 }
 
+// NC (2 or 4) columns per cluster barrier (s2 <= 512): column group pi = (NC pi .. NC pi + NC - 1) -> CTA pi % ncta,
+// warp pi / ncta, all NC columns in the registers of ONE warp.  The owner warp factors its first column, applies
+// that reflector to its other columns, factors the next one, ... and publishes the NC reflectors together; every
+// other warp applies them in turn.  The exchange through L2 (store, cluster barrier, load: the bulk of a step of
+// k_geqrf_cluster) is paid once per NC columns.
+template <int RPL>
+__device__ __forceinline__ double cluster2_reflect(double (&col)[RPL], int j, int lane, double* __restrict__ vout,
+                                                   double (&v)[RPL], double* gflip, int* d_info)
+{
+    double tail2 = 0.0, x1 = 0.0;
+#pragma unroll
+    for (int p = 0; p < RPL; ++p) {
+        const int i = lane + 32 * p;
+        if (i > j) tail2 = fma(col[p], col[p], tail2);
+        if (i == j) x1 = col[p];
+    }
+    tail2 = warp_sum(tail2);
+    x1 = __shfl_sync(0xffffffffu, x1, j & 31);
+    const double nrm = sqrt(tail2 + x1 * x1);
+    const double sgn = (x1 < 0.0) ? -1.0 : 1.0;
+    const double vj = x1 + sgn * nrm;
+    const double vtv = tail2 + vj * vj;
+    const double beta = (vtv > 0.0) ? 2.0 / vtv : 0.0;
+    if (lane == 0) {
+        gflip[j] = (sgn > 0.0) ? 1.0 : 0.0;                   // diagonal becomes -sgn * nrm, the row is negated at the end
+        if (!(nrm > 0.0) || !(nrm < 1.0e308)) rqr_set_info(d_info, RQR_INFO_SINGULAR + j + 1);
+    }
+#pragma unroll
+    for (int p = 0; p < RPL; ++p) {
+        const int i = lane + 32 * p;
+        v[p] = (i > j) ? col[p] : ((i == j) ? vj : 0.0);
+        vout[i] = v[p];
+        if (i == j) col[p] = -sgn * nrm;
+        else if (i > j) col[p] = 0.0;
+    }
+    return beta;
+}
+
+template <int RPL, int NC>
+__global__ void __launch_bounds__(NC == 2 ? 512 : 256, 1)
+k_geqrf_cluster2(double* W, int s2, int n, double* R0, int* d_info, int64_t rows_total, int nb)
+{
+    __shared__ double vs[NC * 32 * RPL];     // the NC reflectors of this step
+    const int ncta = (int)cluster_size(), rank = (int)cluster_rank();
+    if (nb > 0) {                            // one level of a TSQR tree, see k_geqrf_cluster
+        const int64_t cid = blockIdx.x / ncta;
+        const int64_t r0 = cid * rows_total / nb, r1 = (cid + 1) * rows_total / nb;
+        W += r0 * n;
+        s2 = (int)(r1 - r0);
+        R0 += cid * (int64_t)n * n;
+        d_info = nullptr;
+    }
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int pi = w * ncta + rank;          // my column group: columns NC pi .. NC pi + NC - 1
+    double a[NC][RPL];
+#pragma unroll
+    for (int q = 0; q < NC; ++q)
+#pragma unroll
+        for (int p = 0; p < RPL; ++p) {
+            const int c = NC * pi + q, i = lane + 32 * p;
+            a[q][p] = (c < n && i < s2) ? W[(int64_t)i * n + c] : 0.0;
+        }
+    cluster_sync_all();                      // everyone holds its columns: W is scratch from here on
+    double* gv = W;                          // [2 buffers][NC reflectors][32 * RPL]
+    double* gbeta = W + 2 * NC * 32 * RPL;   // [2][NC]
+    double* gflip = gbeta + 2 * NC;          // [n]
+    const int ngroups = (n + NC - 1) / NC;
+    for (int jp = 0; jp < ngroups; ++jp) {
+        double* buf = gv + (jp & 1) * NC * 32 * RPL;
+        if (pi == jp) {                      // the owner warp: factor its NC columns one after the other
+            double beta[NC];
+#pragma unroll
+            for (int q = 0; q < NC; ++q) {
+                beta[q] = 0.0;
+                if (NC * jp + q < n) {
+                    double v[RPL];
+                    beta[q] = cluster2_reflect<RPL>(a[q], NC * jp + q, lane, buf + q * 32 * RPL, v, gflip, d_info);
+                    double d[NC];
+#pragma unroll
+                    for (int q2 = q + 1; q2 < NC; ++q2) {
+                        double d0 = 0.0, d1 = 0.0;
+#pragma unroll
+                        for (int p = 0; p < RPL; p += 2) {
+                            d0 = fma(v[p], a[q2][p], d0);
+                            d1 = fma(v[p + 1], a[q2][p + 1], d1);
+                        }
+                        d[q2] = d0 + d1;
+                    }
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+                        for (int q2 = q + 1; q2 < NC; ++q2) d[q2] += __shfl_xor_sync(0xffffffffu, d[q2], o);
+#pragma unroll
+                    for (int q2 = q + 1; q2 < NC; ++q2) {
+                        const double ws = beta[q] * d[q2];
+#pragma unroll
+                        for (int p = 0; p < RPL; ++p) a[q2][p] = fma(-ws, v[p], a[q2][p]);
+                    }
+                }
+            }
+            if (lane < NC) {
+                double bsel = beta[0];
+#pragma unroll
+                for (int q = 1; q < NC; ++q) bsel = (lane == q) ? beta[q] : bsel;
+                gbeta[(jp & 1) * NC + lane] = bsel;
+            }
+        }
+        cluster_sync_all();
+        for (int i = threadIdx.x; i < NC * 32 * RPL; i += blockDim.x) vs[i] = __ldcg(buf + i);
+        double beta[NC];
+#pragma unroll
+        for (int h = 0; h < NC; ++h) beta[h] = __ldcg(gbeta + (jp & 1) * NC + h);
+        __syncthreads();
+        if (pi > jp && NC * pi < n) {        // groups before jp are finished, jp's own columns were done by the owner
+#pragma unroll
+            for (int h = 0; h < NC; ++h) {
+                if (NC * jp + h >= n) break;
+                const double* v = vs + h * 32 * RPL + lane;
+                double dot[NC];
+#pragma unroll
+                for (int q = 0; q < NC; ++q) {
+                    double s0 = 0.0, s1_ = 0.0;
+#pragma unroll
+                    for (int p = 0; p < RPL; p += 2) {
+                        s0 = fma(v[32 * p], a[q][p], s0);
+                        s1_ = fma(v[32 * (p + 1)], a[q][p + 1], s1_);
+                    }
+                    dot[q] = s0 + s1_;
+                }
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+                    for (int q = 0; q < NC; ++q) dot[q] += __shfl_xor_sync(0xffffffffu, dot[q], o);
+#pragma unroll
+                for (int q = 0; q < NC; ++q) {
+                    const double ws = beta[h] * dot[q];       // a padding column (c >= n) is all zero: ws = 0
+#pragma unroll
+                    for (int p = 0; p < RPL; ++p) a[q][p] = fma(-ws, v[32 * p], a[q][p]);
+                }
+            }
+        }
+    }
+    cluster_sync_all();
+#pragma unroll
+    for (int q = 0; q < NC; ++q)
+#pragma unroll
+        for (int p = 0; p < RPL; ++p) {
+            const int c = NC * pi + q, i = lane + 32 * p;
+            if (c < n && i < n) {
+                double rv = (c >= i) ? a[q][p] : 0.0;
+                if (c >= i && __ldcg(gflip + i) != 0.0) rv = -rv;
+                R0[(int64_t)i * n + c] = rv;
+            }
+        }
+}
+
 template <class K, class... Args>
 static int launch_cluster_grid(K kernel, int nclusters, int ncta, int threads, cudaStream_t st, Args... args)
 {
@@ -527,6 +683,16 @@ extern "C" int rqr_small_geqrf(double* W, int s2, int n, double* R0, int* d_info
     if ((int64_t)s2 * n >= 2 * 32 * rpl + 2 + n) {
         if (rpl <= 16) {
             const int ncta = n <= 128 ? 4 : 8;                     // 16 warps x 2 columns per CTA
+            // NC columns per cluster barrier (k_geqrf_cluster2); its exchange area is NC times as large.
+            // 512 x 256: 0.56 ms (one column per barrier) -> 0.45 (two) -> 0.41 ms (four); 256 x 128: 0.23 -> 0.15 ms
+            if ((int64_t)s2 * n >= 8 * 32 * rpl + 8 + n) {
+                if (rpl <= 8) return launch_cluster(k_geqrf_cluster2<8, 4>, ncta, 256, st, W, s2, n, R0, d_info, (int64_t)0, 0);
+                return launch_cluster(k_geqrf_cluster2<16, 4>, ncta, 256, st, W, s2, n, R0, d_info, (int64_t)0, 0);
+            }
+            if ((int64_t)s2 * n >= 4 * 32 * rpl + 4 + n) {
+                if (rpl <= 8) return launch_cluster(k_geqrf_cluster2<8, 2>, ncta, 512, st, W, s2, n, R0, d_info, (int64_t)0, 0);
+                return launch_cluster(k_geqrf_cluster2<16, 2>, ncta, 512, st, W, s2, n, R0, d_info, (int64_t)0, 0);
+            }
             if (rpl <= 8) return launch_cluster(k_geqrf_cluster<8, 2>, ncta, 512, st, W, s2, n, R0, d_info, (int64_t)0, 0);
             return launch_cluster(k_geqrf_cluster<16, 2>, ncta, 512, st, W, s2, n, R0, d_info, (int64_t)0, 0);
         }
@@ -552,7 +718,7 @@ int rqr_tsqr_r_wide_dev(double* A, int64_t rows, int n, double* R, double* scrat
         if (nb <= 1) return rqr_small_geqrf(in, (int)rows_in, n, R, d_info, st);
         int rc;
         if (n <= 128) rc = launch_cluster_grid(k_geqrf_cluster<32, 1>, (int)nb, 8, 512, st, in, 0, n, out, (int*)nullptr, rows_in, (int)nb);
-        else          rc = launch_cluster_grid(k_geqrf_cluster<16, 2>, (int)nb, 8, 512, st, in, 0, n, out, (int*)nullptr, rows_in, (int)nb);
+        else          rc = launch_cluster_grid(k_geqrf_cluster2<16, 4>, (int)nb, 8, 256, st, in, 0, n, out, (int*)nullptr, rows_in, (int)nb);
         if (rc != RQR_OK) return rc;
         double* t = in; in = out; out = t;
         rows_in = nb * n;
