@@ -502,7 +502,7 @@ __device__ __forceinline__ double cluster2_reflect(double (&col)[RPL], int j, in
 }
 
 template <int RPL, int NC>
-__global__ void __launch_bounds__(NC == 2 ? 512 : 256, 1)
+__global__ void __launch_bounds__(RPL * NC <= 32 ? 512 : 256, 1)
 k_geqrf_cluster2(double* W, int s2, int n, double* R0, int* d_info, int64_t rows_total, int nb)
 {
     __shared__ double vs[NC * 32 * RPL];     // the NC reflectors of this step
@@ -696,8 +696,22 @@ extern "C" int rqr_small_geqrf(double* W, int s2, int n, double* R0, int* d_info
             if (rpl <= 8) return launch_cluster(k_geqrf_cluster<8, 2>, ncta, 512, st, W, s2, n, R0, d_info, (int64_t)0, 0);
             return launch_cluster(k_geqrf_cluster<16, 2>, ncta, 512, st, W, s2, n, R0, d_info, (int64_t)0, 0);
         }
-        if (n <= 128)                                              // tall sketches of the paper's grid (s2 <= 1024)
+        if (n > 64 && n <= 128 && (int64_t)s2 * n >= 4 * 32 * 32 + 4 + n)   // tall sketches of the paper's grid (s2 <= 1024):
+            return launch_cluster(k_geqrf_cluster2<32, 2>, 8, 256, st, W, s2, n, R0, d_info, (int64_t)0, 0);   // 64 pairs, 8 x 8 warps
+        if (n <= 128)
             return launch_cluster(k_geqrf_cluster<32, 1>, n <= 64 ? 4 : 8, 512, st, W, s2, n, R0, d_info, (int64_t)0, 0);
+        if (rpl <= 32 && (int64_t)s2 * n >= 4 * 32 * 32 + 4 + n) {
+            // 512 < s2 <= 1024 with 128 < n <= 256: 128 column pairs need 16 CTAs of 8 warps (64 registers of tile per
+            // column): a non-portable cluster size; if the device refuses it the global-memory kernel below runs
+            static bool np = false;
+            if (!np) {
+                cudaFuncSetAttribute(k_geqrf_cluster2<32, 2>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+                np = true;
+            }
+            if (launch_cluster(k_geqrf_cluster2<32, 2>, 16, 256, st, W, s2, n, R0, d_info, (int64_t)0, 0) == RQR_OK)
+                return RQR_OK;
+            (void)cudaGetLastError();
+        }
     }
     k_geqrf_gmem<<<1, 1024, 0, st>>>(W, s2, n, R0, d_info);
     RQR_LAUNCH_CHECK();

@@ -112,7 +112,8 @@ def test_dense_gauss_sketch_parity(rq, orc):
 
 
 @pytest.mark.parametrize("s2,n", [(32, 16), (128, 64), (140, 70), (256, 128), (512, 256), (9, 9),
-                                  (64, 2), (300, 37), (789, 70), (1000, 100), (700, 30), (1024, 128), (600, 200)])
+                                  (64, 2), (300, 37), (789, 70), (1000, 100), (700, 30), (1024, 128), (600, 200),
+                                  (1024, 256), (900, 150), (513, 129), (140, 69), (512, 255), (200, 97)])
 def test_small_geqrf_parity(rq, orc, s2, n):
     rng = np.random.default_rng(s2 * 1000 + n)
     W = rng.standard_normal((s2, n)) * np.logspace(0, -10, n)
