@@ -188,7 +188,7 @@ def probe_fp64_peak(torch, rq):
     """Measured FP64 peak (TFLOP/s): best of a DFMA chain and a DMMA chain, >= 0.25 s each."""
     sink = torch.empty(148 * 8 * 256, dtype=torch.float64, device="cuda")
     out = {}
-    for kind, name in ((rq.PROBE_DFMA, "dfma"), (rq.PROBE_DMMA, "dmma")):
+    for kind, name in ((rq.PROBE_DFMA, "dfma"), (rq.PROBE_DMMA, "dmma"), (rq.PROBE_MIX, "dfma_dmma_mixed")):
         iters = 20000
         fl = rq.probe_fp64(kind, iters, 148 * 8, sink)        # warm-up
         ms = time_region(torch, lambda: rq.probe_fp64(kind, iters, 148 * 8, sink), 1)

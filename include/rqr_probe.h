@@ -12,6 +12,8 @@ extern "C" {
 
 #define RQR_PROBE_DFMA 0 /* chains of independent double fma                         */
 #define RQR_PROBE_DMMA 1 /* chains of independent mma.sync.m8n8k4.f64 (SASS DMMA)     */
+#define RQR_PROBE_MIX 2  /* even warps DFMA chains, odd warps DMMA chains, in the same CTA: shows whether
+                          * the two kinds share one FP64 data path (sum = one peak) or not (sum of peaks) */
 
 /* Launches one probe kernel on `stream` (asynchronous): grid = blocks CTAs of 256 threads, each
  * thread/warp running `iters` rounds of 8 independent accumulator updates.  `d_sink` is a device

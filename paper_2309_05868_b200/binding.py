@@ -22,8 +22,11 @@ VARIANT_SCATTER = 1
 FLAG_PREPARED = 1
 FLAG_RECOMPUTE_V1 = 2
 S2_RADEMACHER = 16          # OR into `variant` (workspace, prepare, countsketch, rand_cholqr) / `flags` (gauss_sketch)
+MAX_N = 256                 # argument limits of include/rqr.h
+MAX_S2 = 1024
 PROBE_DFMA = 0
 PROBE_DMMA = 1
+PROBE_MIX = 2
 
 _i64, _u64, _u32, _int, _dbl, _vp, _sz = (ctypes.c_int64, ctypes.c_uint64, ctypes.c_uint32, ctypes.c_int,
                                           ctypes.c_double, ctypes.c_void_p, ctypes.c_size_t)

@@ -104,3 +104,19 @@ def test_product_does_not_import_oracle():
         if f.endswith(".py") or f.endswith(".c"):
             for ln in open(os.path.join(ROOT, "oracle", f)).read().splitlines():
                 assert not bad2.search(ln), (f, ln)
+
+
+def test_eps_sweep_sketch_sizes():
+    """Sketch sizes of the eps sweep: constants as printed, natural log (S17).
+    The eps = 0.9 multisketch sizes are the paper grid's; a larger eps always means a smaller sketch."""
+    import math
+    from paper_2309_05868_b200 import eps_sweep as es, paper_grid
+    assert es.gauss_size(100, 0.99) == math.ceil(36.01 * math.log(100)) == 166
+    assert es.gauss_size(100, 0.49) == 343
+    assert es.count_size(10, 0.99) == 748 and es.count_size(10, 0.49) == 3058      # 6.8 * 110, 27.8 * 110
+    for n in range(10, 101, 10):
+        assert es.multi_sizes(n, 0.9) == paper_grid.paper_sketch_sizes(n)
+        assert es.gauss_size(n, 0.99) < es.gauss_size(n, 0.49)
+        assert es.count_size(n, 0.99) < es.count_size(n, 0.9) < es.count_size(n, 0.49)
+        s1, s2 = es.multi_sizes(n, 0.49)
+        assert n <= s2 <= s1 and s2 <= 1024                                      # eq. (20) ordering, library limit

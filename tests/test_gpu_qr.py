@@ -228,6 +228,53 @@ def test_full_size_config_matches_oracle(rq, orc, name):
     assert np.abs(Qs @ Ro - Vh[rows]).max() <= 1e-11 * scale
 
 
+@pytest.mark.parametrize("m,n", [(60000, 30), (90000, 50), (200000, 80)])
+def test_eps_sweep_sketch_sizes_match_oracle(rq, orc, m, n):
+    """SURVEY.md 8(f) N1, the eps sweep (section 6.4): every sketch size of Figs 5-7 -- one Gaussian
+    sketch at eps = 0.99 / 0.49, one CountSketch at 0.99 / 0.49, the multisketch at eps1 = 0.9 / 0.49 -- factors V
+    within the bars and gives the oracle's R.  The large sketches are the library's widest shapes: 27.8 (n^2 + n)
+    buckets, s2 up to 900 rows."""
+    from paper_2309_05868_b200 import eps_sweep as es
+    V = inputs.make_V(m, n, 1e9, 808)
+    Vd, Vh = V.cuda(), V.numpy()
+    Q = torch.empty_like(Vd)
+    R = torch.empty(n, n, dtype=torch.float64, device="cuda")
+    info = rq.new_info()
+
+    def check(Ro, io):
+        torch.cuda.synchronize()
+        assert int(info.item()) == 0 and io == 0
+        assert orth_err(Q) <= ORTH_TOL and resid(Vd, Q, R) <= RES_TOL
+        check_R(R)
+        assert np.linalg.norm(R.cpu().numpy() - Ro) <= R_TOL * np.linalg.norm(Ro)
+
+    for eps in (0.99, 0.49):
+        s = es.gauss_size(n, eps)
+        work = rq.alloc_workspace(m, n, n, s)
+        rq.gauss_randcholqr(Vd, s, 42, Q, R, work, info)
+        _, Ro, io = orc.gauss_rand_cholqr(Vh, s, 42)
+        check(Ro, io)
+    for eps in (0.99, 0.49):
+        s1 = es.count_size(n, eps)
+        if s1 > m:
+            continue
+        work = rq.alloc_workspace(m, n, s1, 2 * n)
+        rq.count_randcholqr(Vd, s1, 42, Q, R, work, info)
+        R0, i0 = orc.hhqr_r(orc.countsketch(Vh, s1, 42))
+        R1, i1 = orc.chol(orc.gram(orc.trsm(Vh, R0)))
+        check(orc.triu_mul(R1, R0), i0 or i1)
+    for eps1 in (0.9, 0.49):
+        s1, s2 = es.multi_sizes(n, eps1)
+        if s1 > m:
+            continue
+        Qm, Rm, im = run_rand(rq, Vd, s1, s2, 42, 0, 0, True)
+        Q.copy_(Qm)
+        R.copy_(Rm)
+        info.fill_(im)
+        _, Ro, io = orc.rand_cholqr(Vh, s1, s2, 42)
+        check(Ro, io)
+
+
 @pytest.mark.parametrize("m,n", [(100000, 70), (100000, 30), (60000, 100)])
 def test_paper_grid_shape_and_sketch_sizes(rq, orc, m, n):
     """the paper's own shapes with its "Multi (0.9, 0.49)" sketch sizes
