@@ -562,56 +562,105 @@ extern "C" int rqr_gauss_sketch(const double* W1, int64_t s1, int n, int s2, uin
 // grid = (P persistent row-chunk walkers, ceil(s/32) sketch-row tiles).
 // =========================================================================================
 #define DG_ROWS 32
+// NJ = column slots per thread (columns cq + 8 j, j < NJ: n <= 8 NJ), RT = sketch rows per thread (rows
+// r + 32 k, k < RT: a tile of 32 RT sketch rows), so that one shared-memory load of V feeds RT fma.
+// The Gaussians of a tile are drawn as Box-Muller PAIRS (entries 2q, 2q + 1 of the row-major S are the two
+// outputs of Philox counter q): adjacent V rows share one evaluation whenever the first entry index is even.
+template <int NJ, int RT>
 __global__ void __launch_bounds__(256)
 k_dense_gauss_sketch(const double* __restrict__ V, int64_t m, int n, int64_t ldv, int64_t row0,
                      int64_t m_total, int s, uint64_t seed, double* __restrict__ part)
 {
     extern __shared__ double sm[];
-    double* St = sm;                         // [32][33]
-    double* Vt = sm + 32 * 33;               // [32][n]
+    constexpr int TR = 32 * RT;              // sketch rows per tile
+    constexpr int LDV = 8 * NJ;              // padded row of the V tile (pad columns are zero)
+    double* St = sm;                         // [TR][33]
+    double* Vt = sm + TR * 33;               // [32][LDV]
     const int tid = threadIdx.x;
     const int r = tid >> 3, cq = tid & 7;
-    const int srow = blockIdx.y * 32 + r;
     const double d = sqrt((double)s);
-    double acc[RQR_MAX_N / 8];
+    double acc[RT][NJ];
 #pragma unroll
-    for (int j = 0; j < RQR_MAX_N / 8; ++j) acc[j] = 0.0;
+    for (int k = 0; k < RT; ++k)
+#pragma unroll
+        for (int j = 0; j < NJ; ++j) acc[k][j] = 0.0;
     const int64_t nchunks = (m + DG_ROWS - 1) / DG_ROWS;
     for (int64_t ch = blockIdx.x; ch < nchunks; ch += gridDim.x) {
         const int64_t i0 = ch * DG_ROWS;
-        for (int t = tid; t < 32 * 32; t += 256) {
-            int rr = t >> 5, ii = t & 31;
-            int sr = blockIdx.y * 32 + rr;
-            double val = 0.0;
+        for (int t = tid; t < TR * 16; t += 256) {
+            const int rr = t >> 4, ii = 2 * (t & 15);
+            const int sr = blockIdx.y * TR + rr;
+            double v0 = 0.0, v1 = 0.0;
             if (sr < s && i0 + ii < m) {
-                uint64_t e = (uint64_t)sr * (uint64_t)m_total + (uint64_t)(row0 + i0 + ii);
-                val = rqr_gauss_entry(seed, e, RQR_PHILOX_STREAM_DENSE) / d;
+                const uint64_t e = (uint64_t)sr * (uint64_t)m_total + (uint64_t)(row0 + i0 + ii);
+                const bool second = i0 + ii + 1 < m;
+                if (!(e & 1)) {
+                    rqr_gauss_pair(seed, e >> 1, RQR_PHILOX_STREAM_DENSE, v0, v1);
+                    if (!second) v1 = 0.0;
+                } else {
+                    v0 = rqr_gauss_entry(seed, e, RQR_PHILOX_STREAM_DENSE);
+                    if (second) v1 = rqr_gauss_entry(seed, e + 1, RQR_PHILOX_STREAM_DENSE);
+                }
+                v0 /= d;
+                v1 /= d;
             }
-            St[rr * 33 + ii] = val;
+            St[rr * 33 + ii] = v0;
+            St[rr * 33 + ii + 1] = v1;
         }
-        for (int t = tid; t < 32 * n; t += 256) {
-            int ii = t / n, c = t - ii * n;
-            Vt[t] = (i0 + ii < m) ? V[(i0 + ii) * ldv + c] : 0.0;
+        for (int t = tid; t < 32 * LDV; t += 256) {
+            const int ii = t / LDV, c = t - ii * LDV;
+            Vt[t] = (c < n && i0 + ii < m) ? V[(i0 + ii) * ldv + c] : 0.0;
         }
         __syncthreads();
+#pragma unroll 4
         for (int ii = 0; ii < 32; ++ii) {
-            const double a = St[r * 33 + ii];
+            double a[RT];
 #pragma unroll
-            for (int j = 0; j < RQR_MAX_N / 8; ++j) {
-                int c = cq + 8 * j;
-                if (c < n) acc[j] = fma(a, Vt[ii * n + c], acc[j]);
+            for (int k = 0; k < RT; ++k) a[k] = St[(r + 32 * k) * 33 + ii];
+#pragma unroll
+            for (int j = 0; j < NJ; ++j) {
+                const double v = Vt[ii * LDV + cq + 8 * j];
+#pragma unroll
+                for (int k = 0; k < RT; ++k) acc[k][j] = fma(a[k], v, acc[k][j]);
             }
         }
         __syncthreads();
     }
-    if (srow < s) {
-        double* P = part + ((int64_t)blockIdx.x * s + srow) * n;
 #pragma unroll
-        for (int j = 0; j < RQR_MAX_N / 8; ++j) {
-            int c = cq + 8 * j;
-            if (c < n) P[c] = acc[j];
+    for (int k = 0; k < RT; ++k) {
+        const int srow = blockIdx.y * TR + r + 32 * k;
+        if (srow < s) {
+            double* P = part + ((int64_t)blockIdx.x * s + srow) * n;
+#pragma unroll
+            for (int j = 0; j < NJ; ++j) {
+                const int c = cq + 8 * j;
+                if (c < n) P[c] = acc[k][j];
+            }
         }
     }
+}
+
+template <int NJ, int RT>
+static int launch_dense_gauss(const double* V, int64_t m, int n, int64_t ldv, int64_t row0, int64_t m_total, int s,
+                              uint64_t seed, double* part, int* P_out, cudaStream_t st)
+{
+    const int stiles = (s + 32 * RT - 1) / (32 * RT);
+    const int64_t nchunks = (m + DG_ROWS - 1) / DG_ROWS;
+    int64_t P = (148 * 4) / stiles;
+    const int64_t Pcap = ((int64_t)RQR_MAX_GRAM_PARTIALS * n) / s;
+    if (P > Pcap) P = Pcap;
+    if (P > nchunks) P = nchunks;
+    if (P < 1) P = 1;
+    const size_t smem = (size_t)(32 * RT * 33 + 32 * 8 * NJ) * sizeof(double);
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaFuncSetAttribute(k_dense_gauss_sketch<NJ, RT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+        attr_set = true;
+    }
+    dim3 grid((unsigned)P, stiles);
+    k_dense_gauss_sketch<NJ, RT><<<grid, 256, smem, st>>>(V, m, n, ldv, row0, m_total, s, seed, part);
+    *P_out = (int)P;
+    return RQR_OK;
 }
 
 extern "C" int rqr_dense_gauss_sketch(const double* V, int64_t m, int n, int64_t ldv, int64_t row0,
@@ -628,24 +677,15 @@ extern "C" int rqr_dense_gauss_sketch(const double* V, int64_t m, int n, int64_t
     if (!work) return -10;
     cudaStream_t st = (cudaStream_t)stream;
     double* part = (double*)((char*)work + 256);      // region A
-    int stiles = (s + 31) / 32;
-    int64_t nchunks = (m + DG_ROWS - 1) / DG_ROWS;
-    int64_t P = (148 * 4) / stiles;
-    int64_t Pcap = ((int64_t)RQR_MAX_GRAM_PARTIALS * n) / s;
-    if (P > Pcap) P = Pcap;
-    if (P > nchunks) P = nchunks;
-    if (P < 1) P = 1;
-    size_t smem = (size_t)(32 * 33 + 32 * n) * sizeof(double);
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaFuncSetAttribute(k_dense_gauss_sketch, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
-        attr_set = true;
-    }
-    dim3 grid((unsigned)P, stiles);
-    k_dense_gauss_sketch<<<grid, 256, smem, st>>>(V, m, n, ldv, row0, m_total, s, seed, part);
+    int P = 1;
+    if (n <= 16) launch_dense_gauss<2, 4>(V, m, n, ldv, row0, m_total, s, seed, part, &P, st);
+    else if (n <= 32) launch_dense_gauss<4, 4>(V, m, n, ldv, row0, m_total, s, seed, part, &P, st);
+    else if (n <= 64) launch_dense_gauss<8, 4>(V, m, n, ldv, row0, m_total, s, seed, part, &P, st);
+    else if (n <= 128) launch_dense_gauss<16, 2>(V, m, n, ldv, row0, m_total, s, seed, part, &P, st);
+    else launch_dense_gauss<32, 1>(V, m, n, ldv, row0, m_total, s, seed, part, &P, st);
     RQR_LAUNCH_CHECK();
     int64_t elems = (int64_t)s * n;
-    k_reduce_partials<<<(int)((elems + 63) / 64), 256, 0, st>>>(part, (int)P, elems, W);
+    k_reduce_partials<<<(int)((elems + 63) / 64), 256, 0, st>>>(part, P, elems, W);
     RQR_LAUNCH_CHECK();
     return RQR_OK;
 }

@@ -101,13 +101,18 @@ def test_gauss_sketch_parity(rq, orc, s1, n, s2):
     assert np.abs(host(W) - Wo).max() <= 1e-13 * np.abs(Wo).max()
 
 
-def test_dense_gauss_sketch_parity(rq, orc):
-    m, n, s = 5000, 20, 40
+@pytest.mark.parametrize("m,n,s,row0,m_total", [(5000, 20, 40, 0, None), (4099, 10, 83, 0, None), (3001, 64, 128, 0, None),
+                                                 (2500, 100, 166, 0, None), (1500, 200, 343, 0, None), (1000, 256, 300, 0, None),
+                                                 (2001, 33, 70, 999, 3001), (2000, 16, 33, 1, 2001), (37, 9, 12, 0, None)])
+def test_dense_gauss_sketch_parity(rq, orc, m, n, s, row0, m_total):
+    """One dense Gaussian sketch W = S V, every column-slot / row-blocking variant of the
+    kernel; odd m_total and odd row0 make the first entry of a row tile fall on the second output of a Box-Muller
+    pair (the unpaired path); row0 / m_total is the row-sharded call of dist.py."""
     V = inputs.make_V(m, n, 1e3, 2)
     W = torch.empty(s, n, dtype=torch.float64, device="cuda")
     work = rq.alloc_workspace(m, n, 2 * n * n, 2 * n)
-    rq.dense_gauss_sketch(V.cuda(), s, 5, W, work)
-    Wo = orc.dense_gauss_sketch(V.numpy(), s, 5)
+    rq.dense_gauss_sketch(V.cuda(), s, 5, W, work, row0, m_total)
+    Wo = orc.dense_gauss_sketch(V.numpy(), s, 5, row0, m_total)
     assert np.abs(host(W) - Wo).max() <= 1e-13 * np.abs(Wo).max()
 
 
