@@ -567,7 +567,7 @@ extern "C" int rqr_gauss_sketch(const double* W1, int64_t s1, int n, int s2, uin
 // The Gaussians of a tile are drawn as Box-Muller PAIRS (entries 2q, 2q + 1 of the row-major S are the two
 // outputs of Philox counter q): adjacent V rows share one evaluation whenever the first entry index is even.
 template <int NJ, int RT>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, NJ * RT <= 16 ? 3 : 2)
 k_dense_gauss_sketch(const double* __restrict__ V, int64_t m, int n, int64_t ldv, int64_t row0,
                      int64_t m_total, int s, uint64_t seed, double* __restrict__ part)
 {
@@ -601,8 +601,6 @@ k_dense_gauss_sketch(const double* __restrict__ V, int64_t m, int n, int64_t ldv
                     v0 = rqr_gauss_entry(seed, e, RQR_PHILOX_STREAM_DENSE);
                     if (second) v1 = rqr_gauss_entry(seed, e + 1, RQR_PHILOX_STREAM_DENSE);
                 }
-                v0 /= d;
-                v1 /= d;
             }
             St[rr * 33 + ii] = v0;
             St[rr * 33 + ii + 1] = v1;
@@ -634,7 +632,7 @@ k_dense_gauss_sketch(const double* __restrict__ V, int64_t m, int n, int64_t ldv
 #pragma unroll
             for (int j = 0; j < NJ; ++j) {
                 const int c = cq + 8 * j;
-                if (c < n) P[c] = acc[k][j];
+                if (c < n) P[c] = acc[k][j] / d;       // the 1/sqrt(s) of S, applied once per partial sum
             }
         }
     }
@@ -647,7 +645,7 @@ static int launch_dense_gauss(const double* V, int64_t m, int n, int64_t ldv, in
     const int stiles = (s + 32 * RT - 1) / (32 * RT);
     const int64_t nchunks = (m + DG_ROWS - 1) / DG_ROWS;
     int64_t P = (148 * 4) / stiles;
-    const int64_t Pcap = ((int64_t)RQR_MAX_GRAM_PARTIALS * n) / s;
+    const int64_t Pcap = ((int64_t)rqr_gram_partial_cap(n) * n) / s;     // region A holds cap n^2 doubles
     if (P > Pcap) P = Pcap;
     if (P > nchunks) P = nchunks;
     if (P < 1) P = 1;
