@@ -44,8 +44,9 @@ __host__ __device__ __forceinline__ void panel_slot_decode(int s, int& Pp, int& 
 
 // One CTA per slot.  off(P',P)[((J'*8+J)*2+s)*32+lane] = -R[64P'+8J'+2(lane%4)+s][64P+8J+lane/4];
 // diag(P) = the Tf / nRf arrays of build_tri_frags for the 64x64 block R[P,P].  Padded with identity.
-// last_nb = 4: the last panel is 32 columns wide (n <= 64 (NP-1) + 32); its diagonal slot holds the NB = 4
-// arrays (Tf 4*64, nRf 6*64 doubles), its off-diagonal slots are used for J < 4 only.
+// last_nb = 2, 4, 6: the last panel is 16, 32, 48 columns wide (n <= 64 (NP-1) + 8 last_nb); its diagonal slot
+// holds the NB = last_nb arrays (Tf NB*64, nRf NB(NB-1)/2*64 doubles), its off-diagonal slots are used for
+// J < last_nb only.
 __global__ void __launch_bounds__(256)
 k_build_panel_frags(const double* __restrict__ R, int n, double* __restrict__ frags, int np, int last_nb)
 {
@@ -55,7 +56,10 @@ k_build_panel_frags(const double* __restrict__ R, int n, double* __restrict__ fr
     panel_slot_decode(blockIdx.x, Pp, P);
     double* out = frags + (size_t)blockIdx.x * PANEL_SLOT;
     if (Pp == P) {
-        if (P == np - 1 && last_nb == 4) build_tri_frags<4>(R, n, out, out + 256, scratch, stage, 64 * P);
+        const int nb = (P == np - 1) ? last_nb : 8;
+        if (nb == 2) build_tri_frags<2>(R, n, out, out + 128, scratch, stage, 64 * P);
+        else if (nb == 4) build_tri_frags<4>(R, n, out, out + 256, scratch, stage, 64 * P);
+        else if (nb == 6) build_tri_frags<6>(R, n, out, out + 384, scratch, stage, 64 * P);
         else build_tri_frags<8>(R, n, out, out + 512, scratch, stage, 64 * P);
     } else {
         for (int t = threadIdx.x; t < PANEL_SLOT; t += blockDim.x) {
@@ -84,7 +88,8 @@ struct PanelPlan {
 };
 
 // X = V R^-1 (npass = 1) or (V Ra^-1) Rb^-1 (npass = 2; fragment sets Ra then Rb), X -> Q.
-// LASTNB = 4: the last panel has 4 column blocks (n <= 64 (NP-1) + 32): its DMMAs for J >= 4 are skipped.
+// LASTNB = 2, 4, 6: the last panel has LASTNB column blocks (n <= 64 (NP-1) + 8 LASTNB): its DMMAs for
+// J >= LASTNB are skipped.
 template <int NP, bool FULL, int LASTNB>
 __global__ void __launch_bounds__((PanelPlan<NP>::CW + 1) * 32, 1)
 k_trsm_panel(const double* V, int64_t m, int n, int64_t ldv, const double* __restrict__ frags,
@@ -214,12 +219,12 @@ k_trsm_panel(const double* V, int64_t m, int n, int64_t ldv, const double* __res
                     trsm_rowblock<8, false, false, FULL>(x[P], nullptr, nullptr, ad, B, B + 512,
                                                          gpp ? gpp + 64 * P : nullptr, colmask[P], lane, g, G, nohook);
                 } else {
-                    double g4[4];
-                    double G4[10][2];
-                    const XsAddr<32> ad4(lane);
-                    trsm_rowblock<4, false, false, FULL>(reinterpret_cast<double (&)[4][2]>(x[P]), nullptr, nullptr, ad4,
-                                                         B, B + 256, gpp ? gpp + 64 * P : nullptr, colmask[P], lane,
-                                                         g4, G4, nohook);
+                    double gl[NBP];
+                    double Gl[NBP * (NBP + 1) / 2][2];
+                    const XsAddr<8 * NBP> adl(lane);
+                    trsm_rowblock<NBP, false, false, FULL>(reinterpret_cast<double (&)[NBP][2]>(x[P]), nullptr, nullptr, adl,
+                                                           B, B + 64 * NBP, gpp ? gpp + 64 * P : nullptr, colmask[P], lane,
+                                                           gl, Gl, nohook);
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(empty + buf);
@@ -387,14 +392,23 @@ static int launch_panel_w(const double* V, int64_t m, int n, int64_t ldv, const 
     return RQR_OK;
 }
 
-static int panel_last_nb(int n, int NP) { return n <= 64 * (NP - 1) + 32 ? 4 : 8; }
+// column blocks of the last panel, in steps of 16 columns (the syrk folds need an even number of blocks)
+static int panel_last_nb(int n, int NP)
+{
+    const int rem = n - 64 * (NP - 1);
+    return rem <= 16 ? 2 : rem <= 32 ? 4 : rem <= 48 ? 6 : 8;
+}
 
 template <int NP>
 static int launch_panel(const double* V, int64_t m, int n, int64_t ldv, const double* frags, int npass,
                         double* Q, int64_t ldq, cudaStream_t st)
 {
-    return panel_last_nb(n, NP) == 4 ? launch_panel_w<NP, 4>(V, m, n, ldv, frags, npass, Q, ldq, st)
-                                     : launch_panel_w<NP, 8>(V, m, n, ldv, frags, npass, Q, ldq, st);
+    switch (panel_last_nb(n, NP)) {
+        case 2: return launch_panel_w<NP, 2>(V, m, n, ldv, frags, npass, Q, ldq, st);
+        case 4: return launch_panel_w<NP, 4>(V, m, n, ldv, frags, npass, Q, ldq, st);
+        case 6: return launch_panel_w<NP, 6>(V, m, n, ldv, frags, npass, Q, ldq, st);
+        default: return launch_panel_w<NP, 8>(V, m, n, ldv, frags, npass, Q, ldq, st);
+    }
 }
 
 template <int NB>
@@ -464,7 +478,13 @@ int rqr_trsm_gram_panel(const double* V, int64_t m, int n, int64_t ldv, const do
         X = V1;
         ldx = ldq;
     }
-    switch (8 * (NP - 1) + panel_last_nb(n, NP)) {        // column blocks: 12, 16, 20, 24, 28, 32
+    switch (8 * (NP - 1) + panel_last_nb(n, NP)) {        // column blocks: 10, 12, ..., 32
+        case 10: return launch_syrk_chunks<10>(X, m, n, ldx, part, nparts, st);
+        case 14: return launch_syrk_chunks<14>(X, m, n, ldx, part, nparts, st);
+        case 18: return launch_syrk_chunks<18>(X, m, n, ldx, part, nparts, st);
+        case 22: return launch_syrk_chunks<22>(X, m, n, ldx, part, nparts, st);
+        case 26: return launch_syrk_chunks<26>(X, m, n, ldx, part, nparts, st);
+        case 30: return launch_syrk_chunks<30>(X, m, n, ldx, part, nparts, st);
         case 12: return launch_syrk_chunks<12>(X, m, n, ldx, part, nparts, st);
         case 16: return launch_syrk_chunks<16>(X, m, n, ldx, part, nparts, st);
         case 20: return launch_syrk_chunks<20>(X, m, n, ldx, part, nparts, st);
