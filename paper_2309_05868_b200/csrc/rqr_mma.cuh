@@ -142,6 +142,7 @@ __device__ __forceinline__ int xs_swz(int r) { return ((r & 1) << 2) | (r & 2); 
 
 template <int N8>
 struct XsAddr {
+    static_assert(N8 % 16 == 0 || N8 == 8, "the XOR swizzle permutes 16-double groups: N8 must be a multiple of 16");
     int c_base;   // C fragment of block J:  c_base + ((8J) ^ c_x)      (double2)
     int c_x;
     int a_base;   // A fragment (J, h):      a_base + ((8J + 4h) ^ a_x)

@@ -30,7 +30,8 @@
 // warps per CTA of A4: bounded by registers (NB = 8: 248 per thread => 8 warps); the narrower
 // shapes have small Gram tiles and little work per row-block, so they run more warps to hide the
 // per-row-block latencies (mbarrier wait, chain start).  Measured at 2^22 x 32: 0.48 -> 0.37 ms.
-template <int NB> struct GramWarps { static constexpr int value = NB >= 8 ? 8 : (NB >= 4 ? 16 : 24); };
+// NB = 6 (32 < n <= 48): 21 Gram blocks = 84 accumulator registers => 12 warps (168 registers each).
+template <int NB> struct GramWarps { static constexpr int value = NB >= 8 ? 8 : (NB >= 5 ? 12 : (NB >= 4 ? 16 : 24)); };
 
 template <int NB, bool HAS_R, bool FULL>
 __global__ void __launch_bounds__(GramWarps<NB>::value * 32, 1)
@@ -502,9 +503,12 @@ int rqr_trsm_gram_mma(const double* V, int64_t m, int n, int64_t ldv, const doub
         const char* e = getenv("RQR_A4_PAIR");
         g_a4_pair = (e && e[0] == '0') ? 0 : 1;
     }
-    if (g_a4_pair && R0 && n > 32) return launch_trsm_gram_pair(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
     if (n <= 16) return launch_trsm_gram<2>(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
     if (n <= 32) return launch_trsm_gram<4>(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
+    // 32 < n <= 48: 6 column blocks instead of 8 (42 + 42 DMMA per 8 rows against 72 + 72).  The column-block count
+    // must be even: the XOR swizzle of the X staging block (XsAddr) permutes 16-double groups of a row.
+    if (n <= 48) return launch_trsm_gram<6>(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
+    if (g_a4_pair && R0) return launch_trsm_gram_pair(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
     return launch_trsm_gram<8>(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
 }
 
@@ -542,5 +546,6 @@ int rqr_apply_mma(const double* V, int64_t m, int n, int64_t ldv, const double* 
     if (!fast_ok(V, n, ldv, Q, ldq)) return RQR_TALL_NOT_HANDLED;
     if (n <= 16) return launch_apply<2>(V, m, n, ldv, R0, R1, Q, ldq, st);
     if (n <= 32) return launch_apply<4>(V, m, n, ldv, R0, R1, Q, ldq, st);
+    if (n <= 48) return launch_apply<6>(V, m, n, ldv, R0, R1, Q, ldq, st);
     return launch_apply<8>(V, m, n, ldv, R0, R1, Q, ldq, st);
 }

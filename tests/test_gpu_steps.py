@@ -147,7 +147,9 @@ def test_small_geqrf_flags_rank_deficiency(rq, orc):
 SHAPES_TALL = [(20000, 16), (4099, 64), (10000, 70), (3000, 32), (2500, 128), (700, 256), (65, 8), (5, 2),
                (40003, 128), (30011, 200), (20000, 256), (9001, 66),
                # last panel of 16 / 48 columns at 2, 3 and 4 panels (panel_last_nb = 2, 6)
-               (3001, 80), (3001, 100), (2003, 112), (2000, 140), (2000, 176), (1500, 208), (1500, 240)]
+               (3001, 80), (3001, 100), (2003, 112), (2000, 140), (2000, 176), (1500, 208), (1500, 240),
+               # 5 and 6 column blocks (32 < n <= 48)
+               (5000, 40), (4099, 36), (5003, 48), (3001, 44)]
 
 
 @pytest.mark.parametrize("m,n", SHAPES_TALL)
