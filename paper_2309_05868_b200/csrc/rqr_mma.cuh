@@ -136,13 +136,15 @@ __device__ void build_tri_frags(const double* __restrict__ R, int n, double* __r
 
 // ------------------------------------------------------------------------------------------
 // xs: per-warp 8 x N8 block, 16-byte units XOR-swizzled by g(r) = 4 (r&1) + (r&2).
-// Element (r, c) lives at r*N8 + (((c>>1) ^ g(r)) << 1) + (c&1).
+// Element (r, c) lives at r*LD + (((c>>1) ^ g(r)) << 1) + (c&1), LD = N8 rounded up to 16.
 // ------------------------------------------------------------------------------------------
 __device__ __forceinline__ int xs_swz(int r) { return ((r & 1) << 2) | (r & 2); }
 
 template <int N8>
 struct XsAddr {
-    static_assert(N8 % 16 == 0 || N8 == 8, "the XOR swizzle permutes 16-double groups: N8 must be a multiple of 16");
+    // the XOR swizzle permutes the 8 units of a 16-double group, so a row occupies a multiple of 16 doubles
+    // (odd column-block counts leave 8 pad doubles per row that are never read)
+    static constexpr int LD = (N8 + 15) & ~15;
     int c_base;   // C fragment of block J:  c_base + ((8J) ^ c_x)      (double2)
     int c_x;
     int a_base;   // A fragment (J, h):      a_base + ((8J + 4h) ^ a_x)
@@ -153,14 +155,14 @@ struct XsAddr {
     {
         const int r = lane >> 2, q = lane & 3;
         // C: (r, 8J + 2q): unit 4J + q ^ g(r)
-        c_base = r * N8; c_x = ((q ^ xs_swz(r)) << 1);
+        c_base = r * LD; c_x = ((q ^ xs_swz(r)) << 1);
         // A: (r, 8J + 4h + q): unit (4J + 2h + (q>>1)) ^ g(r), word q&1
-        a_base = r * N8 + (q & 1); a_x = (((q >> 1) ^ xs_swz(r)) << 1);
+        a_base = r * LD + (q & 1); a_x = (((q >> 1) ^ xs_swz(r)) << 1);
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
             // Gram: (row 4h + q, col 8a + r): unit (4a + (r>>1)) ^ g(row), word r&1
             const int row = 4 * h + q;
-            g_base[h] = row * N8 + (r & 1); g_x[h] = (((r >> 1) ^ xs_swz(row)) << 1);
+            g_base[h] = row * LD + (r & 1); g_x[h] = (((r >> 1) ^ xs_swz(row)) << 1);
         }
     }
     __device__ __forceinline__ int c(int J) const { return c_base + ((8 * J) ^ c_x); }
@@ -345,7 +347,8 @@ struct SmemPlan {
     static constexpr size_t scratch = (size_t)NSETS * TallCfg<NB>::FRAG_DOUBLES;
     static constexpr size_t bars = scratch + NB * 64;
     static constexpr size_t xs = bars + ((WARPS * STAGES + 1) & ~1);
-    static constexpr size_t ring = xs + (size_t)WARPS * XSBUF * 8 * N8;
+    static constexpr int XLD = (N8 + 15) & ~15;                        // row of an xs block (XsAddr<N8>::LD)
+    static constexpr size_t ring = xs + (size_t)WARPS * XSBUF * 8 * XLD;
     static constexpr size_t ring_doubles = (size_t)WARPS * STAGES * 8 * LDL;
     static constexpr size_t red_doubles = XSBUF ? (size_t)WARPS * TallCfg<NB>::NBLK * 64 : 0;   // A4 only
     static constexpr size_t total_doubles =

@@ -30,8 +30,8 @@
 // warps per CTA of A4: bounded by registers (NB = 8: 248 per thread => 8 warps); the narrower
 // shapes have small Gram tiles and little work per row-block, so they run more warps to hide the
 // per-row-block latencies (mbarrier wait, chain start).  Measured at 2^22 x 32: 0.48 -> 0.37 ms.
-// NB = 6 (32 < n <= 48): 21 Gram blocks = 84 accumulator registers => 12 warps (168 registers each).
-template <int NB> struct GramWarps { static constexpr int value = NB >= 8 ? 8 : (NB >= 5 ? 12 : (NB >= 4 ? 16 : 24)); };
+// NB = 5, 6 (32 < n <= 48): 15 / 21 Gram blocks = 60 / 84 accumulator registers => 12 warps (168 registers each).
+template <int NB> struct GramWarps { static constexpr int value = NB >= 8 ? 8 : (NB >= 5 ? 12 : (NB >= 3 ? 16 : 24)); };
 
 template <int NB, bool HAS_R, bool FULL>
 __global__ void __launch_bounds__(GramWarps<NB>::value * 32, 1)
@@ -49,7 +49,8 @@ k_trsm_gram_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + Plan::bars);
     double* ring = smem + Plan::ring;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    double* xs = smem + Plan::xs + (size_t)warp * 2 * 8 * N8;
+    constexpr int XB = 8 * Plan::XLD;                 // doubles of one xs block
+    double* xs = smem + Plan::xs + (size_t)warp * 2 * XB;
 
     static_assert(Plan::ring_doubles >= 64 * NB * NB, "ring too small to stage R");
     if (threadIdx.x < GramWarps<NB>::value * GRAM_STAGES) mbar_init(bars + threadIdx.x, 1);
@@ -97,8 +98,8 @@ k_trsm_gram_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
                 wr.issue(stage, next, lane);
             }
         };
-        double* xsc = xs + (it & 1) * 8 * N8;
-        const double* xsp = xs + ((it & 1) ^ 1) * 8 * N8;
+        double* xsc = xs + (it & 1) * XB;
+        const double* xsp = xs + ((it & 1) ^ 1) * XB;
         if (HAS_R) {
             double* gp = (V1 && (lane >> 2) < valid) ? V1 + rblk * 8 * ldq + lane_off : nullptr;
             if (it > 0) trsm_rowblock<NB, true, true, FULL>(acc, xsc, xsp, ad, Tf, nRf, gp, colmask, lane, g, G, refill);
@@ -116,7 +117,7 @@ k_trsm_gram_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
     }
     if (it > 0) {
         __syncwarp();
-        gram_chunk<NB, N8, 0, 2 * NBLK>(xs + ((it - 1) & 1) * 8 * N8, ad, g, G);
+        gram_chunk<NB, N8, 0, 2 * NBLK>(xs + ((it - 1) & 1) * XB, ad, g, G);
     }
     // fixed-order reduction of the warps' accumulators, then this CTA's partial (upper blocks)
     __syncthreads();
@@ -504,9 +505,11 @@ int rqr_trsm_gram_mma(const double* V, int64_t m, int n, int64_t ldv, const doub
         g_a4_pair = (e && e[0] == '0') ? 0 : 1;
     }
     if (n <= 16) return launch_trsm_gram<2>(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
+    if (n <= 24) return launch_trsm_gram<3>(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
     if (n <= 32) return launch_trsm_gram<4>(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
-    // 32 < n <= 48: 6 column blocks instead of 8 (42 + 42 DMMA per 8 rows against 72 + 72).  The column-block count
-    // must be even: the XOR swizzle of the X staging block (XsAddr) permutes 16-double groups of a row.
+    if (n <= 40) return launch_trsm_gram<5>(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
+    // column blocks of 8: n <= 16, 24, 32, 40, 48 run 2, 3, 4, 5, 6 blocks (NB (NB + 1) DMMA per 8 rows for the
+    // substitution and as many for the Gram), above 48 the 8-block pair kernel
     if (n <= 48) return launch_trsm_gram<6>(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
     if (g_a4_pair && R0) return launch_trsm_gram_pair(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
     return launch_trsm_gram<8>(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
@@ -545,7 +548,9 @@ int rqr_apply_mma(const double* V, int64_t m, int n, int64_t ldv, const double* 
 {
     if (!fast_ok(V, n, ldv, Q, ldq)) return RQR_TALL_NOT_HANDLED;
     if (n <= 16) return launch_apply<2>(V, m, n, ldv, R0, R1, Q, ldq, st);
+    if (n <= 24) return launch_apply<3>(V, m, n, ldv, R0, R1, Q, ldq, st);
     if (n <= 32) return launch_apply<4>(V, m, n, ldv, R0, R1, Q, ldq, st);
+    if (n <= 40) return launch_apply<5>(V, m, n, ldv, R0, R1, Q, ldq, st);
     if (n <= 48) return launch_apply<6>(V, m, n, ldv, R0, R1, Q, ldq, st);
     return launch_apply<8>(V, m, n, ldv, R0, R1, Q, ldq, st);
 }

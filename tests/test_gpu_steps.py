@@ -148,8 +148,10 @@ SHAPES_TALL = [(20000, 16), (4099, 64), (10000, 70), (3000, 32), (2500, 128), (7
                (40003, 128), (30011, 200), (20000, 256), (9001, 66),
                # last panel of 16 / 48 columns at 2, 3 and 4 panels (panel_last_nb = 2, 6)
                (3001, 80), (3001, 100), (2003, 112), (2000, 140), (2000, 176), (1500, 208), (1500, 240),
-               # 5 and 6 column blocks (32 < n <= 48)
-               (5000, 40), (4099, 36), (5003, 48), (3001, 44)]
+               # 5 and 6 column blocks (32 < n <= 48; 5 blocks: X staging row padded from 40 to 48 doubles)
+               (5000, 40), (4099, 36), (5003, 48), (3001, 44),
+               # 3 column blocks (16 < n <= 24): the X staging row is padded to 32 doubles
+               (5000, 20), (4099, 24), (3001, 18)]
 
 
 @pytest.mark.parametrize("m,n", SHAPES_TALL)
