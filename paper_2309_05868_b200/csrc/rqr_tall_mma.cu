@@ -31,7 +31,7 @@
 // shapes have small Gram tiles and little work per row-block, so they run more warps to hide the
 // per-row-block latencies (mbarrier wait, chain start).  Measured at 2^22 x 32: 0.48 -> 0.37 ms.
 // NB = 5, 6 (32 < n <= 48): 15 / 21 Gram blocks = 60 / 84 accumulator registers => 12 warps (168 registers each).
-template <int NB> struct GramWarps { static constexpr int value = NB >= 8 ? 8 : (NB >= 5 ? 12 : (NB >= 3 ? 16 : 24)); };
+template <int NB> struct GramWarps { static constexpr int value = NB >= 7 ? 8 : (NB >= 5 ? 12 : (NB >= 3 ? 16 : 24)); };
 
 template <int NB, bool HAS_R, bool FULL>
 __global__ void __launch_bounds__(GramWarps<NB>::value * 32, 1)
@@ -511,6 +511,7 @@ int rqr_trsm_gram_mma(const double* V, int64_t m, int n, int64_t ldv, const doub
     // column blocks of 8: n <= 16, 24, 32, 40, 48 run 2, 3, 4, 5, 6 blocks (NB (NB + 1) DMMA per 8 rows for the
     // substitution and as many for the Gram), above 48 the 8-block pair kernel
     if (n <= 48) return launch_trsm_gram<6>(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
+    if (n <= 56) return launch_trsm_gram<7>(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
     if (g_a4_pair && R0) return launch_trsm_gram_pair(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
     return launch_trsm_gram<8>(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
 }
@@ -552,5 +553,6 @@ int rqr_apply_mma(const double* V, int64_t m, int n, int64_t ldv, const double* 
     if (n <= 32) return launch_apply<4>(V, m, n, ldv, R0, R1, Q, ldq, st);
     if (n <= 40) return launch_apply<5>(V, m, n, ldv, R0, R1, Q, ldq, st);
     if (n <= 48) return launch_apply<6>(V, m, n, ldv, R0, R1, Q, ldq, st);
+    if (n <= 56) return launch_apply<7>(V, m, n, ldv, R0, R1, Q, ldq, st);
     return launch_apply<8>(V, m, n, ldv, R0, R1, Q, ldq, st);
 }

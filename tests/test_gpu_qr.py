@@ -55,7 +55,8 @@ def run_rand(rq, Vd, s1, s2, seed, variant=0, flags=0, prepared=False):
 CASES = [("C1", 20000, 16, 1e10), ("n64", 65536, 64, 1e12), ("n70", 100000, 70, 1e8),
          ("n32", 40000, 32, 1e14), ("n128", 40000, 128, 1e12), ("n256", 140000, 256, 1e14),
          ("tiny", 600, 8, 1e5), ("ragged", 4099, 24, 1e6), ("n40", 50000, 40, 1e10), ("n48", 50001, 48, 1e12),
-         ("n80", 60000, 80, 1e10), ("n112", 50000, 112, 1e12), ("n20", 70000, 20, 1e12), ("n36", 50000, 36, 1e10)]
+         ("n80", 60000, 80, 1e10), ("n112", 50000, 112, 1e12), ("n20", 70000, 20, 1e12), ("n36", 50000, 36, 1e10),
+         ("n50", 50000, 50, 1e12)]
 
 
 @pytest.mark.parametrize("name,m,n,kappa", CASES)

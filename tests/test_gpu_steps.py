@@ -151,7 +151,9 @@ SHAPES_TALL = [(20000, 16), (4099, 64), (10000, 70), (3000, 32), (2500, 128), (7
                # 5 and 6 column blocks (32 < n <= 48; 5 blocks: X staging row padded from 40 to 48 doubles)
                (5000, 40), (4099, 36), (5003, 48), (3001, 44),
                # 3 column blocks (16 < n <= 24): the X staging row is padded to 32 doubles
-               (5000, 20), (4099, 24), (3001, 18)]
+               (5000, 20), (4099, 24), (3001, 18),
+               # 7 column blocks (48 < n <= 56)
+               (5000, 50), (4099, 56), (3001, 52)]
 
 
 @pytest.mark.parametrize("m,n", SHAPES_TALL)
