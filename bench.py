@@ -112,7 +112,8 @@ def launches_per_step(n, m=0):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # ncu --set full captures (profiles/): workload -> bytes
-NCU_TRAFFIC = {"C2": 537.0e6 + 491.5e6}
+NCU_TRAFFIC = {"C2": 537.0e6 + 491.5e6,                               # k_trsm_gram_pair, profiles/r1_final_summary.md section 2
+               "C4": 4.295e9 + 4.245e9 + 6.086e9 + 0.007e9}             # k_trsm_panel + k_syrk_fold, profiles/r1_c4_summary.md section 2
 
 
 def measured_peaks():
@@ -410,7 +411,7 @@ def main():
         ach = flops.trsm_gram_flops(m, n) / (bd[dom] * 1e-3) / 1e12
         roof = {"kernel": "rqr_trsm_gram", "bound": "tensor", "achieved": ach, "peak": p64, "unit": "TFLOP/s",
                 "frac": ach / p64, "traffic": NCU_TRAFFIC.get(args.workload),
-                "traffic_source": "profiles/r1_final_summary.md section 2 (ncu --set full, per launch)",
+                "traffic_source": "profiles/%s section 2 (ncu --set full, per launch)" % ("r1_c4_summary.md" if args.workload == "C4" else "r1_final_summary.md"),
                 "algorithmic": "2 m n^2 flops per launch (n^2 substitution + n^2 symmetric Gram per row); "
                                "16 m n bytes (read V, write V1)",
                 "peak_source": "FP64 probe measured live in this run (max of DFMA %.1f / DMMA %.1f TFLOP/s); "

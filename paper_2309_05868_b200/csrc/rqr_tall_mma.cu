@@ -143,7 +143,7 @@ k_trsm_gram_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
 }
 
 // ------------------------------------------------------------------------------------------
-// A4, pair version for 32 < n <= 64 (NB = 8).  The single-warp kernel above needs 248 registers
+// A4, pair version for 56 < n <= 64 (NB = 8; narrower shapes run k_trsm_gram_mma<NB> with NB = ceil(n / 8)).  The single-warp kernel above needs 248 registers
 // (36 Gram accumulators), i.e. 2 warps per SM sub-partition, and loses ~15% of the DMMA pipe to
 // moments when both are stalled.  Here two warps form a PAIR: each runs the substitution chain of its
 // own row-block, both write X into a pair-shared staging block, and each accumulates HALF of the
