@@ -413,7 +413,7 @@ def main():
                 "frac": ach / p64, "traffic": NCU_TRAFFIC.get(args.workload),
                 "traffic_source": "profiles/%s section 2 (ncu --set full, per launch)" % ("r1_c4_summary.md" if args.workload == "C4" else "r1_final_summary.md"),
                 "algorithmic": "2 m n^2 flops per launch (n^2 substitution + n^2 symmetric Gram per row); "
-                               "16 m n bytes (read V, write V1)",
+                               "16 m n bytes (read V, write V1)" + ("; n > 64: two kernels, the syrk re-reads V1 (24 m n)" if n > 64 else ""),
                 "peak_source": "FP64 probe measured live in this run (max of DFMA %.1f / DMMA %.1f TFLOP/s); "
                                "MEASURED_PEAKS.json has no FP64 figure; bf16 x nominal ratio would give %.1f"
                                % (p64s["dfma"], p64s["dmma"], ratio_peak)}
