@@ -202,16 +202,22 @@ template <int VEC>
 __global__ void __launch_bounds__(256)
 k_countsketch_gather(const double* __restrict__ V, int64_t ldv, int n,
                      const uint32_t* __restrict__ off, const uint32_t* __restrict__ entries,
-                     uint32_t s1, double* __restrict__ W1)
+                     uint32_t s1, double* __restrict__ W1, uint32_t split)
 {
+    // split > 1 (fewer buckets than resident CTAs): work item w = bucket b, segment j of its row list; the
+    // segment sums go to W1[j][b][:] (a scratch of split partial sketches) and are added in order j = 0, 1, ...
+    // by k_reduce_partials.
     extern __shared__ double red[];                 // R * n doubles
     const int lpr = (n + VEC - 1) / VEC;            // lanes per row
     const int R = max(1, 256 / lpr);
     const int slot = threadIdx.x / lpr;
     const int col = (threadIdx.x % lpr) * VEC;
     const bool active = slot < R && col < n;
-    for (uint32_t b = blockIdx.x; b < s1; b += gridDim.x) {
-        const uint32_t beg = off[b], end = off[b + 1];
+    for (uint32_t w = blockIdx.x; w < s1 * split; w += gridDim.x) {
+        const uint32_t b = w / split, j = w - b * split;
+        const uint32_t beg0 = off[b], len = off[b + 1] - beg0;
+        const uint32_t beg = beg0 + (uint32_t)((uint64_t)len * j / split);
+        const uint32_t end = beg0 + (uint32_t)((uint64_t)len * (j + 1) / split);
         double a0 = 0.0, a1 = 0.0;
         if (active) {
             uint32_t k = beg + slot;
@@ -252,11 +258,13 @@ k_countsketch_gather(const double* __restrict__ V, int64_t ldv, int n,
         for (int c = threadIdx.x; c < n; c += blockDim.x) {
             double s = red[c];
             for (int r = 1; r < R; ++r) s += red[r * n + c];
-            W1[(int64_t)b * n + c] = s;
+            W1[((int64_t)j * s1 + b) * n + c] = s;
         }
         __syncthreads();
     }
 }
+
+__global__ void __launch_bounds__(256) k_reduce_partials(const double* __restrict__ part, int nparts, int64_t elems, double* __restrict__ out);
 
 // SCATTER variant: stream V in row order, hash on the fly, red.global.add.f64 into W1 (which
 // lives in L2).  Order of the atomics is not fixed => last bits vary run to run.
@@ -322,10 +330,29 @@ extern "C" int rqr_countsketch(const double* V, int64_t m, int n, int64_t ldv, i
     const int lpr = vec2 ? n / 2 : n;
     const int R = 256 / lpr > 1 ? 256 / lpr : 1;
     size_t smem = (size_t)R * n * sizeof(double);
-    int blocks = (int)(s1 < 148 * 8 ? s1 : 148 * 8);
-    if (vec2) k_countsketch_gather<2><<<blocks, 256, smem, st>>>(V, ldv, n, off, ent, (uint32_t)s1, W1);
-    else      k_countsketch_gather<1><<<blocks, 256, smem, st>>>(V, ldv, n, off, ent, (uint32_t)s1, W1);
+    // fewer buckets than half the resident CTAs (148 x 8): split every bucket's row list into `split` segments so
+    // that the grid is full; the partial sketches live in region A of the workspace (free during A1)
+    int64_t split = 1;
+    if (s1 * 2 <= 148 * 8) {
+        split = (148 * 8 + s1 - 1) / s1;
+        const int64_t fit = (int64_t)rqr_gram_partial_cap(n) * n / s1;          // region A holds cap n^2 doubles
+        const int64_t rows = m / (s1 * 4 * R);                                  // >= 4 R rows per segment
+        if (split > fit) split = fit;
+        if (split > rows) split = rows;
+        if (split > 64) split = 64;
+        if (split < 2) split = 1;
+    }
+    double* dst = split > 1 ? (double*)(w + L.A) : W1;
+    const int64_t items = s1 * split;
+    int blocks = (int)(items < 148 * 8 ? items : 148 * 8);
+    if (vec2) k_countsketch_gather<2><<<blocks, 256, smem, st>>>(V, ldv, n, off, ent, (uint32_t)s1, dst, (uint32_t)split);
+    else      k_countsketch_gather<1><<<blocks, 256, smem, st>>>(V, ldv, n, off, ent, (uint32_t)s1, dst, (uint32_t)split);
     RQR_LAUNCH_CHECK();
+    if (split > 1) {
+        const int64_t elems = s1 * n;
+        k_reduce_partials<<<(int)((elems + 63) / 64), 256, 0, st>>>(dst, (int)split, elems, W1);
+        RQR_LAUNCH_CHECK();
+    }
     return RQR_OK;
 }
 

@@ -55,7 +55,9 @@ def test_prepared_S2_matches_oracle(rq, orc):
 
 
 @pytest.mark.parametrize("m,n,s1", [(20000, 16, 512), (100000, 70, 9940), (65536, 64, 8192),
-                                    (5000, 33, 64), (3000, 256, 4000), (37, 8, 16), (8192, 2, 8)])
+                                    (5000, 33, 64), (3000, 256, 4000), (37, 8, 16), (8192, 2, 8),
+                                    # few buckets: every bucket's row list is split over several CTAs (two-stage sum)
+                                    (200000, 10, 200), (150001, 16, 64), (120000, 7, 37), (300000, 24, 500)])
 @pytest.mark.parametrize("variant", [0, 1])
 def test_countsketch_parity(rq, orc, m, n, s1, variant):
     V = inputs.make_V(m, n, 1e8, 7)
