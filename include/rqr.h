@@ -33,9 +33,12 @@
  *    dimensions and 16-byte aligned bases (2 <= n <= 64: fused kernels; 64 < n <= 256: panel
  *    kernels); rqr_gauss_sketch uses its DMMA GEMM for even n >= 96 with s1 % 16 == 0.  Any other
  *    shape runs the generic kernels: same results to rounding, much slower.
- *  - Thread safety: calls on different streams with different buffers are independent.  The only
- *    global state is one-time kernel-attribute initialisation and the two debug switches
- *    (rqr_debug_force_generic, environment variable RQR_A4_PAIR=0 read once).
+ *  - Thread safety: calls on different streams with different buffers are independent, from any host thread and on
+ *    any device.  The library keeps no state besides the per-device "kernel attributes set" flags (atomic; the
+ *    opt-in to > 48 KB of shared memory is per device and is repeated on the first call on each device).
+ *  - Dynamic range: the Householder and Cholesky kernels form sums of squares of the sketch entries without
+ *    scaling, so |V| must stay within about [1e-140, 1e140] (entries of W = S2 S1 V below 1e-154 or above 1e154
+ *    would under/overflow in the squares and be reported as RQR_INFO_SINGULAR).
  */
 #ifndef RQR_H
 #define RQR_H
@@ -49,6 +52,7 @@ extern "C" {
 
 #define RQR_OK 0
 #define RQR_ERR_LAUNCH (-1000)
+#define RQR_ERR_COMM (-1001)   /* the caller's all-reduce callback of rqr_rand_cholqr_sharded returned non-zero */
 #define RQR_INFO_NOT_SPD 1000
 #define RQR_INFO_SINGULAR 2000
 
@@ -68,6 +72,13 @@ extern "C" {
                                  the apply pass with bit-identical arithmetic (32mn bytes of
                                  traffic instead of 40mn, 4mn^2 flops instead of 3mn^2).
                                  Honoured for n <= 64; for n > 64 V1 is always stored.       */
+#define RQR_FLAG_STORE_V1 4   /* one-shot drivers: store V1 into Q in A4 and transform it in place in A6.
+                                 With neither flag the drivers choose per n: recomputed for n <= 40 (the
+                                 path is HBM-bound there and moves 32mn instead of 40mn bytes), stored above
+                                 (A4 / A6 are FP64-bound and the extra mn^2 flops would not hide).  When V and
+                                 Q would not take the same kernel family (Q not 16-byte aligned while V is,
+                                 even n) V1 is stored whatever the flags say: a V1 re-formed by different
+                                 arithmetic would break the orthogonality of Q (DESIGN.md hazard H1).      */
 
 #define RQR_S2_RADEMACHER 16  /* SURVEY.md 8(f) N4, PAPER.md:947 ("dense Rademacher sketch matrices in
                                  place of dense Gaussian sketches"): S2 has entries +-1/sqrt(s2)
@@ -140,6 +151,21 @@ int rqr_rand_cholqr(const double* V, int64_t m, int n, int64_t s1, int s2, uint6
                     double* Q, double* R, void* work, int* d_info, int variant, int flags,
                     void* stream);
 
+/* Row-sharded Alg. 3 over several GPUs, one process per GPU: this rank holds the rows
+ * [row0, row0 + m) of an m_total x n matrix (V, Q: m x n, ld n; a rank may hold fewer than n rows).  Bucket and
+ * sign of a row are functions of its GLOBAL index, S2 is replicated, and the ranks meet exactly twice -- "rand_cholQR
+ * only requires two synchronizations total": the sum of the local sketches W_k = S2 (S1)_k V_k
+ * (s2 x n; PAPER.md:228 footnote 3) and the sum of the local Gram matrices (n x n).  The library links no
+ * communication library: `allreduce(ctx, buf, count, stream)` is the caller's in-place sum of `count` doubles at
+ * the DEVICE pointer `buf` over all ranks, enqueued on `stream` (e.g. ncclAllReduce(buf, buf, count, ncclDouble,
+ * ncclSum, comm, stream)); it must return 0, give every rank the same bits, and be capturable if the call is
+ * captured.  allreduce == NULL: one rank.  Every rank ends with the same R; Q holds this rank's rows.
+ * A workspace prepared with RQR_FLAG_PREPARED must have been prepared with the same row0.                      */
+typedef int (*rqr_allreduce_fn)(void* ctx, double* buf, int64_t count, void* stream);
+int rqr_rand_cholqr_sharded(const double* V, int64_t m, int64_t row0, int64_t m_total, int n, int64_t s1, int s2,
+                            uint64_t seed, double* Q, double* R, void* work, int* d_info, int variant, int flags,
+                            rqr_allreduce_fn allreduce, void* ctx, void* stream);
+
 /* Batched / strided form for block-Krylov use ("Krylov subspace methods that
  * require tall-and-skinny QR factorizations, particularly block ..."): `batch` problems of the same shape,
  * problem b at V + b strideV (m x n, ld n), Q + b strideQ, R + b n^2, d_info + b.  The sketch operator is the
@@ -182,12 +208,22 @@ int rqr_debug_gauss(uint64_t seed, uint32_t stream_id, uint64_t first, int64_t c
 /* Pointer to S2 (s2 x s1) inside a workspace prepared for (n, s1).  Row r starts at r * ld with
  * ld = s1 rounded up to a multiple of 16; the pad columns hold zeros.                         */
 const double* rqr_workspace_S2(void* work, int n, int64_t s1);
+/* Pointers to the bucket offsets (s1 + 1 uint32) and the bucket-sorted row list (m uint32: local row index in the
+ * low 31 bits, sign bit 31 set for sigma = -1) that rqr_sketch_prepare (RQR_VARIANT_SORTED) wrote into a workspace
+ * sized for (m, n, s1, variant).                                                                           */
+int rqr_workspace_rows(void* work, int64_t m, int n, int64_t s1, int variant, const uint32_t** offsets,
+                       const uint32_t** entries);
+/* Device pointer to the shift the last rqr_scholqr3 call on this workspace used (reading S9).                 */
+const double* rqr_workspace_scholqr3_shift(void* work);
 /* test hook: the signs (+1 / -1) of the Rademacher S2 entries (row, c0 .. c0 + count) for sketch width s1 */
 int rqr_debug_rademacher(uint64_t seed, int64_t s1, int row, int64_t c0, int64_t count, int8_t* sign,
                          void* stream);
 
-/* Test hook: on != 0 forces the generic (non-DMMA) kernels in rqr_trsm_gram / rqr_apply.       */
-void rqr_debug_force_generic(int on);
+/* Test hooks: rqr_trsm_gram / rqr_apply on the generic (non-DMMA) kernels whatever the shape.    */
+int rqr_debug_trsm_gram_generic(const double* V, int64_t m, int n, int64_t ldv, const double* R0, double* G,
+                                double* V1, int64_t ldq, void* work, void* stream);
+int rqr_debug_apply_generic(const double* V, int64_t m, int n, int64_t ldv, const double* R0, const double* R1,
+                            double* Q, int64_t ldq, void* work, void* stream);
 
 /* Library version string. */
 const char* rqr_version(void);

@@ -1,7 +1,7 @@
 /*
- * rqr_probe.h -- measurement helpers of librqr (not on the hot path): FP64 peak probes used as
- * the roofline denominator.  MEASURED_PEAKS.json has no FP64 figure, so
- * bench.py measures it with these two register-resident kernels and CUDA events.
+ * rqr_probe.h -- bench-only measurement helper (librqr_probe.so, NOT part of librqr.so or of include/): FP64 peak
+ * probes used as the roofline denominator.  MEASURED_PEAKS.json has no FP64 figure, so bench.py
+ * measures it with these register-resident kernels and CUDA events.
  */
 #ifndef RQR_PROBE_H
 #define RQR_PROBE_H

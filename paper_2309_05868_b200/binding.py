@@ -21,17 +21,15 @@ VARIANT_SORTED = 0
 VARIANT_SCATTER = 1
 FLAG_PREPARED = 1
 FLAG_RECOMPUTE_V1 = 2
+FLAG_STORE_V1 = 4
 S2_RADEMACHER = 16          # OR into `variant` (workspace, prepare, countsketch, rand_cholqr) / `flags` (gauss_sketch)
 MAX_N = 256                 # argument limits of include/rqr.h
 MAX_S2 = 1024
-PROBE_DFMA = 0
-PROBE_DMMA = 1
-PROBE_MIX = 2
 
 _i64, _u64, _u32, _int, _dbl, _vp, _sz = (ctypes.c_int64, ctypes.c_uint64, ctypes.c_uint32, ctypes.c_int,
                                           ctypes.c_double, ctypes.c_void_p, ctypes.c_size_t)
 
-# name -> (restype, argtypes); mirrors include/rqr.h and include/rqr_probe.h
+# name -> (restype, argtypes); mirrors include/rqr.h
 SIGNATURES = {
     "rqr_workspace_bytes": (_sz, [_i64, _int, _i64, _int, _int]),
     "rqr_sketch_prepare": (_int, [_i64, _int, _i64, _i64, _int, _u64, _int, _vp, _vp]),
@@ -43,6 +41,8 @@ SIGNATURES = {
     "rqr_apply": (_int, [_vp, _i64, _int, _i64, _vp, _vp, _vp, _i64, _vp, _vp]),
     "rqr_triu_mul": (_int, [_vp, _vp, _int, _vp, _vp]),
     "rqr_rand_cholqr": (_int, [_vp, _i64, _int, _i64, _int, _u64, _vp, _vp, _vp, _vp, _int, _int, _vp]),
+    "rqr_rand_cholqr_sharded": (_int, [_vp, _i64, _i64, _i64, _int, _i64, _int, _u64, _vp, _vp, _vp, _vp, _int, _int, _vp,
+                                       _vp, _vp]),
     "rqr_rand_cholqr_batched": (_int, [_vp, _i64, _int, _int, _i64, _i64, _int, _u64, _vp, _i64, _vp, _vp, _vp, _int, _int,
                                        _vp]),
     "rqr_cholqr2": (_int, [_vp, _i64, _int, _vp, _vp, _vp, _vp, _vp]),
@@ -54,10 +54,12 @@ SIGNATURES = {
     "rqr_debug_hash_sign": (_int, [_u64, _i64, _i64, _i64, _vp, _vp, _vp]),
     "rqr_debug_gauss": (_int, [_u64, _u32, _u64, _i64, _vp, _vp]),
     "rqr_workspace_S2": (_vp, [_vp, _int, _i64]),
+    "rqr_workspace_rows": (_int, [_vp, _i64, _int, _i64, _int, _vp, _vp]),
+    "rqr_workspace_scholqr3_shift": (_vp, [_vp]),
     "rqr_debug_rademacher": (_int, [_u64, _i64, _int, _i64, _i64, _vp, _vp]),
-    "rqr_debug_force_generic": (None, [_int]),
+    "rqr_debug_trsm_gram_generic": (_int, [_vp, _i64, _int, _i64, _vp, _vp, _vp, _i64, _vp, _vp]),
+    "rqr_debug_apply_generic": (_int, [_vp, _i64, _int, _i64, _vp, _vp, _vp, _i64, _vp, _vp]),
     "rqr_version": (ctypes.c_char_p, []),
-    "rqr_probe_fp64": (_int, [_int, _int, _int, _vp, _vp, _vp]),
 }
 
 _lib = None
@@ -152,8 +154,8 @@ def trsm_gram(V, R0, G, V1, work):
     _f64(V, "V"); _f64(G, "G")
     m, n = V.shape
     ldq = V1.stride(0) if V1 is not None else n
-    _chk(lib().rqr_trsm_gram(_ptr(V), m, n, V.stride(0), _ptr(R0), _ptr(G), _ptr(V1), ldq, _ptr(work), _stream()),
-         "rqr_trsm_gram")
+    f = lib().rqr_debug_trsm_gram_generic if _force_generic else lib().rqr_trsm_gram
+    _chk(f(_ptr(V), m, n, V.stride(0), _ptr(R0), _ptr(G), _ptr(V1), ldq, _ptr(work), _stream()), "rqr_trsm_gram")
 
 
 def chol(G, R1, info=None, shift=0.0):
@@ -164,8 +166,8 @@ def chol(G, R1, info=None, shift=0.0):
 def apply(V, R0, R1, Q, work=None):
     _f64(V, "V"); _f64(Q, "Q")
     m, n = V.shape
-    _chk(lib().rqr_apply(_ptr(V), m, n, V.stride(0), _ptr(R0), _ptr(R1), _ptr(Q), Q.stride(0), _ptr(work), _stream()),
-         "rqr_apply")
+    f = lib().rqr_debug_apply_generic if _force_generic else lib().rqr_apply
+    _chk(f(_ptr(V), m, n, V.stride(0), _ptr(R0), _ptr(R1), _ptr(Q), Q.stride(0), _ptr(work), _stream()), "rqr_apply")
 
 
 def triu_mul(R1, R0, R):
@@ -178,6 +180,36 @@ def rand_cholqr(V, s1, s2, seed, Q, R, work, info, variant=VARIANT_SORTED, flags
     assert V.is_contiguous() and Q.is_contiguous()
     _chk(lib().rqr_rand_cholqr(_ptr(V), m, n, s1, s2, seed, _ptr(Q), _ptr(R), _ptr(work), _ptr(info), variant, flags,
                                _stream()), "rqr_rand_cholqr")
+
+
+ALLREDUCE_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p)
+
+
+def rand_cholqr_sharded(V, row0, m_total, s1, s2, seed, Q, R, work, info, variant=VARIANT_SORTED, flags=0,
+                        allreduce=None):
+    """Row-sharded one-shot on this rank's rows.  `allreduce(t)` sums the float64 device tensor t in place over the
+    ranks on torch's current stream (e.g. torch.distributed.all_reduce); the library hands it W (s2 x n) and G
+    (n x n), both views into `work`.  None: one rank."""
+    _f64(V, "V"); _f64(Q, "Q"); _f64(R, "R")
+    m, n = V.shape
+    assert V.is_contiguous() and Q.is_contiguous()
+    base = work.data_ptr()
+    err = []
+
+    def _cb(ctx, buf, count, stream):
+        try:
+            off = buf - base
+            allreduce(work[off: off + 8 * count].view(torch.float64))
+            return 0
+        except BaseException as e:              # an exception must not unwind through the C frames
+            err.append(e)
+            return 1
+    cb = ALLREDUCE_FN(_cb) if allreduce is not None else None
+    rc = lib().rqr_rand_cholqr_sharded(_ptr(V), m, row0, m_total, n, s1, s2, seed, _ptr(Q), _ptr(R), _ptr(work),
+                                       _ptr(info), variant, flags, cb, None, _stream())
+    if err:
+        raise err[0]
+    _chk(rc, "rqr_rand_cholqr_sharded")
 
 
 def rand_cholqr_batched(V, s1, s2, seed, Q, R, work, info, variant=VARIANT_SORTED, flags=0):
@@ -254,11 +286,25 @@ def workspace_S2(work, n, s1, s2):
     return work[off: off + s2 * ld * 8].view(torch.float64).view(s2, ld)[:, :s1]
 
 
+def workspace_rows(work, m, n, s1, variant=VARIANT_SORTED):
+    """Views of the bucket offsets (s1 + 1, int32 bit patterns) and the sorted row list (m, int32 bit patterns of
+    uint32 row | sign << 31) inside a prepared workspace."""
+    po, pe = ctypes.c_void_p(0), ctypes.c_void_p(0)
+    _chk(lib().rqr_workspace_rows(_ptr(work), m, n, s1, variant, ctypes.byref(po), ctypes.byref(pe)), "rqr_workspace_rows")
+    o0, e0 = po.value - work.data_ptr(), pe.value - work.data_ptr()
+    return work[o0: o0 + 4 * (s1 + 1)].view(torch.int32), work[e0: e0 + 4 * m].view(torch.int32)
+
+
+def workspace_scholqr3_shift(work):
+    off = lib().rqr_workspace_scholqr3_shift(_ptr(work)) - work.data_ptr()
+    return work[off: off + 8].view(torch.float64)
+
+
+_force_generic = False
+
+
 def force_generic(on: bool):
-    lib().rqr_debug_force_generic(1 if on else 0)
-
-
-def probe_fp64(kind, iters, blocks, sink):
-    fl = _dbl(0.0)
-    _chk(lib().rqr_probe_fp64(kind, iters, blocks, _ptr(sink), ctypes.addressof(fl), _stream()), "rqr_probe_fp64")
-    return fl.value
+    """Test hook (binding-side switch, no state in the library): trsm_gram / apply call the library's
+    rqr_debug_*_generic entry points, which run the generic (non-DMMA) kernels."""
+    global _force_generic
+    _force_generic = bool(on)

@@ -7,7 +7,9 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "librqr.so")
-SOURCES = ["rqr_sketch.cu", "rqr_gauss_mma.cu", "rqr_small.cu", "rqr_tall.cu", "rqr_tall_mma.cu", "rqr_tall_panel.cu", "rqr_api.cu", "rqr_probe.cu"]
+PROBE_DIR = os.path.join(HERE, "bench_probe")
+PROBE_LIB = os.path.join(HERE, "librqr_probe.so")       # bench-only FP64 peak probe, not part of librqr.so
+SOURCES = ["rqr_sketch.cu", "rqr_gauss_mma.cu", "rqr_small.cu", "rqr_tall.cu", "rqr_tall_mma.cu", "rqr_tall_panel.cu", "rqr_api.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
@@ -50,5 +52,20 @@ def build_lib(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_probe(force: bool = False) -> str:
+    """The FP64 peak probe of bench.py / sweep.py (bench_probe/): its own small shared object."""
+    src = os.path.join(PROBE_DIR, "rqr_probe.cu")
+    if not force and os.path.exists(PROBE_LIB) and all(
+            os.path.getmtime(os.path.join(PROBE_DIR, f)) <= os.path.getmtime(PROBE_LIB) for f in os.listdir(PROBE_DIR)):
+        return PROBE_LIB
+    cmd = ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
+           "-shared", src, "-o", PROBE_LIB]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if r.returncode != 0:
+        raise RuntimeError("nvcc failed for the probe:\n" + r.stderr)
+    return PROBE_LIB
+
+
 if __name__ == "__main__":
     print(build_lib(force=True, verbose=True))
+    print(build_probe(force=True))

@@ -11,6 +11,13 @@ int rqr_tsqr_r_wide_dev(double* A, int64_t rows, int n, double* R, double* scrat
 
 extern "C" const char* rqr_version(void) { return "rqr 0.1 (sm_100a)"; }
 
+// header slot of the workspace that rqr_scholqr3 writes its shift to
+#define RQR_HDR_SHIFT_SLOT 8
+extern "C" const double* rqr_workspace_scholqr3_shift(void* work)
+{
+    return work ? (const double*)work + RQR_HDR_SHIFT_SLOT : nullptr;
+}
+
 extern "C" size_t rqr_workspace_bytes(int64_t m, int n, int64_t s1, int s2, int variant)
 {
     if (m < 1 || n < 2 || n > RQR_MAX_N || s1 < 1 || s2 < 1 || s2 > RQR_MAX_S2) return 0;
@@ -37,31 +44,53 @@ static int check_common(const double* V, int64_t m, int n, double* Q, double* R,
     return RQR_OK;
 }
 
-// cholQR of V R0^-1: shared tail of every driver.  A4 with R0 writes V1 into Q, A5 (which also forms
-// Rprod = R1 R0, the drivers' A7, when Rprod != NULL), A6 in place.
-static int tail_cholqr(const double* V, int64_t m, int n, const double* R0, double* Q, double* R1,
-                       double* G, void* work, int* d_info, int recompute, cudaStream_t st, double* Rprod)
+// V1 = V R0^-1 stored or recomputed (PAPER.md:220-222 flop terms; reading S20).  Stored: A4 writes V1
+// into Q and A6 transforms it in place: 40mn bytes, 3mn^2 flops.  Recomputed: A4 stores nothing and A6 re-forms V1
+// with the bit-identical routine: 32mn bytes, 4mn^2 flops.  The path is HBM-bound for n <= 32 (n/8 flop/B in A6
+// against a ridge of 5.7) and FP64-bound from n = 48 up, so the default is "recompute iff n <= RQR_AUTO_RECOMPUTE_MAX_N"
+// (measured: profiles/r2_v1_mode.md); RQR_FLAG_RECOMPUTE_V1 / RQR_FLAG_STORE_V1 override it.  Every driver
+// (CholeskyQR2 and sCholQR3 included) takes the same decision: the comparison stays on the same kernels.
+#define RQR_AUTO_RECOMPUTE_MAX_N 40
+static bool use_recompute(const double* V, int n, const double* R0, const double* Q, int flags)
 {
-    if (recompute && R0 && n <= 64) {     // n > 64: A4 is FP64-bound either way and V1 is always stored
-        RQR_TRY(rqr_trsm_gram(V, m, n, n, R0, G, nullptr, n, work, st));
-        RQR_TRY(rqr_chol_dev(G, n, 0.0, nullptr, R1, d_info, st, R0, Rprod));
-        RQR_TRY(rqr_apply(V, m, n, n, R0, R1, Q, n, work, st));
-    } else {
-        RQR_TRY(rqr_trsm_gram(V, m, n, n, R0, G, Q, n, work, st));
-        RQR_TRY(rqr_chol_dev(G, n, 0.0, nullptr, R1, d_info, st, R0, Rprod));
-        RQR_TRY(rqr_apply(Q, m, n, n, nullptr, R1, Q, n, work, st));
-    }
+    if (!R0 || n > 64) return false;      // n > 64: A4 is FP64-bound either way and V1 is always stored
+    bool want = n <= RQR_AUTO_RECOMPUTE_MAX_N;
+    if (flags & RQR_FLAG_RECOMPUTE_V1) want = true;
+    if (flags & RQR_FLAG_STORE_V1) want = false;
+    // A4 (no V1 stored) dispatches on V alone, A6 on V and Q: a V1 re-formed by the other kernel family would have
+    // other rounding (hazard H1).  Both take the same family iff n is odd (generic for both), V is misaligned
+    // (generic for both) or Q is aligned too (DMMA for both); otherwise V1 is stored.
+    const bool same_family = (n & 1) || (((uintptr_t)V & 15) != 0) || (((uintptr_t)Q & 15) == 0);
+    return want && same_family;
+}
+
+// cholQR of V R0^-1: shared tail of every driver.  A4 with R0 (stores V1 into Q unless V1 is recomputed), A5 (which
+// also forms Rprod = R1 R0, the drivers' A7, when Rprod != NULL), A6.
+// ar != NULL (row-sharded form): the Gram matrices of the ranks are summed between A4 and A5 (the
+// second of the two synchronizations).
+static int tail_cholqr(const double* V, int64_t m, int n, const double* R0, double* Q, double* R1,
+                       double* G, void* work, int* d_info, int flags, cudaStream_t st, double* Rprod,
+                       rqr_allreduce_fn ar = nullptr, void* ar_ctx = nullptr)
+{
+    const bool recompute = use_recompute(V, n, R0, Q, flags);
+    RQR_TRY(rqr_trsm_gram(V, m, n, n, R0, G, recompute ? nullptr : Q, n, work, st));
+    if (ar && ar(ar_ctx, G, (int64_t)n * n, (void*)st) != 0) return RQR_ERR_COMM;
+    RQR_TRY(rqr_chol_dev(G, n, 0.0, nullptr, R1, d_info, st, R0, Rprod));
+    if (recompute) RQR_TRY(rqr_apply(V, m, n, n, R0, R1, Q, n, work, st));
+    else           RQR_TRY(rqr_apply(Q, m, n, n, nullptr, R1, Q, n, work, st));
     return RQR_OK;
 }
 
-extern "C" int rqr_rand_cholqr(const double* V, int64_t m, int n, int64_t s1, int s2, uint64_t seed,
-                               double* Q, double* R, void* work, int* d_info, int variant,
-                               int flags, void* stream)
+// Alg. 3 on the rows [row0, row0 + m) of an m_total-row matrix; ar == NULL: the whole matrix (row0 = 0, m_total = m)
+static int rand_cholqr_impl(const double* V, int64_t m, int64_t row0, int64_t m_total, int n, int64_t s1, int s2,
+                            uint64_t seed, double* Q, double* R, void* work, int* d_info, int variant, int flags,
+                            rqr_allreduce_fn ar, void* ar_ctx, void* stream)
 {
     int rc = check_common(V, m, n, Q, R, work);
     if (rc == -100) return !Q ? -7 : (!R ? -8 : -9);
+    if (rc == -3 && n >= 2 && n <= RQR_MAX_N && n <= m_total) rc = RQR_OK;    // a shard may hold fewer than n rows
     if (rc != RQR_OK) return rc;
-    if (s1 < 1 || s1 >= ((int64_t)1 << 31) || s1 > m) return -4;
+    if (s1 < 1 || s1 >= ((int64_t)1 << 31) || s1 > m_total) return -4;
     if (s2 < n || s2 > s1 || s2 > RQR_MAX_S2) return -5;      // eq. (20)
     const int rad = variant & RQR_S2_RADEMACHER;                 // N4: Count-Rademacher multisketch
     if ((variant & ~RQR_S2_RADEMACHER) != RQR_VARIANT_SORTED && (variant & ~RQR_S2_RADEMACHER) != RQR_VARIANT_SCATTER)
@@ -75,14 +104,45 @@ extern "C" int rqr_rand_cholqr(const double* V, int64_t m, int n, int64_t s1, in
     double* W = (double*)((char*)work + L.F_W);
     if (d_info && cudaMemsetAsync(d_info, 0, sizeof(int), st) != cudaSuccess) return RQR_ERR_LAUNCH;
     if (!(flags & RQR_FLAG_PREPARED))
-        RQR_TRY(rqr_sketch_prepare(m, n, 0, s1, s2, seed, variant, work, st));
+        RQR_TRY(rqr_sketch_prepare(m, n, row0, s1, s2, seed, variant, work, st));
     // Alg. 1 randQR: W = S2 S1 V; R0 = hhqr(W).R; V1 = V R0^-1
-    RQR_TRY(rqr_countsketch(V, m, n, n, 0, s1, seed, W1, work, variant, RQR_FLAG_PREPARED, st));
+    RQR_TRY(rqr_countsketch(V, m, n, n, row0, s1, seed, W1, work, variant, RQR_FLAG_PREPARED, st));
     RQR_TRY(rqr_gauss_sketch(W1, s1, n, s2, seed, W, work, RQR_FLAG_PREPARED | rad, st));
+    // row-sharded: W = sum over the ranks of S2 (S1)_k V_k (PAPER.md:228 footnote 3), the first synchronization
+    if (ar && ar(ar_ctx, W, (int64_t)s2 * n, stream) != 0) return RQR_ERR_COMM;
     RQR_TRY(rqr_small_geqrf(W, s2, n, R0, d_info, st));
     // Alg. 2 cholQR of V1; Alg. 3 step 3
-    RQR_TRY(tail_cholqr(V, m, n, R0, Q, R1, G, work, d_info, flags & RQR_FLAG_RECOMPUTE_V1, st, R));
+    RQR_TRY(tail_cholqr(V, m, n, R0, Q, R1, G, work, d_info, flags, st, R, ar, ar_ctx));
     return RQR_OK;
+}
+
+extern "C" int rqr_rand_cholqr(const double* V, int64_t m, int n, int64_t s1, int s2, uint64_t seed,
+                               double* Q, double* R, void* work, int* d_info, int variant,
+                               int flags, void* stream)
+{
+    return rand_cholqr_impl(V, m, 0, m, n, s1, s2, seed, Q, R, work, d_info, variant, flags, nullptr, nullptr, stream);
+}
+
+// Row-sharded Alg. 3 (SURVEY.md 8(e); PAPER.md:208 "only requires two synchronizations total", :228 footnote 3).
+extern "C" int rqr_rand_cholqr_sharded(const double* V, int64_t m, int64_t row0, int64_t m_total, int n, int64_t s1,
+                                       int s2, uint64_t seed, double* Q, double* R, void* work, int* d_info,
+                                       int variant, int flags, rqr_allreduce_fn allreduce, void* ctx, void* stream)
+{
+    if (row0 < 0) return -3;
+    if (m_total < row0 + m || m_total >= ((int64_t)1 << 40)) return -4;
+    int rc = rand_cholqr_impl(V, m, row0, m_total, n, s1, s2, seed, Q, R, work, d_info, variant, flags, allreduce,
+                              ctx, stream);
+    // argument numbers of this entry point: V 1, m 2, n 5, s1 6, s2 7, Q 9, R 10, work 11, variant 13
+    switch (rc) {
+        case -3: return -5;
+        case -4: return -6;
+        case -5: return -7;
+        case -7: return -9;
+        case -8: return -10;
+        case -9: return -11;
+        case -11: return -13;
+        default: return rc;
+    }
 }
 
 extern "C" int rqr_rand_cholqr_batched(const double* V, int64_t m, int n, int batch, int64_t strideV, int64_t s1,
@@ -123,8 +183,11 @@ extern "C" int rqr_gauss_randcholqr(const double* V, int64_t m, int n, int s, ui
     return RQR_OK;
 }
 
-// rows the TSQR scratch (region A of the workspace) can take
-static int64_t tsqr_max_rows(int n) { return (int64_t)128 * rqr_gram_partial_cap(n) * 2 / 3; }
+// rows the TSQR scratch (region A of the workspace: cap blocks of n^2 doubles) can take.  The stacked R factors
+// ping-pong inside region A: level 1 writes nb0 = ceil(rows / 128) blocks, level 2 the next ceil(nb0 n / 128) <=
+// nb0 / 2 + 1 (n <= 64) behind them, and every later level fits into the space of the level two before it.
+// nb0 + nb0 / 2 + 1 <= cap - 1 holds for rows <= 128 * ((cap - 2) * 2 / 3).
+static int64_t tsqr_max_rows(int n) { return (int64_t)128 * (((int64_t)rqr_gram_partial_cap(n) - 2) * 2 / 3); }
 
 extern "C" int rqr_tsqr_r(const double* A, int64_t rows, int n, double* R, void* work, int* d_info, void* stream)
 {
@@ -159,7 +222,7 @@ extern "C" int rqr_count_randcholqr(const double* V, int64_t m, int n, int64_t s
     RQR_TRY(rqr_countsketch(V, m, n, n, 0, s1, seed, W1, work, variant, flags & RQR_FLAG_PREPARED, st));
     if (n <= 64) RQR_TRY(rqr_tsqr_r_dev(W1, s1, n, R0, (double*)((char*)work + 256), d_info, st));
     else RQR_TRY(rqr_tsqr_r_wide_dev(W1, s1, n, R0, (double*)((char*)work + 256), d_info, st));
-    RQR_TRY(tail_cholqr(V, m, n, R0, Q, R1, G, work, d_info, flags & RQR_FLAG_RECOMPUTE_V1, st, R));
+    RQR_TRY(tail_cholqr(V, m, n, R0, Q, R1, G, work, d_info, flags, st, R));
     return RQR_OK;
 }
 
@@ -196,7 +259,7 @@ extern "C" int rqr_scholqr3(const double* V, int64_t m, int n, double* Q, double
     double* RC = small_mat(work, L, n, RQR_SM_RC);
     double* T = small_mat(work, L, n, RQR_SM_R0);
     double* G = small_mat(work, L, n, RQR_SM_G);
-    double* d_shift = (double*)work + 8;               // header slot
+    double* d_shift = (double*)work + RQR_HDR_SHIFT_SLOT;
     if (d_info && cudaMemsetAsync(d_info, 0, sizeof(int), st) != cudaSuccess) return RQR_ERR_LAUNCH;
     RQR_TRY(rqr_trsm_gram(V, m, n, n, nullptr, G, nullptr, n, work, st));
     RQR_TRY(rqr_scholqr3_shift(G, n, m, d_shift, st));

@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stddef.h>
+#include <atomic>
 #include "../../include/rqr.h"
 
 #define RQR_MAX_N 256
@@ -21,6 +22,28 @@
 #define RQR_LAUNCH_CHECK()                                   \
     do {                                                     \
         if (cudaGetLastError() != cudaSuccess) return RQR_ERR_LAUNCH; \
+    } while (0)
+
+// Kernel attributes (dynamic shared memory opt-in, non-portable cluster size) are per device: the opt-in runs once
+// per DEVICE, keyed by cudaGetDevice, with an atomic flag per device (two threads racing on a first call both set
+// the same attribute: idempotent).  A device index outside the table sets the attributes on every call.
+#define RQR_MAX_DEVICES 64
+struct RqrOncePerDevice {
+    std::atomic<unsigned char> done[RQR_MAX_DEVICES];
+    int device() const
+    {
+        int d = -1;
+        return (cudaGetDevice(&d) == cudaSuccess && d >= 0 && d < RQR_MAX_DEVICES) ? d : -1;
+    }
+};
+#define RQR_ONCE_PER_DEVICE(...)                                                          \
+    do {                                                                                  \
+        static RqrOncePerDevice once__;                                                   \
+        const int dev__ = once__.device();                                                \
+        if (dev__ < 0 || !once__.done[dev__].load(std::memory_order_acquire)) {           \
+            __VA_ARGS__                                                                   \
+            if (dev__ >= 0) once__.done[dev__].store(1, std::memory_order_release);       \
+        }                                                                                 \
     } while (0)
 
 static inline size_t rqr_align256(size_t x) { return (x + 255) & ~(size_t)255; }

@@ -129,11 +129,9 @@ static int launch_gauss_mma(const double* S2, const double* W1, int64_t s1, int 
 {
     using Plan = GaussPlan<NBN>;
     static_assert(Plan::bytes <= 227 * 1024, "k_gauss_gemm_mma shared memory plan too large");
-    static bool attr = false;
-    if (!attr) {
+    RQR_ONCE_PER_DEVICE({
         cudaFuncSetAttribute(k_gauss_gemm_mma<NBN, RAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
-        attr = true;
-    }
+    });
     const int tiles_m = (s2 + 63) / 64;
     int64_t ks = 296 / tiles_m;
     if (ks > ks_cap) ks = ks_cap;

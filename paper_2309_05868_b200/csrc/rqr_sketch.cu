@@ -535,6 +535,17 @@ extern "C" const double* rqr_workspace_S2(void* work, int n, int64_t s1)
     return (const double*)((char*)work + L.C);
 }
 
+extern "C" int rqr_workspace_rows(void* work, int64_t m, int n, int64_t s1, int variant, const uint32_t** offsets,
+                                  const uint32_t** entries)
+{
+    if (!work) return -1;
+    if (m < 1 || n < 2 || n > RQR_MAX_N || s1 < 1) return -2;
+    RqrLayout L = rqr_layout(m, n, s1, (variant & RQR_S2_RADEMACHER) != 0);
+    if (offsets) *offsets = (const uint32_t*)((char*)work + L.B_off);
+    if (entries) *entries = (const uint32_t*)((char*)work + L.E);
+    return RQR_OK;
+}
+
 extern "C" int rqr_gauss_sketch(const double* W1, int64_t s1, int n, int s2, uint64_t seed,
                                 double* W, void* work, int flags, void* stream)
 {
@@ -677,11 +688,9 @@ static int launch_dense_gauss(const double* V, int64_t m, int n, int64_t ldv, in
     if (P > nchunks) P = nchunks;
     if (P < 1) P = 1;
     const size_t smem = (size_t)(32 * RT * 33 + 32 * 8 * NJ) * sizeof(double);
-    static bool attr_set = false;
-    if (!attr_set) {
+    RQR_ONCE_PER_DEVICE({
         cudaFuncSetAttribute(k_dense_gauss_sketch<NJ, RT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
-        attr_set = true;
-    }
+    });
     dim3 grid((unsigned)P, stiles);
     k_dense_gauss_sketch<NJ, RT><<<grid, 256, smem, st>>>(V, m, n, ldv, row0, m_total, s, seed, part);
     *P_out = (int)P;

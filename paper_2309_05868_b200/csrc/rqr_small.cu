@@ -703,11 +703,9 @@ extern "C" int rqr_small_geqrf(double* W, int s2, int n, double* R0, int* d_info
         if (rpl <= 32 && (int64_t)s2 * n >= 4 * 32 * 32 + 4 + n) {
             // 512 < s2 <= 1024 with 128 < n <= 256: 128 column pairs need 16 CTAs of 8 warps (64 registers of tile per
             // column): a non-portable cluster size; if the device refuses it the global-memory kernel below runs
-            static bool np = false;
-            if (!np) {
+            RQR_ONCE_PER_DEVICE({
                 cudaFuncSetAttribute(k_geqrf_cluster2<32, 2>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
-                np = true;
-            }
+            });
             if (launch_cluster(k_geqrf_cluster2<32, 2>, 16, 256, st, W, s2, n, R0, d_info, (int64_t)0, 0) == RQR_OK)
                 return RQR_OK;
             (void)cudaGetLastError();
@@ -1042,11 +1040,9 @@ int rqr_chol_dev(const double* G, int n, double shift, const double* d_shift, do
     if (n < 2 || n > RQR_MAX_N) return -2;
     if (!R1) return -4;
     if (G == R1) return -4;
-    static bool attr = false;
-    if (!attr) {
+    RQR_ONCE_PER_DEVICE({
         cudaFuncSetAttribute(k_chol_blocked, cudaFuncAttributeMaxDynamicSharedMemorySize, 144 * 1024);
-        attr = true;
-    }
+    });
     auto smem_of = [](int nn) { const int np = (nn + 7) & ~7; return (size_t)np * (np + 8 + (np & 8)) * sizeof(double); };
     if (n <= 128) {
         k_chol_blocked<<<1, 256, smem_of(n), st>>>(G, n, n, shift, d_shift, R1, n, d_info, 0, Rprev, Rprod,

@@ -21,8 +21,8 @@ __device__ __forceinline__ void row_trsm_inplace(double* __restrict__ x, const d
 // Generic A4: per 64-row tile: load, optional row-wise substitution, optional store of V1, then
 // this CTA's partial Gram (upper triangle) accumulated in its own slice of `part`.
 __global__ void __launch_bounds__(256)
-k_trsm_gram_generic(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
-                    const double* __restrict__ R0, double* __restrict__ V1, int64_t ldq,
+k_trsm_gram_generic(const double* V, int64_t m, int n, int64_t ldv,      // V1 == V allowed: no restrict on either
+                    const double* __restrict__ R0, double* V1, int64_t ldq,
                     double* __restrict__ part)
 {
     extern __shared__ double Xs[];                // GEN_TR x (n+1)
@@ -92,9 +92,9 @@ k_gram_reduce(const double* __restrict__ part, int nparts, int n, double* __rest
 
 // Generic A6: Q = (V R0^-1) R1^-1 row by row; R0 == NULL: Q = V R1^-1.
 __global__ void __launch_bounds__(256)
-k_apply_generic(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
+k_apply_generic(const double* V, int64_t m, int n, int64_t ldv,          // Q == V allowed: no restrict on either
                 const double* __restrict__ R0, const double* __restrict__ R1,
-                double* __restrict__ Q, int64_t ldq)
+                double* Q, int64_t ldq)
 {
     extern __shared__ double Xs[];
     const int ld = n + 1;
@@ -130,18 +130,14 @@ static int generic_grid(int64_t m)
 
 static void generic_attrs()
 {
-    static bool done = false;
-    if (done) return;
-    cudaFuncSetAttribute(k_trsm_gram_generic, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
-    cudaFuncSetAttribute(k_apply_generic, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
-    done = true;
+    RQR_ONCE_PER_DEVICE({
+        cudaFuncSetAttribute(k_trsm_gram_generic, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
+        cudaFuncSetAttribute(k_apply_generic, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
+    });
 }
 
-static int g_force_generic = 0;
-extern "C" void rqr_debug_force_generic(int on) { g_force_generic = on; }
-
-extern "C" int rqr_trsm_gram(const double* V, int64_t m, int n, int64_t ldv, const double* R0,
-                             double* G, double* V1, int64_t ldq, void* work, void* stream)
+static int trsm_gram_impl(const double* V, int64_t m, int n, int64_t ldv, const double* R0,
+                          double* G, double* V1, int64_t ldq, void* work, void* stream, bool force_generic)
 {
     if (!V) return -1;
     if (m < 1 || m >= ((int64_t)1 << 31)) return -2;
@@ -159,7 +155,7 @@ extern "C" int rqr_trsm_gram(const double* V, int64_t m, int n, int64_t ldv, con
     int64_t chunk = RQR_GRAM_CHUNK_ROWS;
     while ((m + chunk - 1) / chunk * 148 > cap) chunk *= 2;
     int rc = RQR_TALL_NOT_HANDLED;
-    if (!g_force_generic) {
+    if (!force_generic) {
         for (int64_t r0 = 0; r0 < m; r0 += chunk) {
             const int64_t mc = (m - r0) < chunk ? (m - r0) : chunk;
             int np = 0;
@@ -186,8 +182,19 @@ extern "C" int rqr_trsm_gram(const double* V, int64_t m, int n, int64_t ldv, con
     return RQR_OK;
 }
 
-extern "C" int rqr_apply(const double* V, int64_t m, int n, int64_t ldv, const double* R0,
-                         const double* R1, double* Q, int64_t ldq, void* work, void* stream)
+extern "C" int rqr_trsm_gram(const double* V, int64_t m, int n, int64_t ldv, const double* R0,
+                             double* G, double* V1, int64_t ldq, void* work, void* stream)
+{
+    return trsm_gram_impl(V, m, n, ldv, R0, G, V1, ldq, work, stream, false);
+}
+extern "C" int rqr_debug_trsm_gram_generic(const double* V, int64_t m, int n, int64_t ldv, const double* R0,
+                                           double* G, double* V1, int64_t ldq, void* work, void* stream)
+{
+    return trsm_gram_impl(V, m, n, ldv, R0, G, V1, ldq, work, stream, true);
+}
+
+static int apply_impl(const double* V, int64_t m, int n, int64_t ldv, const double* R0,
+                      const double* R1, double* Q, int64_t ldq, void* work, void* stream, bool force_generic)
 {
     if (!V) return -1;
     if (m < 1 || m >= ((int64_t)1 << 31)) return -2;
@@ -197,8 +204,8 @@ extern "C" int rqr_apply(const double* V, int64_t m, int n, int64_t ldv, const d
     if (!Q) return -7;
     if (ldq < n) return -8;
     cudaStream_t st = (cudaStream_t)stream;
-    int rc = g_force_generic ? RQR_TALL_NOT_HANDLED : rqr_apply_mma(V, m, n, ldv, R0, R1, Q, ldq, st);
-    if (rc == RQR_TALL_NOT_HANDLED && !g_force_generic && n > 64) {
+    int rc = force_generic ? RQR_TALL_NOT_HANDLED : rqr_apply_mma(V, m, n, ldv, R0, R1, Q, ldq, st);
+    if (rc == RQR_TALL_NOT_HANDLED && !force_generic && n > 64) {
         if (!work) return -9;
         rc = rqr_apply_panel(V, m, n, ldv, R0, R1, Q, ldq,
                              (double*)((char*)work + rqr_layout(1, n, 1).A_frags), st);
@@ -213,4 +220,15 @@ extern "C" int rqr_apply(const double* V, int64_t m, int n, int64_t ldv, const d
         return RQR_OK;
     }
     return rc;
+}
+
+extern "C" int rqr_apply(const double* V, int64_t m, int n, int64_t ldv, const double* R0,
+                         const double* R1, double* Q, int64_t ldq, void* work, void* stream)
+{
+    return apply_impl(V, m, n, ldv, R0, R1, Q, ldq, work, stream, false);
+}
+extern "C" int rqr_debug_apply_generic(const double* V, int64_t m, int n, int64_t ldv, const double* R0,
+                                       const double* R1, double* Q, int64_t ldq, void* work, void* stream)
+{
+    return apply_impl(V, m, n, ldv, R0, R1, Q, ldq, work, stream, true);
 }

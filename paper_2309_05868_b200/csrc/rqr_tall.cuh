@@ -16,5 +16,4 @@ int rqr_trsm_gram_panel(const double* V, int64_t m, int n, int64_t ldv, const do
                         int64_t ldq, double* part, int* nparts, double* frags, int64_t chunk_rows, cudaStream_t st);
 int rqr_apply_panel(const double* V, int64_t m, int n, int64_t ldv, const double* R0, const double* R1,
                     double* Q, int64_t ldq, double* frags, cudaStream_t st);
-// test hook: 0 = auto, 1 = force the generic kernels
-extern "C" void rqr_debug_force_generic(int on);
+

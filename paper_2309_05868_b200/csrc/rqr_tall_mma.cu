@@ -22,7 +22,6 @@
 //     register (lane l holds X[l%4][l/4] of a 4-row slab).
 // The same trsm routine serves rqr_apply, so V1 re-formed there has the same bits (H1).
 #include "rqr_mma.cuh"
-#include <stdlib.h>
 
 // ------------------------------------------------------------------------------------------
 // A4: V1 = V R0^-1 (optional), store V1 (optional), partial Gram per CTA.
@@ -35,8 +34,8 @@ template <int NB> struct GramWarps { static constexpr int value = NB >= 7 ? 8 : 
 
 template <int NB, bool HAS_R, bool FULL>
 __global__ void __launch_bounds__(GramWarps<NB>::value * 32, 1)
-k_trsm_gram_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
-                const double* __restrict__ R0, double* __restrict__ V1, int64_t ldq,
+k_trsm_gram_mma(const double* V, int64_t m, int n, int64_t ldv,          // V1 == V allowed: no restrict on either
+                const double* __restrict__ R0, double* V1, int64_t ldq,
                 double* __restrict__ part)
 {
     using Plan = SmemPlan<NB, GramWarps<NB>::value, GRAM_STAGES, 1, 2>;
@@ -229,8 +228,8 @@ struct PairPlan {
 };
 
 template <int SIDE, bool FULL>
-__device__ __forceinline__ void pair_body(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
-                                          double* __restrict__ V1, int64_t ldq, double* smem, double (&G)[18][2])
+__device__ __forceinline__ void pair_body(const double* V, int64_t m, int n, int64_t ldv,
+                                          double* V1, int64_t ldq, double* smem, double (&G)[18][2])
 {
     constexpr int LDL = PairPlan::LDL;
     const double* Tf = smem;
@@ -300,8 +299,8 @@ __device__ __forceinline__ void pair_body(const double* __restrict__ V, int64_t 
 
 template <bool FULL>
 __global__ void __launch_bounds__(PAIR_WARPS * 32, 1)
-k_trsm_gram_pair(const double* __restrict__ V, int64_t m, int n, int64_t ldv, const double* __restrict__ R0,
-                 double* __restrict__ V1, int64_t ldq, double* __restrict__ part)
+k_trsm_gram_pair(const double* V, int64_t m, int n, int64_t ldv, const double* __restrict__ R0,
+                 double* V1, int64_t ldq, double* __restrict__ part)
 {
     extern __shared__ __align__(16) double smem[];
     double* ring = smem + PairPlan::ring;
@@ -362,9 +361,9 @@ template <int NB, bool TWO> struct ApplyCfg {
 
 template <int NB, bool TWO, bool FULL>
 __global__ void __launch_bounds__(ApplyCfg<NB, TWO>::WARPS * 32, 1)
-k_apply_mma(const double* __restrict__ V, int64_t m, int n, int64_t ldv,
+k_apply_mma(const double* V, int64_t m, int n, int64_t ldv,              // Q == V allowed: no restrict on either
             const double* __restrict__ R0, const double* __restrict__ R1,
-            double* __restrict__ Q, int64_t ldq)
+            double* Q, int64_t ldq)
 {
     using Plan = SmemPlan<NB, ApplyCfg<NB, TWO>::WARPS, ApplyCfg<NB, TWO>::STAGES, 2, 0>;
     constexpr int LDL = Plan::LDL, N8 = Plan::N8;
@@ -457,13 +456,11 @@ static int launch_trsm_gram(const double* V, int64_t m, int n, int64_t ldv, cons
 {
     using Plan = SmemPlan<NB, GramWarps<NB>::value, GRAM_STAGES, 1, 2>;
     static_assert(Plan::bytes <= 227 * 1024, "A4 shared memory plan too large");
-    static bool attr = false;
-    if (!attr) {
+    RQR_ONCE_PER_DEVICE({
         cudaFuncSetAttribute(k_trsm_gram_mma<NB, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
         cudaFuncSetAttribute(k_trsm_gram_mma<NB, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
         cudaFuncSetAttribute(k_trsm_gram_mma<NB, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
-        attr = true;
-    }
+    });
     const int grid = grid_for(m, GramWarps<NB>::value);
     *nparts = grid;
     if (R0 && n == 8 * NB) k_trsm_gram_mma<NB, true, true><<<grid, GramWarps<NB>::value * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, V1, ldq, part);
@@ -473,18 +470,19 @@ static int launch_trsm_gram(const double* V, int64_t m, int n, int64_t ldv, cons
     return RQR_OK;
 }
 
-static int g_a4_pair = -1;       // -1: read RQR_A4_PAIR from the environment once (default on)
+// A/B switch of the 56 < n <= 64 kernel, compile time only (-DRQR_A4_PAIR=0 builds the single-warp kernel in)
+#ifndef RQR_A4_PAIR
+#define RQR_A4_PAIR 1
+#endif
 
 static int launch_trsm_gram_pair(const double* V, int64_t m, int n, int64_t ldv, const double* R0, double* V1,
                                  int64_t ldq, double* part, int* nparts, cudaStream_t st)
 {
     static_assert(PairPlan::bytes <= 227 * 1024, "A4 pair shared memory plan too large");
-    static bool attr = false;
-    if (!attr) {
+    RQR_ONCE_PER_DEVICE({
         cudaFuncSetAttribute(k_trsm_gram_pair<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PairPlan::bytes);
         cudaFuncSetAttribute(k_trsm_gram_pair<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PairPlan::bytes);
-        attr = true;
-    }
+    });
     const int64_t npair_blocks = ((m + 7) / 8 + 1) / 2;
     int64_t g = (npair_blocks + PAIR_WARPS / 2 - 1) / (PAIR_WARPS / 2);
     const int grid = (int)(g < 148 ? (g < 1 ? 1 : g) : 148);
@@ -500,10 +498,6 @@ int rqr_trsm_gram_mma(const double* V, int64_t m, int n, int64_t ldv, const doub
 {
     if (!fast_ok(V, n, ldv, V1, ldq)) return RQR_TALL_NOT_HANDLED;
     if (!R0 && V1) return RQR_TALL_NOT_HANDLED;       // plain copy + Gram: generic kernel
-    if (g_a4_pair < 0) {
-        const char* e = getenv("RQR_A4_PAIR");
-        g_a4_pair = (e && e[0] == '0') ? 0 : 1;
-    }
     if (n <= 16) return launch_trsm_gram<2>(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
     if (n <= 24) return launch_trsm_gram<3>(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
     if (n <= 32) return launch_trsm_gram<4>(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
@@ -512,7 +506,7 @@ int rqr_trsm_gram_mma(const double* V, int64_t m, int n, int64_t ldv, const doub
     // substitution and as many for the Gram), above 48 the 8-block pair kernel
     if (n <= 48) return launch_trsm_gram<6>(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
     if (n <= 56) return launch_trsm_gram<7>(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
-    if (g_a4_pair && R0) return launch_trsm_gram_pair(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
+    if (RQR_A4_PAIR && R0) return launch_trsm_gram_pair(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
     return launch_trsm_gram<8>(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
 }
 
@@ -523,12 +517,10 @@ static int launch_apply_mode(const double* V, int64_t m, int n, int64_t ldv, con
     constexpr int W = ApplyCfg<NB, TWO>::WARPS;
     using Plan = SmemPlan<NB, W, ApplyCfg<NB, TWO>::STAGES, 2, 0>;
     static_assert(Plan::bytes <= 227 * 1024, "A6 shared memory plan too large");
-    static bool attr = false;
-    if (!attr) {
+    RQR_ONCE_PER_DEVICE({
         cudaFuncSetAttribute(k_apply_mma<NB, TWO, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
         cudaFuncSetAttribute(k_apply_mma<NB, TWO, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
-        attr = true;
-    }
+    });
     const int grid = grid_for(m, W);
     if (n == 8 * NB) k_apply_mma<NB, TWO, true><<<grid, W * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, R1, Q, ldq);
     else             k_apply_mma<NB, TWO, false><<<grid, W * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, R1, Q, ldq);

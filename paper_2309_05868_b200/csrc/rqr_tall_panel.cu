@@ -375,12 +375,10 @@ static int launch_panel_w(const double* V, int64_t m, int n, int64_t ldv, const 
 {
     using Plan = PanelPlan<NP>;
     static_assert(Plan::bytes <= 227 * 1024, "k_trsm_panel shared memory plan too large");
-    static bool attr = false;
-    if (!attr) {
+    RQR_ONCE_PER_DEVICE({
         cudaFuncSetAttribute(k_trsm_panel<NP, true, LASTNB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
         cudaFuncSetAttribute(k_trsm_panel<NP, false, LASTNB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
-        attr = true;
-    }
+    });
     const int64_t ntiles = ((m + 7) / 8 + Plan::CW - 1) / Plan::CW;
     const int grid = (int)(ntiles < 148 ? ntiles : 148);
     const int threads = (Plan::CW + 1) * 32;
@@ -417,11 +415,9 @@ static int launch_syrk(const double* X, int64_t m, int n, int64_t ldx, double* p
 {
     using Plan = SyrkPlan<NB>;
     static_assert(Plan::bytes <= 227 * 1024, "k_syrk_fold shared memory plan too large");
-    static bool attr = false;
-    if (!attr) {
+    RQR_ONCE_PER_DEVICE({
         cudaFuncSetAttribute(k_syrk_fold<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
-        attr = true;
-    }
+    });
     constexpr int PARTS = (NB / 2 + PANEL_WARPS - 1) / PANEL_WARPS;
     const int64_t ntiles = (m + SYRK_TR - 1) / SYRK_TR;
     int walkers = 148 / PARTS;

@@ -26,11 +26,25 @@ S2_RADEMACHER = 16      # same value as RQR_S2_RADEMACHER in include/rqr.h
 
 
 def rand_cholqr_sharded(ops, V_local, row0, s1, s2, seed, Q_local, R, bufs, group=None, flags=0,
-                        variant=0):
+                        variant=0, m_total=None, fused=True):
     """One factorization step on this rank's block rows.  bufs: dict with W1 (s1 x n), W (s2 x n),
     R0, R1, G (n x n), work, info.  All ranks end with the same R; Q_local holds this rank's rows.
     variant | S2_RADEMACHER: the replicated S2 is the on-the-fly Rademacher sketch (N4): no rank stores it
-    (bufs must come from alloc_bufs with the same variant)."""
+    (bufs must come from alloc_bufs with the same variant).
+
+    With the CUDA binding (`ops.rand_cholqr_sharded` exists) and fused=True this is ONE library call,
+    rqr_rand_cholqr_sharded, with the two all-reduces issued from inside it through a callback on the same stream
+    (CUDA-graph capturable); m_total (all ranks' rows) is then required unless there is one rank.  Otherwise the
+    step entry points are called one by one (the CPU tests' adapter; fused=False on CUDA)."""
+    multi = dist.is_initialized() and dist.get_world_size(group) > 1
+    if fused and hasattr(ops, "rand_cholqr_sharded"):
+        if m_total is None:
+            assert not multi, "m_total is required with more than one rank"
+            m_total = row0 + V_local.shape[0]
+        ar = (lambda t: dist.all_reduce(t, op=dist.ReduceOp.SUM, group=group)) if multi else None
+        ops.rand_cholqr_sharded(V_local, row0, m_total, s1, s2, seed, Q_local, R, bufs["work"], bufs["info"],
+                                variant, flags, ar)
+        return
     rad = variant & S2_RADEMACHER
     ops.countsketch(V_local, s1, seed, bufs["W1"], bufs["work"], variant, flags, row0)
     ops.gauss_sketch(bufs["W1"], s2, seed, bufs["W"], bufs["work"], flags | rad)

@@ -17,7 +17,7 @@ import sys
 
 import torch
 
-from . import binding as rq, flops, inputs
+from . import bench_probe as probe, binding as rq, flops, inputs
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 KAPPA = 1e12
@@ -40,9 +40,9 @@ def _time(fn, reps):
 def _fp64_peak():
     sink = torch.empty(148 * 8 * 256, dtype=torch.float64, device="cuda")
     best = 0.0
-    for kind in (rq.PROBE_DFMA, rq.PROBE_DMMA):
-        fl = rq.probe_fp64(kind, 20000, 148 * 8, sink)
-        ms = _time(lambda: rq.probe_fp64(kind, 20000, 148 * 8, sink), 5)
+    for kind in (probe.DFMA, probe.DMMA):
+        fl = probe.probe_fp64(kind, 20000, 148 * 8, sink)
+        ms = _time(lambda: probe.probe_fp64(kind, 20000, 148 * 8, sink), 5)
         best = max(best, fl / (ms * 1e-3) / 1e12)
     return best
 

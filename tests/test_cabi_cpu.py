@@ -68,7 +68,6 @@ def test_argument_validation_without_gpu(lib):
     assert lib.rqr_rand_cholqr(one, 4, 8, 4, 8, 1, one, one, one, z, 0, 0, z) == -3        # n > m
     assert lib.rqr_cholqr2(z, 100, 8, one, one, one, z, z) == -1
     assert lib.rqr_sketch_prepare(100, 8, 0, 64, 600, 1, 0, one, z) == -5
-    assert lib.rqr_probe_fp64(5, 1, 1, one, z, z) == -1
     # batched / strided one-shot and the Rademacher test hook
     assert lib.rqr_rand_cholqr_batched(one, 100, 8, 0, 800, 64, 16, 1, one, 800, one, one, z, 0, 1, z) == -4     # batch < 1
     assert lib.rqr_rand_cholqr_batched(one, 100, 8, 2, 799, 64, 16, 1, one, 800, one, one, z, 0, 1, z) == -5     # stride < m n

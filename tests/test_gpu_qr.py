@@ -66,7 +66,8 @@ def test_rand_cholqr_matches_oracle(rq, orc, name, m, n, kappa):
     Vd = V.cuda()
     Qo, Ro, io = orc.rand_cholqr(V.numpy(), s1, s2, 42)
     assert io == 0
-    for variant, flags, prepared in [(0, 0, False), (0, rq.FLAG_RECOMPUTE_V1, True), (1, 0, True)]:
+    for variant, flags, prepared in [(0, 0, False), (0, rq.FLAG_RECOMPUTE_V1, True), (0, rq.FLAG_STORE_V1, True),
+                                     (1, 0, True)]:
         Q, R, info = run_rand(rq, Vd, s1, s2, 42, variant, flags, prepared)
         assert info == 0
         assert orth_err(Q) <= ORTH_TOL
@@ -156,6 +157,96 @@ def test_comparators_match_oracle(rq, orc):
     assert int(info.item()) == 0 and io == 0
     assert np.linalg.norm(R.cpu().numpy() - Ro) <= R_TOL * np.linalg.norm(Ro)
     assert orth_err(Q) <= ORTH_TOL and resid(Vd, Q, R) <= RES_TOL
+
+
+def test_scholqr3_shift_equals_the_oracles(rq, orc):
+    """Reading S9 (the reference cites sCholQR3 and does not write it): neither side can be pinned
+    to the paper, so the recorded reading is pinned ACROSS the two sides: the library's shift
+    11 (mn + n(n+1)) 2^-53 tr(V^T V) must equal the oracle's to rounding of the trace (a shift 10x off on either
+    side fails here)."""
+    m, n = 30000, 24
+    V = inputs.make_V(m, n, 1e5, 9)
+    Vd = V.cuda()
+    work = rq.alloc_workspace(m, n, 2 * n * n, 2 * n)
+    info = rq.new_info()
+    Q = torch.empty_like(Vd)
+    R = torch.empty(n, n, dtype=torch.float64, device="cuda")
+    rq.scholqr3(Vd, Q, R, work, info)
+    shift = float(rq.workspace_scholqr3_shift(work).item())
+    _, _, io, shift_o = orc.scholqr3(V.numpy())
+    assert int(info.item()) == 0 and io == 0 and shift_o > 0
+    assert abs(shift - shift_o) <= 1e-13 * shift_o          # the traces are sums of n terms in different orders
+    tr = float(torch.sum(Vd * Vd))
+    assert abs(shift - 11.0 * (m * n + n * (n + 1)) * 2.0 ** -53 * tr) <= 1e-12 * shift
+
+
+@pytest.mark.parametrize("n", [16, 32, 40, 48, 64])
+def test_v1_modes_give_bit_identical_factors(rq, n):
+    """DESIGN.md reading S20 / hazard H1: V1 stored (A4 writes it, A6 in place) and V1 recomputed (A6 re-forms it with
+    the same instruction sequence) must give the same bits; the default picks one of them per n."""
+    m = 70001
+    s1, s2 = inputs.sketch_sizes(n)
+    Vd = inputs.make_V(m, n, 1e12, 3).cuda()
+    outs = []
+    for flags in (0, rq.FLAG_STORE_V1, rq.FLAG_RECOMPUTE_V1):
+        Q, R, info = run_rand(rq, Vd, s1, s2, 42, 0, flags)
+        assert info == 0 and orth_err(Q) <= ORTH_TOL
+        outs.append((Q, R))
+    for Q, R in outs[1:]:
+        assert torch.equal(Q, outs[0][0]) and torch.equal(R, outs[0][1])
+    # CholeskyQR2 on the same kernels takes the same decision and must meet its bars at low kappa
+    Vl = inputs.make_V(m, n, 1e4, 3).cuda()
+    work = rq.alloc_workspace(m, n, s1, s2)
+    info = rq.new_info()
+    Q = torch.empty_like(Vl); R = torch.empty(n, n, dtype=torch.float64, device="cuda")
+    rq.cholqr2(Vl, Q, R, work, info)
+    assert int(info.item()) == 0 and orth_err(Q) <= ORTH_TOL and resid(Vl, Q, R) <= RES_TOL
+
+
+def test_recompute_falls_back_to_stored_when_Q_is_misaligned(rq):
+    """A4 without a V1 buffer dispatches on V alone, A6 on V and Q: with V 16-byte aligned and Q not, a recomputed V1
+    would come from another kernel family (other rounding) and orthogonality would drop to u kappa(V).  The driver
+    must store V1 then, whatever the flag says."""
+    m, n = 40000, 32
+    s1, s2 = inputs.sketch_sizes(n)
+    Vd = inputs.make_V(m, n, 1e13, 4).cuda()
+    buf = torch.empty(m * n + 1, dtype=torch.float64, device="cuda")
+    Q = buf[1:].view(m, n)                                    # 8 bytes off a 16-byte boundary
+    assert Q.data_ptr() % 16 == 8 and Vd.data_ptr() % 16 == 0
+    R = torch.empty(n, n, dtype=torch.float64, device="cuda")
+    work = rq.alloc_workspace(m, n, s1, s2)
+    info = rq.new_info()
+    rq.rand_cholqr(Vd, s1, s2, 42, Q, R, work, info, 0, rq.FLAG_RECOMPUTE_V1)
+    assert int(info.item()) == 0 and orth_err(Q) <= ORTH_TOL and resid(Vd, Q, R) <= RES_TOL
+
+
+@pytest.mark.parametrize("scale", [1e-100, 1e100])
+def test_scaled_inputs_inside_the_documented_range(rq, scale):
+    """include/rqr.h "Dynamic range": |V| within [1e-140, 1e140] must factor like the unscaled matrix."""
+    m, n = 40000, 64
+    s1, s2 = inputs.sketch_sizes(n)
+    Vd = inputs.make_V(m, n, 1e8, 6).cuda() * scale
+    Q, R, info = run_rand(rq, Vd, s1, s2, 42)
+    assert info == 0 and orth_err(Q) <= ORTH_TOL and resid(Vd, Q, R) <= RES_TOL
+    check_R(R)
+
+
+def test_first_call_on_a_second_device(rq):
+    """The > 48 KB shared-memory opt-in is per device: a process whose first call on device 1 comes
+    after calls on device 0 must still launch the DMMA kernels there."""
+    if torch.cuda.device_count() < 2:
+        pytest.skip("one visible device")
+    m, n = 50000, 64
+    s1, s2 = inputs.sketch_sizes(n)
+    V = inputs.make_V(m, n, 1e8, 6)
+    run_rand(rq, V.cuda(), s1, s2, 42)
+    with torch.cuda.device(1):
+        Vd = V.to("cuda:1")
+        Q = torch.empty_like(Vd); R = torch.empty(n, n, dtype=torch.float64, device="cuda:1")
+        work = rq.alloc_workspace(m, n, s1, s2, device="cuda:1")
+        info = rq.new_info("cuda:1")
+        rq.rand_cholqr(Vd, s1, s2, 42, Q, R, work, info)
+        assert int(info.item()) == 0 and orth_err(Q) <= ORTH_TOL
 
 
 def test_stress_inputs(rq):
@@ -277,7 +368,7 @@ def test_eps_sweep_sketch_sizes_match_oracle(rq, orc, m, n):
         check(Ro, io)
 
 
-@pytest.mark.parametrize("m,n", [(100000, 70), (100000, 30), (60000, 100)])
+@pytest.mark.parametrize("m,n", [(100000, 70), (100000, 30), (100000, 100)])
 def test_paper_grid_shape_and_sketch_sizes(rq, orc, m, n):
     """the paper's own shapes with its "Multi (0.9, 0.49)" sketch sizes
     s1 = ceil(8.24 (n^2 + n)), s2 = ceil(74.3 log s1): non-power-of-two s1 (general bucket map),

@@ -54,6 +54,25 @@ def test_prepared_S2_matches_oracle(rq, orc):
     assert np.all(np.abs(S2 - S2o) <= 1e-15 * np.maximum(np.abs(S2o), 1.0 / np.sqrt(s2)))
 
 
+@pytest.mark.parametrize("m,s1,row0", [(100000, 8192, 0), (70001, 9940, 12345), (300000, 200, 0), (5000, 131072, 7),
+                                       (1 << 21, 2048, 1 << 33)])
+def test_sorted_row_list_is_the_stable_sort(rq, orc, m, s1, row0):
+    """A0: the row list rqr_sketch_prepare writes must be, bit for bit, the STABLE sort of the rows by the oracle's
+    bucket (ascending row inside a bucket) with the oracle's sign in bit 31, and the offsets the bucket histogram's
+    exclusive scan ("sorted row list: bit-exact")."""
+    n = 16
+    s2 = 32
+    work = rq.alloc_workspace(m, n, s1, s2)
+    rq.sketch_prepare(m, n, s1, s2, 42, work, 0, row0)
+    off, ent = rq.workspace_rows(work, m, n, s1)
+    off = host(off).view(np.uint32); ent = host(ent).view(np.uint32)
+    bo, so = orc.hash_sign(42, row0, m, s1)
+    order = np.argsort(bo, kind="stable").astype(np.uint32)
+    expect = order | ((so[order] < 0).astype(np.uint32) << np.uint32(31))
+    assert np.array_equal(ent, expect)
+    assert np.array_equal(off, np.concatenate([[0], np.cumsum(np.bincount(bo, minlength=s1))]).astype(np.uint32))
+
+
 @pytest.mark.parametrize("m,n,s1", [(20000, 16, 512), (100000, 70, 9940), (65536, 64, 8192),
                                     (5000, 33, 64), (3000, 256, 4000), (37, 8, 16), (8192, 2, 8),
                                     # few buckets: every bucket's row list is split over several CTAs (two-stage sum)
@@ -272,6 +291,7 @@ def test_triu_mul_parity(rq, orc, n):
 
 
 @pytest.mark.parametrize("rows,n", [(8192, 64), (2048, 32), (5000, 64), (129, 64), (128, 64), (1000, 16), (34277, 64),
+                                    (103552, 64),      # = the largest row count the TSQR scratch takes at n = 64 (cap 1216)
                                     (77, 8)])
 def test_tsqr_r_matches_householder(rq, orc, rows, n):
     """TSQR tree of 128-row Householder blocks vs the oracle's plain Householder QR of the whole matrix: R with a
