@@ -62,6 +62,14 @@ extern "C" {
 #define RQR_VARIANT_SCATTER 1 /* stream V, hash on the fly, red.global.add.f64; the last
                                  bits depend on the order of the atomics                    */
 
+#define RQR_VARIANT_STREAM 2  /* stream V in row order through shared memory (bulk async copies), hash on
+                                 the fly, flip the sign in shared memory, and add every row to its bucket with
+                                 ONE bulk reduction (cp.reduce.async.bulk ... add.f64, SASS UBLKRED) instead of n
+                                 atomics: no stored S1 at all ("storage of only O(n) values"; :947
+                                 "adding/subtracting subsets of rows"), nothing to prepare in A0; the order of
+                                 the reductions is not fixed.  Needs even n and ld and 16-byte aligned bases
+                                 (else it runs as RQR_VARIANT_SCATTER).                                  */
+
 /* flags */
 #define RQR_FLAG_PREPARED 1   /* `work` already holds the sketch state written by
                                  rqr_sketch_prepare with the same (m, n, row0, s1, s2,
@@ -73,9 +81,10 @@ extern "C" {
                                  traffic instead of 40mn, 4mn^2 flops instead of 3mn^2).
                                  Honoured for n <= 64; for n > 64 V1 is always stored.       */
 #define RQR_FLAG_STORE_V1 4   /* one-shot drivers: store V1 into Q in A4 and transform it in place in A6.
-                                 With neither flag the drivers choose per n: recomputed for n <= 40 (the
+                                 With neither flag the drivers choose per n: recomputed for n <= 16 (the
                                  path is HBM-bound there and moves 32mn instead of 40mn bytes), stored above
-                                 (A4 / A6 are FP64-bound and the extra mn^2 flops would not hide).  When V and
+                                 (measured: from n = 24 up A4 is bound by the FP64 tensor pipe with or without
+                                 the store, and the extra mn^2 flops of A6 do not hide).  When V and
                                  Q would not take the same kernel family (Q not 16-byte aligned while V is,
                                  even n) V1 is stored whatever the flags say: a V1 re-formed by different
                                  arithmetic would break the orthogonality of Q (DESIGN.md hazard H1).      */
@@ -103,9 +112,9 @@ int rqr_sketch_prepare(int64_t m, int n, int64_t row0, int64_t s1, int s2, uint6
 
 /* A1 -- CountSketch, Alg. 1 step 1 first half: W1 = S1 V,
  * W1[h(i),:] += sigma(i) V[i,:], S1 unscaled.  W1 (s1 x n) is overwritten.
- * RQR_VARIANT_SORTED with few buckets (2 s1 <= 1184): the bucket row lists are split over several
- * CTAs and the partial sketches pass through the Gram-partial scratch of `work` (contents lost),
- * summed in a fixed order: the result stays bit-reproducible.                                 */
+ * RQR_VARIANT_SORTED: when s1 buckets do not fill the rounds of the 1184 resident CTAs to 95% (s1 < 1184,
+ * s1 = 2048, ...), the bucket row lists are split into segments and the partial sketches pass through the
+ * Gram-partial scratch of `work` (contents lost), summed in a fixed order: the result stays bit-reproducible. */
 int rqr_countsketch(const double* V, int64_t m, int n, int64_t ldv, int64_t row0, int64_t s1,
                     uint64_t seed, double* W1, void* work, int variant, int flags, void* stream);
 
@@ -198,6 +207,10 @@ int rqr_tsqr_r(const double* A, int64_t rows, int n, double* R, void* work, int*
 int rqr_dense_gauss_sketch(const double* V, int64_t m, int n, int64_t ldv, int64_t row0,
                            int64_t m_total, int s, uint64_t seed, double* W, void* work,
                            void* stream);
+
+/* Measurement hook: only the draw of the s x m Gaussians of rqr_dense_gauss_sketch (same launch shape, no V traffic,
+ * no products): the generation bound of the single-Gaussian-sketch comparator.  n even.                          */
+int rqr_debug_dense_gauss_draw_only(int64_t m, int n, int s, uint64_t seed, void* work, void* stream);
 
 /* Inspection helpers for parity tests (device outputs): bucket (uint32) and sign (int8, +-1)
  * of rows [row0, row0+count); Gaussian stream entries z(first .. first+count-1).            */

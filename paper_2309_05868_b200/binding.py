@@ -19,6 +19,7 @@ INFO_NOT_SPD = 1000
 INFO_SINGULAR = 2000
 VARIANT_SORTED = 0
 VARIANT_SCATTER = 1
+VARIANT_STREAM = 2
 FLAG_PREPARED = 1
 FLAG_RECOMPUTE_V1 = 2
 FLAG_STORE_V1 = 4
@@ -51,6 +52,7 @@ SIGNATURES = {
     "rqr_count_randcholqr": (_int, [_vp, _i64, _int, _i64, _u64, _vp, _vp, _vp, _vp, _int, _int, _vp]),
     "rqr_tsqr_r": (_int, [_vp, _i64, _int, _vp, _vp, _vp, _vp]),
     "rqr_dense_gauss_sketch": (_int, [_vp, _i64, _int, _i64, _i64, _i64, _int, _u64, _vp, _vp, _vp]),
+    "rqr_debug_dense_gauss_draw_only": (_int, [_i64, _int, _int, _u64, _vp, _vp]),
     "rqr_debug_hash_sign": (_int, [_u64, _i64, _i64, _i64, _vp, _vp, _vp]),
     "rqr_debug_gauss": (_int, [_u64, _u32, _u64, _i64, _vp, _vp]),
     "rqr_workspace_S2": (_vp, [_vp, _int, _i64]),
@@ -257,6 +259,10 @@ def dense_gauss_sketch(V, s, seed, W, work, row0=0, m_total=None):
     m, n = V.shape
     _chk(lib().rqr_dense_gauss_sketch(_ptr(_f64(V, "V")), m, n, V.stride(0), row0, m if m_total is None else m_total,
                                       s, seed, _ptr(W), _ptr(work), _stream()), "rqr_dense_gauss_sketch")
+
+
+def debug_dense_gauss_draw_only(m, n, s, seed, work):
+    _chk(lib().rqr_debug_dense_gauss_draw_only(m, n, s, seed, _ptr(work), _stream()), "rqr_debug_dense_gauss_draw_only")
 
 
 def debug_hash_sign(seed, row0, count, s1, device="cuda"):

@@ -46,11 +46,14 @@ static int check_common(const double* V, int64_t m, int n, double* Q, double* R,
 
 // V1 = V R0^-1 stored or recomputed (PAPER.md:220-222 flop terms; reading S20).  Stored: A4 writes V1
 // into Q and A6 transforms it in place: 40mn bytes, 3mn^2 flops.  Recomputed: A4 stores nothing and A6 re-forms V1
-// with the bit-identical routine: 32mn bytes, 4mn^2 flops.  The path is HBM-bound for n <= 32 (n/8 flop/B in A6
-// against a ridge of 5.7) and FP64-bound from n = 48 up, so the default is "recompute iff n <= RQR_AUTO_RECOMPUTE_MAX_N"
-// (measured: profiles/r2_v1_mode.md); RQR_FLAG_RECOMPUTE_V1 / RQR_FLAG_STORE_V1 override it.  Every driver
-// (CholeskyQR2 and sCholQR3 included) takes the same decision: the comparison stays on the same kernels.
-#define RQR_AUTO_RECOMPUTE_MAX_N 40
+// with the bit-identical routine: 32mn bytes, 4mn^2 flops.  Measured (profiles/r2_v1_mode.md): with 8 x 8 tiles A4
+// executes NB (NB + 1) DMMA per 8 rows for the substitution and as many for the Gram, so it is already bound by the
+// FP64 tensor pipe at n = 32 (0.36 ms at 2^22 x 32 with or without the store: the 8mn-byte write hides under it),
+// and the second substitution in A6 is not free from n = 24 up.  Recomputing wins only for n <= 16 (2^22 x 16: 0.542
+// vs 0.569 ms), ties at n = 24 and loses above (n = 32: 0.994 vs 0.972; n = 40: 1.43 vs 1.31; n = 64: 2.82 vs 2.41).
+// Default: "recompute iff n <= RQR_AUTO_RECOMPUTE_MAX_N"; RQR_FLAG_RECOMPUTE_V1 / RQR_FLAG_STORE_V1 override it.
+// Every driver (CholeskyQR2 and sCholQR3 included) takes the same decision: the comparison stays on the same kernels.
+#define RQR_AUTO_RECOMPUTE_MAX_N 16
 static bool use_recompute(const double* V, int n, const double* R0, const double* Q, int flags)
 {
     if (!R0 || n > 64) return false;      // n > 64: A4 is FP64-bound either way and V1 is always stored
@@ -93,8 +96,10 @@ static int rand_cholqr_impl(const double* V, int64_t m, int64_t row0, int64_t m_
     if (s1 < 1 || s1 >= ((int64_t)1 << 31) || s1 > m_total) return -4;
     if (s2 < n || s2 > s1 || s2 > RQR_MAX_S2) return -5;      // eq. (20)
     const int rad = variant & RQR_S2_RADEMACHER;                 // N4: Count-Rademacher multisketch
-    if ((variant & ~RQR_S2_RADEMACHER) != RQR_VARIANT_SORTED && (variant & ~RQR_S2_RADEMACHER) != RQR_VARIANT_SCATTER)
-        return -11;
+    {
+        const int cs = variant & ~RQR_S2_RADEMACHER;
+        if (cs != RQR_VARIANT_SORTED && cs != RQR_VARIANT_SCATTER && cs != RQR_VARIANT_STREAM) return -11;
+    }
     cudaStream_t st = (cudaStream_t)stream;
     RqrLayout L = rqr_layout(m, n, s1, rad != 0);
     double* R0 = small_mat(work, L, n, RQR_SM_R0);
@@ -211,7 +216,7 @@ extern "C" int rqr_count_randcholqr(const double* V, int64_t m, int n, int64_t s
     // n <= 64: tree of 128-row register-resident blocks; n > 64: blocks of 1024 / 512 rows in the cluster kernel
     const int64_t max_rows = n <= 64 ? tsqr_max_rows(n) : (int64_t)(n <= 128 ? 1024 : 512) * rqr_gram_partial_cap(n);
     if (s1 < n || s1 >= ((int64_t)1 << 31) || s1 > m || s1 > max_rows) return -4;
-    if (variant != RQR_VARIANT_SORTED && variant != RQR_VARIANT_SCATTER) return -10;
+    if (variant != RQR_VARIANT_SORTED && variant != RQR_VARIANT_SCATTER && variant != RQR_VARIANT_STREAM) return -10;
     cudaStream_t st = (cudaStream_t)stream;
     RqrLayout L = rqr_layout(m, n, s1);
     double* R0 = small_mat(work, L, n, RQR_SM_R0);

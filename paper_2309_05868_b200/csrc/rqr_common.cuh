@@ -6,6 +6,7 @@
 #include <stddef.h>
 #include <atomic>
 #include "../../include/rqr.h"
+#include "rqr_gauss.cuh"
 
 #define RQR_MAX_N 256
 #define RQR_MAX_S2 1024
@@ -61,6 +62,20 @@ static inline int rqr_gram_partial_cap(int n)
 // row is 128-byte aligned for the bulk copies of the DMMA GEMM whatever s1 is (paper grid: odd s1)
 __host__ __device__ static inline int64_t rqr_s2_ld(int64_t s1) { return (s1 + 15) & ~(int64_t)15; }
 
+// A0 radix sort (rqr_sketch.cu): rows per tile and words of its digit-count scratch ((bins + 1) x tiles + bins)
+#define RQR_SORT_MAX_BINS 512
+static inline int64_t rqr_sort_tile_rows(int64_t m)
+{
+    int64_t t = 2048;
+    while (t < 16384 && t * 512 < m) t *= 2;
+    return t;
+}
+static inline size_t rqr_sort_hist_words(int64_t m)
+{
+    const int64_t T = rqr_sort_tile_rows(m), C = (m + T - 1) / T;
+    return (size_t)RQR_SORT_MAX_BINS * (size_t)C + RQR_SORT_MAX_BINS;
+}
+
 // ---------------------------------------------------------------------------------------
 // Workspace layout.  Offsets of a region depend only on
 // arguments every user of that region has.
@@ -73,9 +88,10 @@ __host__ __device__ static inline int64_t rqr_s2_ld(int64_t s1) { return (s1 + 1
 //   E  sorted rows     f(m)      m u32 (row | sign<<31)
 //   W  one-shot W      (s2max x n), in the n-only part (before B)
 //   F  one-shot W1     (s1 x n)
+//   G  A0 sort scratch f(m)      m u32 (second row list of the radix sort) + per-tile digit counts
 // ---------------------------------------------------------------------------------------
 struct RqrLayout {
-    size_t hdr, A, A_small, A_frags, B_off, B_cur, C, D, E, F_W1, F_W, total;
+    size_t hdr, A, A_small, A_frags, B_off, B_cur, C, D, E, F_W1, F_W, G_sort, total;
 };
 
 // no_S2: the Rademacher S2 of N4 is generated on the fly, region C is empty
@@ -96,7 +112,10 @@ static inline RqrLayout rqr_layout(int64_t m, int n, int64_t s1, bool no_S2 = fa
     L.D = L.C + (no_S2 ? 0 : rqr_align256((size_t)RQR_MAX_S2 * (size_t)rqr_s2_ld(s1) * sizeof(double)));
     L.E = L.D + rqr_align256((size_t)RQR_GAUSS_PARTIAL_ROWS * n * sizeof(double));
     L.F_W1 = L.E + rqr_align256((size_t)m * 4);
-    L.total = L.F_W1 + rqr_align256((size_t)s1 * n * sizeof(double));
+    // G: scratch of the A0 radix sort (rqr_sketch_prepare only): the second row list of the ping-pong and the
+    // per-tile digit counts
+    L.G_sort = L.F_W1 + rqr_align256((size_t)s1 * n * sizeof(double));
+    L.total = L.G_sort + rqr_align256((size_t)m * 4) + rqr_align256(rqr_sort_hist_words(m) * 4);
     return L;
 }
 
@@ -114,16 +133,7 @@ __host__ __device__ __forceinline__ void rqr_philox(uint64_t seed, uint64_t idx,
     uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
-#ifdef __CUDA_ARCH__
-        uint32_t h0 = __umulhi(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;
-        uint32_t h1 = __umulhi(0xCD9E8D57u, c2), l1 = 0xCD9E8D57u * c2;
-#else
-        uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
-        uint32_t h0 = (uint32_t)(p0 >> 32), l0 = (uint32_t)p0;
-        uint32_t h1 = (uint32_t)(p1 >> 32), l1 = (uint32_t)p1;
-#endif
-        uint32_t n0 = h1 ^ c1 ^ k0, n2 = h0 ^ c3 ^ k1;
-        c0 = n0; c1 = l1; c2 = n2; c3 = l0;
+        rqr_philox_round(c0, c1, c2, c3, k0, k1);       // rqr_gauss.cuh
         k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
     }
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
@@ -145,21 +155,16 @@ __device__ __forceinline__ void rqr_hash_sign(uint64_t seed, uint64_t i, uint32_
     neg = o[1] & 1u;
 }
 
-// Box-Muller pair q of a stream (reading S3): returns z_even, z_odd (standard normal).
+// Box-Muller pair q of a stream (reading S3): returns z_even, z_odd (standard normal).  Branch-free staged routine
+// of rqr_gauss.cuh; `tab` = its logarithm table (the copy in global memory, or a shared-memory copy in hot loops).
 __device__ __forceinline__ void rqr_gauss_pair(uint64_t seed, uint64_t q, uint32_t stream,
-                                               double& z0, double& z1)
+                                               double& z0, double& z1, const RqrLogEntry* tab = d_rqr_log_tab)
 {
-    uint32_t o[4];
-    rqr_philox(seed, q, stream, o);
-    uint64_t x1 = (((uint64_t)o[0] << 32) | o[1]) >> 12;
-    uint64_t x2 = (((uint64_t)o[2] << 32) | o[3]) >> 12;
-    double u1 = (double)(2 * x1 + 1) * 0x1p-53;      // exact: 2x+1 < 2^53
-    double u2 = (double)(2 * x2 + 1) * 0x1p-53;
-    double rho = sqrt(-2.0 * log(u1));
-    double s, c;
-    sincospi(2.0 * u2, &s, &c);
-    z0 = rho * c;
-    z1 = rho * s;
+    RqrPairDraw d;
+    d.begin(seed, q, stream);
+    rqr_pair_draw_run<0>(d, tab);
+    z0 = d.z0;
+    z1 = d.z1;
 }
 
 __device__ __forceinline__ double rqr_gauss_entry(uint64_t seed, uint64_t e, uint32_t stream)

@@ -3,7 +3,10 @@
 // for the kernel designs.  sm_100a.
 #include "rqr_common.cuh"
 #include "rqr_tall.cuh"
+#include "rqr_mma.cuh"
 
+int rqr_dense_gauss_mma(const double* V, int64_t m, int n, int64_t ldv, int64_t row0, int64_t m_total, int s,
+                        uint64_t seed, double* part, int64_t Pcap, int* P_out, bool draw_only, cudaStream_t st);
 int rqr_gauss_gemm_mma(const double* S2, const double* W1, int64_t s1, int n, int s2, double* part,
                        int64_t ks_cap, int* ks_out, cudaStream_t st, uint64_t seed);
 
@@ -26,29 +29,61 @@ __global__ void k_gen_S2(uint64_t seed, int s2, int64_t s1, int64_t ld, int64_t 
     }
 }
 
-__global__ void k_bucket_hist(uint64_t seed, int64_t row0, int64_t m, uint32_t s1,
-                              uint32_t* __restrict__ hist)
+// -----------------------------------------------------------------------------------------------------------------
+// Bucket-sorted row list = STABLE sort of the rows by bucket, as an LSD radix sort on the bucket id with digits of
+// `bits` <= 9 bits.  A pass is three launches -- digit counts per tile of T consecutive positions, an exclusive scan of
+// the counts of every digit over the tiles, a stable scatter -- and every step has a fixed order, so the list is the same
+// bits run to run (W1 is then bit-reproducible) and equals numpy's stable argsort of the oracle's buckets
+// (tests/test_gpu_steps.py::test_sorted_row_list_is_the_stable_sort).  The bucket of an entry is recomputed from its
+// row index (Philox) in every pass: the only arrays are the two m-word row lists of the ping-pong.
+// Replaces round 1's histogram / cursor fill with global atomics + a bitonic sort per bucket (0.88 ms at 2^23 rows).
+// -----------------------------------------------------------------------------------------------------------------
+#define SORT_THREADS 512
+#define SORT_WARPS (SORT_THREADS / 32)
+
+// entry (row | sign << 31) at position pos of the pass input (in == NULL: the identity list) and its digit
+__device__ __forceinline__ void sort_load(const uint32_t* __restrict__ in, int64_t pos, uint64_t seed, int64_t row0,
+                                          uint32_t s1, int shift, uint32_t mask, uint32_t& entry, uint32_t& digit)
 {
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < m;
-         i += (int64_t)gridDim.x * blockDim.x) {
-        uint32_t b, neg;
-        rqr_hash_sign(seed, (uint64_t)(row0 + i), s1, b, neg);
-        atomicAdd(&hist[b], 1u);
-    }
+    uint32_t row = in ? (in[pos] & 0x7fffffffu) : (uint32_t)pos;
+    uint32_t b, neg;
+    rqr_hash_sign(seed, (uint64_t)(row0 + row), s1, b, neg);
+    entry = in ? in[pos] : (row | (neg << 31));
+    digit = (b >> shift) & mask;
 }
 
-// single CTA: exclusive scan of hist[0..s1) -> off[0..s1]; cursor[b] = off[b]
-__global__ void k_bucket_scan(const uint32_t* hist, uint32_t s1, uint32_t* __restrict__ off,
-                              uint32_t* cursor)   // hist may alias cursor
+// counts[d * C + tile] = number of positions of the tile whose digit is d
+__global__ void __launch_bounds__(SORT_THREADS)
+k_sort_count(uint64_t seed, int64_t row0, int64_t m, uint32_t s1, const uint32_t* __restrict__ in, int shift, int bits,
+             int T, int C, uint32_t* __restrict__ counts)
+{
+    __shared__ uint32_t h[RQR_SORT_MAX_BINS];
+    const int bins = 1 << bits;
+    for (int d = threadIdx.x; d < bins; d += SORT_THREADS) h[d] = 0;
+    __syncthreads();
+    const int64_t base = (int64_t)blockIdx.x * T;
+    for (int i = threadIdx.x; i < T && base + i < m; i += SORT_THREADS) {
+        uint32_t e, d;
+        sort_load(in, base + i, seed, row0, s1, shift, (uint32_t)bins - 1, e, d);
+        atomicAdd(&h[d], 1u);
+    }
+    __syncthreads();
+    for (int d = threadIdx.x; d < bins; d += SORT_THREADS) counts[(size_t)d * C + blockIdx.x] = h[d];
+}
+
+// one CTA per digit: exclusive scan of counts[d][0..C) in place, total[d] = the digit's count
+__global__ void __launch_bounds__(1024)
+k_sort_scan_tiles(uint32_t* __restrict__ counts, int C, uint32_t* __restrict__ total)
 {
     __shared__ uint32_t warp_tot[32];
     __shared__ uint32_t carry;
+    uint32_t* c = counts + (size_t)blockIdx.x * C;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     if (tid == 0) carry = 0;
     __syncthreads();
-    for (uint32_t base = 0; base < s1; base += blockDim.x) {
-        uint32_t idx = base + tid;
-        uint32_t v = idx < s1 ? hist[idx] : 0u;
+    for (int base = 0; base < C; base += 1024) {
+        const int idx = base + tid;
+        const uint32_t v = idx < C ? c[idx] : 0u;
         uint32_t x = v;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
@@ -58,80 +93,110 @@ __global__ void k_bucket_scan(const uint32_t* hist, uint32_t s1, uint32_t* __res
         if (lane == 31) warp_tot[wid] = x;
         __syncthreads();
         if (wid == 0) {
-            uint32_t t = lane < (int)(blockDim.x >> 5) ? warp_tot[lane] : 0u;
+            uint32_t t = warp_tot[lane];
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
                 uint32_t y = __shfl_up_sync(0xffffffffu, t, o);
                 if (lane >= o) t += y;
             }
-            warp_tot[lane] = t;   // inclusive scan of warp totals
+            warp_tot[lane] = t;
         }
         __syncthreads();
-        uint32_t excl = carry + (wid ? warp_tot[wid - 1] : 0u) + x - v;
-        if (idx < s1) { off[idx] = excl; cursor[idx] = excl; }
+        if (idx < C) c[idx] = carry + (wid ? warp_tot[wid - 1] : 0u) + x - v;
         __syncthreads();
-        if (tid == 0) carry += warp_tot[(blockDim.x >> 5) - 1];
+        if (tid == 0) carry += warp_tot[31];
         __syncthreads();
     }
-    if (tid == 0) off[s1] = carry;
+    if (tid == 0) total[blockIdx.x] = carry;
 }
 
-__global__ void k_bucket_fill(uint64_t seed, int64_t row0, int64_t m, uint32_t s1,
-                              uint32_t* __restrict__ cursor, uint32_t* __restrict__ entries)
+// stable scatter of one tile: out[digit_base[d] + tile_off[d][tile] + rank within the tile] = entry.
+// Warp w owns the positions [w T/16, (w+1) T/16) of the tile and walks them 32 at a time, in order; the rank of an
+// element among the tile's elements with its digit = (count in earlier warps) + (count in earlier rounds of the warp)
+// + (lower lanes of the round with the same digit, match.any).
+__global__ void __launch_bounds__(SORT_THREADS)
+k_sort_scatter(uint64_t seed, int64_t row0, int64_t m, uint32_t s1, const uint32_t* __restrict__ in,
+               uint32_t* __restrict__ out, int shift, int bits, int T, int C, const uint32_t* __restrict__ tile_off,
+               const uint32_t* __restrict__ total)
 {
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < m;
-         i += (int64_t)gridDim.x * blockDim.x) {
-        uint32_t b, neg;
-        rqr_hash_sign(seed, (uint64_t)(row0 + i), s1, b, neg);
-        uint32_t pos = atomicAdd(&cursor[b], 1u);
-        entries[pos] = (uint32_t)i | (neg << 31);
+    extern __shared__ uint32_t sm_sort[];
+    const int bins = 1 << bits;
+    uint32_t* ent = sm_sort;                                        // T
+    uint32_t* dbase = ent + T;                                      // bins
+    uint16_t* dig = reinterpret_cast<uint16_t*>(dbase + bins);      // T
+    uint16_t* cnt = dig + T;                                        // SORT_WARPS x bins
+    __shared__ uint32_t warp_tot[SORT_WARPS];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int64_t base = (int64_t)blockIdx.x * T;
+    for (int i = tid; i < T; i += SORT_THREADS) {
+        uint32_t e = 0, d = 0xFFFFu;
+        if (base + i < m) sort_load(in, base + i, seed, row0, s1, shift, (uint32_t)bins - 1, e, d);
+        ent[i] = e;
+        dig[i] = (uint16_t)d;
+    }
+    for (int i = tid; i < SORT_WARPS * bins; i += SORT_THREADS) cnt[i] = 0;
+    {   // dbase = exclusive scan of total[0..bins), bins <= 512 = one element per thread
+        const uint32_t v = tid < bins ? total[tid] : 0u;
+        uint32_t x = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= o) x += y;
+        }
+        if (lane == 31) warp_tot[wid] = x;
+        __syncthreads();
+        uint32_t before = 0;
+        for (int w = 0; w < wid; ++w) before += warp_tot[w];
+        if (tid < bins) dbase[tid] = before + x - v;
+    }
+    __syncthreads();
+    const int per_warp = T / SORT_WARPS;                            // T is a multiple of 512
+    const uint32_t lt = (1u << lane) - 1u;
+    uint16_t* mycnt = cnt + wid * bins;
+    for (int r = 0; r < per_warp; r += 32) {
+        const uint32_t d = dig[wid * per_warp + r + lane];
+        const uint32_t peers = __match_any_sync(0xffffffffu, d);
+        if (d != 0xFFFFu && (peers & lt) == 0) mycnt[d] += (uint16_t)__popc(peers);
+        __syncwarp();
+    }
+    __syncthreads();
+    for (int d = tid; d < bins; d += SORT_THREADS) {                // per digit: exclusive scan over the warps
+        uint32_t run = 0;
+        for (int w = 0; w < SORT_WARPS; ++w) {
+            const uint32_t t = cnt[w * bins + d];
+            cnt[w * bins + d] = (uint16_t)run;
+            run += t;
+        }
+    }
+    __syncthreads();
+    for (int r = 0; r < per_warp; r += 32) {
+        const int i = wid * per_warp + r + lane;
+        const uint32_t d = dig[i];
+        const uint32_t peers = __match_any_sync(0xffffffffu, d);
+        uint32_t rank = 0;
+        if (d != 0xFFFFu) rank = (uint32_t)mycnt[d] + __popc(peers & lt);
+        __syncwarp();
+        if (d != 0xFFFFu && (peers & lt) == 0) mycnt[d] += (uint16_t)__popc(peers);
+        __syncwarp();
+        if (d != 0xFFFFu) out[dbase[d] + tile_off[(size_t)d * C + blockIdx.x] + rank] = ent[i];
     }
 }
 
-// One CTA per bucket (grid-stride): sort the bucket's entries by row (low 31 bits), so that the
-// list is the STABLE counting sort of the rows and W1 is reproducible run to run.  Bitonic
-// network in its all-ascending form, which tolerates virtual +inf padding, in shared memory
-// when the segment fits, else in place in global memory.
-#define RQR_SORT_SMEM_ENTRIES 8192
-__global__ void k_bucket_sort(const uint32_t* __restrict__ off, uint32_t s1,
-                              uint32_t* __restrict__ entries)
+// off[b] = first position of the sorted list whose bucket is >= b (b = 0 .. s1): bucket boundaries of the list
+__global__ void __launch_bounds__(256)
+k_bucket_bounds(uint64_t seed, int64_t row0, int64_t m, uint32_t s1, const uint32_t* __restrict__ entries,
+                uint32_t* __restrict__ off)
 {
-    __shared__ uint32_t sbuf[RQR_SORT_SMEM_ENTRIES];
-    for (uint32_t b = blockIdx.x; b < s1; b += gridDim.x) {
-        const uint32_t beg = off[b], len = off[b + 1] - beg;
-        if (len < 2) continue;
-        uint32_t* g = entries + beg;
-        const bool in_smem = len <= RQR_SORT_SMEM_ENTRIES;
-        uint32_t* a = in_smem ? sbuf : g;
-        if (in_smem) {
-            for (uint32_t i = threadIdx.x; i < len; i += blockDim.x) sbuf[i] = g[i];
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < m; i += (int64_t)gridDim.x * blockDim.x) {
+        uint32_t b, bp = 0, neg;
+        rqr_hash_sign(seed, (uint64_t)(row0 + (entries[i] & 0x7fffffffu)), s1, b, neg);
+        if (i > 0) {
+            rqr_hash_sign(seed, (uint64_t)(row0 + (entries[i - 1] & 0x7fffffffu)), s1, bp, neg);
+            bp += 1;
         }
-        __syncthreads();
-        uint32_t P = 1; while (P < len) P <<= 1;
-        for (uint32_t k = 2; k <= P; k <<= 1) {
-            for (uint32_t i = threadIdx.x; i < len; i += blockDim.x) {
-                uint32_t p = i ^ (k - 1);
-                if (p > i && p < len) {
-                    uint32_t x = a[i], y = a[p];
-                    if ((x & 0x7fffffffu) > (y & 0x7fffffffu)) { a[i] = y; a[p] = x; }
-                }
-            }
-            __syncthreads();
-            for (uint32_t j = k >> 2; j > 0; j >>= 1) {
-                for (uint32_t i = threadIdx.x; i < len; i += blockDim.x) {
-                    uint32_t p = i ^ j;
-                    if (p > i && p < len) {
-                        uint32_t x = a[i], y = a[p];
-                        if ((x & 0x7fffffffu) > (y & 0x7fffffffu)) { a[i] = y; a[p] = x; }
-                    }
-                }
-                __syncthreads();
-            }
-        }
-        if (in_smem) {
-            for (uint32_t i = threadIdx.x; i < len; i += blockDim.x) g[i] = sbuf[i];
-        }
-        __syncthreads();
+        for (uint32_t bb = bp; bb <= b; ++bb) off[bb] = (uint32_t)i;          // empty buckets in between share the offset
+        if (i == m - 1)
+            for (uint32_t bb = b + 1; bb <= s1; ++bb) off[bb] = (uint32_t)m;
     }
 }
 
@@ -148,20 +213,41 @@ static int launch_prepare_S2(int64_t s1, int s2, uint64_t seed, double* S2, cuda
     return RQR_OK;
 }
 
+// `scratch`: m words (second row list) followed by the digit-count words (rqr_sort_hist_words)
 static int launch_prepare_sorted(int64_t m, int64_t row0, int64_t s1, uint64_t seed, uint32_t* off,
-                                 uint32_t* cursor, uint32_t* entries, cudaStream_t st)
+                                 uint32_t* entries, uint32_t* scratch, cudaStream_t st)
 {
-    if (cudaMemsetAsync(cursor, 0, (size_t)s1 * 4, st) != cudaSuccess) return RQR_ERR_LAUNCH;
+    int key_bits = 0;
+    while (((int64_t)1 << key_bits) < s1) ++key_bits;
+    const int passes = key_bits <= 9 ? 1 : (key_bits + 8) / 9;
+    int bits = (key_bits + passes - 1) / passes;
+    if (bits < 1) bits = 1;
+    const int bins = 1 << bits;
+    const int T = (int)rqr_sort_tile_rows(m);
+    const int C = (int)((m + T - 1) / T);
+    uint32_t* other = scratch;
+    uint32_t* counts = scratch + (((size_t)m + 63) & ~(size_t)63);
+    uint32_t* total = counts + (size_t)RQR_SORT_MAX_BINS * C;
+    const size_t smem = (size_t)T * 4 + (size_t)bins * 4 + (size_t)T * 2 + (size_t)SORT_WARPS * bins * 2;
+    RQR_ONCE_PER_DEVICE({
+        cudaFuncSetAttribute(k_sort_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
+    });
+    // the last pass must land in `entries`: an odd number of passes starts by writing `entries`
+    const uint32_t* in = nullptr;
+    uint32_t* out = (passes & 1) ? entries : other;
+    for (int p = 0; p < passes; ++p) {
+        const int shift = p * bits;
+        k_sort_count<<<C, SORT_THREADS, 0, st>>>(seed, row0, m, (uint32_t)s1, in, shift, bits, T, C, counts);
+        RQR_LAUNCH_CHECK();
+        k_sort_scan_tiles<<<bins, 1024, 0, st>>>(counts, C, total);
+        RQR_LAUNCH_CHECK();
+        k_sort_scatter<<<C, SORT_THREADS, smem, st>>>(seed, row0, m, (uint32_t)s1, in, out, shift, bits, T, C, counts, total);
+        RQR_LAUNCH_CHECK();
+        in = out;
+        out = (out == entries) ? other : entries;
+    }
     int blocks = (int)((m + 255) / 256 < 148 * 16 ? (m + 255) / 256 : 148 * 16);
-    if (blocks < 1) blocks = 1;
-    k_bucket_hist<<<blocks, 256, 0, st>>>(seed, row0, m, (uint32_t)s1, cursor);
-    RQR_LAUNCH_CHECK();
-    k_bucket_scan<<<1, 1024, 0, st>>>(cursor, (uint32_t)s1, off, cursor);
-    RQR_LAUNCH_CHECK();
-    k_bucket_fill<<<blocks, 256, 0, st>>>(seed, row0, m, (uint32_t)s1, cursor, entries);
-    RQR_LAUNCH_CHECK();
-    int sb = (int)(s1 < 148 * 8 ? s1 : 148 * 8);
-    k_bucket_sort<<<sb, 256, 0, st>>>(off, (uint32_t)s1, entries);
+    k_bucket_bounds<<<blocks, 256, 0, st>>>(seed, row0, m, (uint32_t)s1, entries, off);
     RQR_LAUNCH_CHECK();
     return RQR_OK;
 }
@@ -176,7 +262,7 @@ extern "C" int rqr_sketch_prepare(int64_t m, int n, int64_t row0, int64_t s1, in
     if (s2 < 1 || s2 > RQR_MAX_S2 || s2 > s1) return -5;
     const bool rademacher = (variant & RQR_S2_RADEMACHER) != 0;
     variant &= ~RQR_S2_RADEMACHER;
-    if (variant != RQR_VARIANT_SORTED && variant != RQR_VARIANT_SCATTER) return -7;
+    if (variant != RQR_VARIANT_SORTED && variant != RQR_VARIANT_SCATTER && variant != RQR_VARIANT_STREAM) return -7;
     if (!work) return -8;
     cudaStream_t st = (cudaStream_t)stream;
     RqrLayout L = rqr_layout(m, n, s1, rademacher);
@@ -184,8 +270,8 @@ extern "C" int rqr_sketch_prepare(int64_t m, int n, int64_t row0, int64_t s1, in
     int rc = rademacher ? RQR_OK : launch_prepare_S2(s1, s2, seed, (double*)(w + L.C), st);
     if (rc != RQR_OK) return rc;
     if (variant == RQR_VARIANT_SORTED)
-        rc = launch_prepare_sorted(m, row0, s1, seed, (uint32_t*)(w + L.B_off),
-                                   (uint32_t*)(w + L.B_cur), (uint32_t*)(w + L.E), st);
+        rc = launch_prepare_sorted(m, row0, s1, seed, (uint32_t*)(w + L.B_off), (uint32_t*)(w + L.E),
+                                   (uint32_t*)(w + L.G_sort), st);
     return rc;
 }
 
@@ -291,6 +377,109 @@ k_countsketch_scatter(const double* __restrict__ V, int64_t m, int64_t ldv, int 
     }
 }
 
+// STREAM variant: no stored S1.  Every warp is its own pipeline over 8-row blocks of V (rows in order: a sequential
+// HBM stream): bulk async copy into a private ring, bucket and sign of the 8 rows from Philox (lanes 0..7), sign flip in
+// shared memory, then ONE bulk reduction per row, cp.reduce.async.bulk.global.shared::cta.add.f64 (SASS UBLKRED):
+// the L2 adds 8n contiguous bytes to row h(i) of W1 -- n/4 32-byte sectors per request instead of n element-wise
+// atomics issued by the LSU.  W1 must be zero on entry.
+#define CS_MAX_STAGES 8
+#define CS_MAX_WARPS 16
+template <bool CONTIG>
+__global__ void __launch_bounds__(CS_MAX_WARPS * 32, 1)
+k_countsketch_stream(const double* __restrict__ V, int64_t m, int64_t ldv, int n, int64_t row0, uint64_t seed,
+                     uint32_t s1, double* __restrict__ W1, int warps, int stages)
+{
+    extern __shared__ __align__(16) double smem[];
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem);                         // warps x stages
+    double* ring = smem + ((warps * stages + 1) & ~1);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (warp >= warps) return;
+    if (lane < stages) mbar_init(bars + warp * stages + lane, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    __syncwarp();
+    uint64_t* bar = bars + warp * stages;
+    double* buf = ring + (size_t)warp * stages * 8 * n;
+    const int64_t nrb = (m + 7) / 8;
+    const int64_t gw = (int64_t)blockIdx.x * warps + warp;
+    const int64_t stride = (int64_t)gridDim.x * warps;
+    auto issue = [&](int stage, int64_t rblk) {
+        const int valid = (int)((m - rblk * 8) < 8 ? (m - rblk * 8) : 8);
+        if (lane == 0) mbar_expect_tx(bar + stage, (uint32_t)(valid * n * 8));
+        __syncwarp();
+        if (CONTIG) {
+            if (lane == 0) bulk_g2s(buf + (size_t)stage * 8 * n, V + rblk * 8 * ldv, (uint32_t)(valid * n * 8), bar + stage);
+        } else if (lane < valid) {
+            bulk_g2s(buf + ((size_t)stage * 8 + lane) * n, V + (rblk * 8 + lane) * ldv, (uint32_t)(n * 8), bar + stage);
+        }
+    };
+    // stages of the ring at iteration i: block i (in use), block i - 1 (its reductions may still read it) and the
+    // blocks i + 1 .. i + stages - 2 in flight
+    for (int s = 0; s < stages - 2; ++s)
+        if (gw + s * stride < nrb) issue(s, gw + s * stride);
+    int stage = 0, it = 0;
+    uint32_t phase = 0;
+    for (int64_t rblk = gw; rblk < nrb; rblk += stride, ++it) {
+        // refill the stage consumed two iterations ago: its bulk reductions have READ shared memory once every lane
+        // has at most its newest group pending; row-block i + stages - 2 goes into it
+        asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
+        __syncwarp();
+        {
+            const int64_t next = rblk + (int64_t)(stages - 2) * stride;
+            const int ps = stage >= 2 ? stage - 2 : stage + stages - 2;
+            if (next < nrb) issue(ps, next);
+        }
+        const int valid = (int)((m - rblk * 8) < 8 ? (m - rblk * 8) : 8);
+        uint32_t b = 0, neg = 0;
+        if (lane < valid) rqr_hash_sign(seed, (uint64_t)(row0 + rblk * 8 + lane), s1, b, neg);
+        const uint32_t negmask = __ballot_sync(0xffffffffu, neg != 0);
+        mbar_wait(bar + stage, phase);
+        double* rb = buf + (size_t)stage * 8 * n;
+        for (uint32_t msk = negmask; msk; msk &= msk - 1) {                   // rows with sigma = -1
+            double* row = rb + (size_t)(__ffs(msk) - 1) * n;
+            for (int c = 2 * lane; c < n; c += 64) {
+                double2 v = *reinterpret_cast<double2*>(row + c);
+                *reinterpret_cast<double2*>(row + c) = make_double2(-v.x, -v.y);
+            }
+        }
+        fence_proxy_async();
+        __syncwarp();
+        if (lane < valid) {
+            asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.f64 [%0], [%1], %2;"
+                         :: "l"(W1 + (size_t)b * n), "r"(smem_u32(rb + (size_t)lane * n)), "r"((uint32_t)(n * 8)) : "memory");
+        }
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        if (++stage == stages) { stage = 0; phase ^= 1u; }
+    }
+    asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+}
+
+static int launch_countsketch_stream(const double* V, int64_t m, int n, int64_t ldv, int64_t row0, int64_t s1,
+                                     uint64_t seed, double* W1, cudaStream_t st)
+{
+    if ((n & 1) || (ldv & 1) || (((uintptr_t)V | (uintptr_t)W1) & 15)) return RQR_TALL_NOT_HANDLED;
+    // The per-warp loop is latency-bound (copy in, hash, flip, reduce out): what counts is row-blocks in flight per SM.
+    // Ring = warps x stages x 8 rows x n doubles within 192 KB, as many warps as leave >= 5 stages (3 in flight):
+    // n <= 38: 16 warps, n <= 76: 8 (n = 64: 8 x 6), n <= 153: 4, above: 4 x 3.
+    int warps = CS_MAX_WARPS;
+    while (warps > 4 && (size_t)warps * 5 * 64 * n > 192 * 1024) warps >>= 1;
+    int stages = (int)((192 * 1024) / ((size_t)warps * 64 * n));
+    if (stages > CS_MAX_STAGES) stages = CS_MAX_STAGES;
+    if (stages < 3) stages = 3;
+    while (warps > 1 && (size_t)warps * stages * 64 * n > 200 * 1024) warps >>= 1;
+    const size_t smem = (size_t)(((warps * stages + 1) & ~1) + (size_t)warps * stages * 8 * n) * sizeof(double);
+    RQR_ONCE_PER_DEVICE({
+        cudaFuncSetAttribute(k_countsketch_stream<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        cudaFuncSetAttribute(k_countsketch_stream<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    });
+    const int64_t nrb = (m + 7) / 8;
+    int64_t g = (nrb + warps - 1) / warps;
+    const int grid = (int)(g < 148 ? (g < 1 ? 1 : g) : 148);
+    if (ldv == n) k_countsketch_stream<true><<<grid, CS_MAX_WARPS * 32, smem, st>>>(V, m, ldv, n, row0, seed, (uint32_t)s1, W1, warps, stages);
+    else          k_countsketch_stream<false><<<grid, CS_MAX_WARPS * 32, smem, st>>>(V, m, ldv, n, row0, seed, (uint32_t)s1, W1, warps, stages);
+    RQR_LAUNCH_CHECK();
+    return RQR_OK;
+}
+
 extern "C" int rqr_countsketch(const double* V, int64_t m, int n, int64_t ldv, int64_t row0,
                                int64_t s1, uint64_t seed, double* W1, void* work, int variant,
                                int flags, void* stream)
@@ -304,8 +493,15 @@ extern "C" int rqr_countsketch(const double* V, int64_t m, int n, int64_t ldv, i
     if (!W1) return -8;
     const bool rademacher = (variant & RQR_S2_RADEMACHER) != 0;      // only moves region E of the workspace
     variant &= ~RQR_S2_RADEMACHER;
-    if (variant != RQR_VARIANT_SORTED && variant != RQR_VARIANT_SCATTER) return -10;
+    if (variant != RQR_VARIANT_SORTED && variant != RQR_VARIANT_SCATTER && variant != RQR_VARIANT_STREAM) return -10;
     cudaStream_t st = (cudaStream_t)stream;
+    if (variant == RQR_VARIANT_STREAM) {
+        if (cudaMemsetAsync(W1, 0, (size_t)s1 * n * sizeof(double), st) != cudaSuccess)
+            return RQR_ERR_LAUNCH;
+        int rc = launch_countsketch_stream(V, m, n, ldv, row0, s1, seed, W1, st);
+        if (rc != RQR_TALL_NOT_HANDLED) return rc;
+        variant = RQR_VARIANT_SCATTER;              // odd n / ld or unaligned bases: per-element atomics (W1 is zeroed)
+    }
     if (variant == RQR_VARIANT_SCATTER) {
         if (cudaMemsetAsync(W1, 0, (size_t)s1 * n * sizeof(double), st) != cudaSuccess)
             return RQR_ERR_LAUNCH;
@@ -320,27 +516,34 @@ extern "C" int rqr_countsketch(const double* V, int64_t m, int n, int64_t ldv, i
     RqrLayout L = rqr_layout(m, n, s1, rademacher);
     char* w = (char*)work;
     uint32_t* off = (uint32_t*)(w + L.B_off);
-    uint32_t* cur = (uint32_t*)(w + L.B_cur);
     uint32_t* ent = (uint32_t*)(w + L.E);
     if (!(flags & RQR_FLAG_PREPARED)) {
-        int rc = launch_prepare_sorted(m, row0, s1, seed, off, cur, ent, st);
+        int rc = launch_prepare_sorted(m, row0, s1, seed, off, ent, (uint32_t*)(w + L.G_sort), st);
         if (rc != RQR_OK) return rc;
     }
     const bool vec2 = (n % 2 == 0) && (ldv % 2 == 0) && (((uintptr_t)V & 15) == 0);
     const int lpr = vec2 ? n / 2 : n;
     const int R = 256 / lpr > 1 ? 256 / lpr : 1;
     size_t smem = (size_t)R * n * sizeof(double);
-    // fewer buckets than half the resident CTAs (148 x 8): split every bucket's row list into `split` segments so
-    // that the grid is full; the partial sketches live in region A of the workspace (free during A1)
+    // One CTA walks one bucket at a time, 148 x 8 CTAs are resident: with s1 buckets of equal expected length the
+    // pass takes ceil(s1 / 1184) rounds, i.e. it runs at (s1 / 1184) / ceil(s1 / 1184) of its speed (s1 = 2048:
+    // 1.73 / 2 = 86%; s1 = 200: 17%).  Every bucket's row list is therefore split into `split` segments, the smallest
+    // count that fills the last round to >= 95% (and the grid at all when s1 < 1184); the segment sums go to `split`
+    // partial sketches in region A of the workspace (free during A1) and are added in a fixed order.
     int64_t split = 1;
-    if (s1 * 2 <= 148 * 8) {
-        split = (148 * 8 + s1 - 1) / s1;
+    {
+        const double slots = 148.0 * 8.0;
         const int64_t fit = (int64_t)rqr_gram_partial_cap(n) * n / s1;          // region A holds cap n^2 doubles
         const int64_t rows = m / (s1 * 4 * R);                                  // >= 4 R rows per segment
-        if (split > fit) split = fit;
-        if (split > rows) split = rows;
-        if (split > 64) split = 64;
-        if (split < 2) split = 1;
+        int64_t best = 1;
+        double best_eff = 0.0;
+        for (int64_t sp = 1; sp <= 64 && sp <= fit && (sp == 1 || sp <= rows); ++sp) {
+            const double waves = (double)(s1 * sp) / slots;
+            const double eff = waves / ceil(waves);
+            if (eff > best_eff + 1e-9) { best_eff = eff; best = sp; }
+            if (eff >= 0.95) break;
+        }
+        split = best;
     }
     double* dst = split > 1 ? (double*)(w + L.A) : W1;
     const int64_t items = s1 * split;
@@ -712,16 +915,41 @@ extern "C" int rqr_dense_gauss_sketch(const double* V, int64_t m, int n, int64_t
     cudaStream_t st = (cudaStream_t)stream;
     double* part = (double*)((char*)work + 256);      // region A
     int P = 1;
+    const int64_t elems = (int64_t)s * n;
+    {
+        // FP64 tensor-pipe kernel (rqr_dense_mma.cu): even n and ld, 16-byte aligned V
+        const int64_t Pcap = ((int64_t)rqr_gram_partial_cap(n) * n) / s;
+        int rc = rqr_dense_gauss_mma(V, m, n, ldv, row0, m_total, s, seed, part, Pcap, &P, false, st);
+        if (rc == RQR_OK) {
+            k_reduce_partials<<<(int)((elems + 63) / 64), 256, 0, st>>>(part, P, elems, W);
+            RQR_LAUNCH_CHECK();
+            return RQR_OK;
+        }
+        if (rc != RQR_TALL_NOT_HANDLED) return rc;
+    }
     if (n <= 16) launch_dense_gauss<2, 4>(V, m, n, ldv, row0, m_total, s, seed, part, &P, st);
     else if (n <= 32) launch_dense_gauss<4, 4>(V, m, n, ldv, row0, m_total, s, seed, part, &P, st);
     else if (n <= 64) launch_dense_gauss<8, 4>(V, m, n, ldv, row0, m_total, s, seed, part, &P, st);
     else if (n <= 128) launch_dense_gauss<16, 2>(V, m, n, ldv, row0, m_total, s, seed, part, &P, st);
     else launch_dense_gauss<32, 1>(V, m, n, ldv, row0, m_total, s, seed, part, &P, st);
     RQR_LAUNCH_CHECK();
-    int64_t elems = (int64_t)s * n;
     k_reduce_partials<<<(int)((elems + 63) / 64), 256, 0, st>>>(part, P, elems, W);
     RQR_LAUNCH_CHECK();
     return RQR_OK;
+}
+
+// Measurement hook: the DRAW of the s x m Gaussians of rqr_dense_gauss_sketch alone (same launch shape, same
+// per-lane Box-Muller pairs, no V traffic and no products): the generation bound of B''.  `work` as above.
+extern "C" int rqr_debug_dense_gauss_draw_only(int64_t m, int n, int s, uint64_t seed, void* work, void* stream)
+{
+    if (m < 1) return -1;
+    if (n < 2 || n > RQR_MAX_N || (n & 1)) return -2;
+    if (s < 1 || s > RQR_MAX_S2) return -3;
+    if (!work) return -5;
+    double* part = (double*)((char*)work + 256);
+    int P = 1;
+    const int64_t Pcap = ((int64_t)rqr_gram_partial_cap(n) * n) / s;
+    return rqr_dense_gauss_mma((const double*)work, m, n, n, 0, m, s, seed, part, Pcap, &P, true, (cudaStream_t)stream);
 }
 
 // =========================================================================================

@@ -63,6 +63,7 @@ def main(argv=None):
     t["A0_sketch_prepare"] = _time(lambda: rq.sketch_prepare(m, n, s1, s2, 42, work), max(2, reps // 3))
     t["A1_countsketch_sorted"] = _time(lambda: rq.countsketch(V, s1, 42, W1, work, rq.VARIANT_SORTED, P), reps)
     t["A1_countsketch_scatter"] = _time(lambda: rq.countsketch(V, s1, 42, W1, work, rq.VARIANT_SCATTER, 0), reps)
+    t["A1_countsketch_stream"] = _time(lambda: rq.countsketch(V, s1, 42, W1, work, rq.VARIANT_STREAM, 0), reps)
     rq.countsketch(V, s1, 42, W1, work, rq.VARIANT_SORTED, P)
     t["A2_gauss_sketch"] = _time(lambda: rq.gauss_sketch(W1, s2, 42, W, work, P), reps)
     Wc = W.clone()
@@ -73,6 +74,8 @@ def main(argv=None):
     t_copy = _time(lambda: W.copy_(Wc), reps)
     t["A3_small_geqrf"] = _time(geqrf, reps) - t_copy
     t["A4_trsm_gram_store_V1"] = _time(lambda: rq.trsm_gram(V, R0, G, Q, work), reps)
+    if n <= 64:
+        t["A4_trsm_gram_no_store"] = _time(lambda: rq.trsm_gram(V, R0, G, None, work), reps)
     t["A4_gram_only"] = _time(lambda: rq.trsm_gram(V, None, G, None, work), reps)
     rq.trsm_gram(V, R0, G, Q, work)
     t["A5_chol"] = _time(lambda: rq.chol(G, R1, info), reps)
@@ -82,7 +85,12 @@ def main(argv=None):
     t["A7_triu_mul"] = _time(lambda: rq.triu_mul(R1, R0, R), reps)
     # N4: Rademacher S2 generated on the fly (no S2 in the workspace), and the one-shot with either S2
     RAD = rq.S2_RADEMACHER
+    t["one_shot_stream_variant"] = _time(lambda: rq.rand_cholqr(V, s1, s2, 42, Q, R, work, info, rq.VARIANT_STREAM, P), reps)
     t["one_shot_gauss_S2"] = _time(lambda: rq.rand_cholqr(V, s1, s2, 42, Q, R, work, info, 0, P), reps)
+    if n <= 64:
+        t["one_shot_store_V1"] = _time(lambda: rq.rand_cholqr(V, s1, s2, 42, Q, R, work, info, 0, P | rq.FLAG_STORE_V1), reps)
+        t["one_shot_recompute_V1"] = _time(lambda: rq.rand_cholqr(V, s1, s2, 42, Q, R, work, info, 0, P | rq.FLAG_RECOMPUTE_V1), reps)
+        t["cholqr2"] = _time(lambda: rq.cholqr2(V, Q, R, work, info), reps)
     del work
     workr = rq.alloc_workspace(m, n, s1, s2, RAD)
     t["A0_sketch_prepare_rademacher"] = _time(lambda: rq.sketch_prepare(m, n, s1, s2, 42, workr, RAD), max(2, reps // 3))
@@ -93,6 +101,7 @@ def main(argv=None):
     out["achieved"] = {
         "A1_sorted_GBs": 8.0 * mn / t["A1_countsketch_sorted"] / 1e6,
         "A1_scatter_GBs": 8.0 * mn / t["A1_countsketch_scatter"] / 1e6,
+        "A1_stream_GBs": 8.0 * mn / t["A1_countsketch_stream"] / 1e6,
         "A4_TFLOPs": 2.0 * mn * n / t["A4_trsm_gram_store_V1"] / 1e9,
         "A4_GBs": 16.0 * mn / t["A4_trsm_gram_store_V1"] / 1e6,
         "A6_GBs": 16.0 * mn / t["A6_apply_in_place"] / 1e6,

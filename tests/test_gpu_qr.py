@@ -67,7 +67,7 @@ def test_rand_cholqr_matches_oracle(rq, orc, name, m, n, kappa):
     Qo, Ro, io = orc.rand_cholqr(V.numpy(), s1, s2, 42)
     assert io == 0
     for variant, flags, prepared in [(0, 0, False), (0, rq.FLAG_RECOMPUTE_V1, True), (0, rq.FLAG_STORE_V1, True),
-                                     (1, 0, True)]:
+                                     (1, 0, True), (2, 0, True)]:
         Q, R, info = run_rand(rq, Vd, s1, s2, 42, variant, flags, prepared)
         assert info == 0
         assert orth_err(Q) <= ORTH_TOL

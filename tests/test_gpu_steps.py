@@ -77,7 +77,7 @@ def test_sorted_row_list_is_the_stable_sort(rq, orc, m, s1, row0):
                                     (5000, 33, 64), (3000, 256, 4000), (37, 8, 16), (8192, 2, 8),
                                     # few buckets: every bucket's row list is split over several CTAs (two-stage sum)
                                     (200000, 10, 200), (150001, 16, 64), (120000, 7, 37), (300000, 24, 500)])
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 def test_countsketch_parity(rq, orc, m, n, s1, variant):
     V = inputs.make_V(m, n, 1e8, 7)
     Vd = V.cuda()
@@ -103,7 +103,7 @@ def test_countsketch_strided_and_row_offset(rq, orc):
     V = big[:, :n]                        # ldv = n + 6
     W1 = torch.empty(s1, n, dtype=torch.float64, device="cuda")
     work = rq.alloc_workspace(m, n, s1, 2 * n)
-    for variant in (0, 1):
+    for variant in (0, 1, 2):
         rq.countsketch(V, s1, 9, W1, work, variant=variant, row0=1000)
         ref = orc.countsketch(host(V), s1, 9, row0=1000)
         assert np.array_equal(host(W1), ref)
