@@ -79,7 +79,7 @@ def test_argument_validation_without_gpu(lib):
     full = lib.rqr_workspace_bytes(1 << 20, 64, 8192, 128, 0)
     lean = lib.rqr_workspace_bytes(1 << 20, 64, 8192, 128, 16)
     assert full - lean == 8 * 1024 * 8192
-    assert lib.rqr_rand_cholqr(one, 100, 8, 64, 16, 1, one, one, one, z, 2, 0, z) == -11                         # variant
+    assert lib.rqr_rand_cholqr(one, 100, 8, 64, 16, 1, one, one, one, z, 3, 0, z) == -11                         # variant
     assert lib.rqr_rand_cholqr(one, 100, 8, 64, 16, 1, one, one, one, z, 32, 0, z) == -11
 
 
