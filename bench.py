@@ -109,16 +109,11 @@ class ClockSampler(threading.Thread):
 
 def launches_per_step(n, m=0, s1=0):
     """Kernels of ours launched by one rqr_rand_cholqr with a prepared sketch (sorted variant):
-    countsketch 1 (+ 1 partial reduction when the bucket lists are split: s1 / 1184 not within 5% of an integer from
-    below), Gaussian GEMM + reduce 2,
+    countsketch 1 (+ 1 partial reduction when the bucket lists are split, 2 s1 <= 1184), Gaussian GEMM + reduce 2,
     Householder 1, A4 2 (n <= 64: fused kernel + partial reduce) or 4 (n > 64: fragment build, panel substitution,
     syrk, reduce), Cholesky 1 (the product R = R1 R0 is fused into it for n <= 128; a separate launch above),
     A6 1 (n > 64: + fragment build).  Stored or recomputed V1: the same count."""
-    split = 0
-    if s1:                                          # rqr_countsketch splits the bucket lists unless they fill the rounds
-        import math
-        w = s1 / 1184.0
-        split = 0 if w / math.ceil(w) >= 0.95 else 1
+    split = 1 if (s1 and 2 * s1 <= 1184) else 0
     if n <= 64:
         return 8 + split + max(0, -(-m // (1 << 23)) - 1)          # one more A4 launch per further 2^23-row chunk
     return (11 if n <= 128 else 12) + max(0, -(-m // (1 << 21)) - 1)   # the syrk runs per 2^21-row chunk

@@ -112,9 +112,9 @@ int rqr_sketch_prepare(int64_t m, int n, int64_t row0, int64_t s1, int s2, uint6
 
 /* A1 -- CountSketch, Alg. 1 step 1 first half: W1 = S1 V,
  * W1[h(i),:] += sigma(i) V[i,:], S1 unscaled.  W1 (s1 x n) is overwritten.
- * RQR_VARIANT_SORTED: when s1 buckets do not fill the rounds of the 1184 resident CTAs to 95% (s1 < 1184,
- * s1 = 2048, ...), the bucket row lists are split into segments and the partial sketches pass through the
- * Gram-partial scratch of `work` (contents lost), summed in a fixed order: the result stays bit-reproducible. */
+ * RQR_VARIANT_SORTED with few buckets (2 s1 <= 1184): the bucket row lists are split into segments so that the
+ * grid is full, and the partial sketches pass through the Gram-partial scratch of `work` (contents lost), summed
+ * in a fixed order: the result stays bit-reproducible.                                                        */
 int rqr_countsketch(const double* V, int64_t m, int n, int64_t ldv, int64_t row0, int64_t s1,
                     uint64_t seed, double* W1, void* work, int variant, int flags, void* stream);
 

@@ -63,12 +63,12 @@ static inline int rqr_gram_partial_cap(int n)
 __host__ __device__ static inline int64_t rqr_s2_ld(int64_t s1) { return (s1 + 15) & ~(int64_t)15; }
 
 // A0 radix sort (rqr_sketch.cu): rows per tile and words of its digit-count scratch ((bins + 1) x tiles + bins)
-#define RQR_SORT_MAX_BINS 512
+#define RQR_SORT_MAX_BINS 256
 static inline int64_t rqr_sort_tile_rows(int64_t m)
 {
-    int64_t t = 2048;
-    while (t < 16384 && t * 512 < m) t *= 2;
-    return t;
+    // about eight tiles per SM (two resident CTAs, four rounds), a multiple of 1024 rows, 1024 .. 8192
+    int64_t t = ((m + 1183) / 1184 + 1023) / 1024 * 1024;
+    return t < 1024 ? 1024 : (t > 8192 ? 8192 : t);
 }
 static inline size_t rqr_sort_hist_words(int64_t m)
 {

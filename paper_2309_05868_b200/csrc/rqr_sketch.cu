@@ -31,7 +31,7 @@ __global__ void k_gen_S2(uint64_t seed, int s2, int64_t s1, int64_t ld, int64_t 
 
 // -----------------------------------------------------------------------------------------------------------------
 // Bucket-sorted row list = STABLE sort of the rows by bucket, as an LSD radix sort on the bucket id with digits of
-// `bits` <= 9 bits.  A pass is three launches -- digit counts per tile of T consecutive positions, an exclusive scan of
+// `bits` <= 8 bits.  A pass is three launches -- digit counts per tile of T consecutive positions, an exclusive scan of
 // the counts of every digit over the tiles, a stable scatter -- and every step has a fixed order, so the list is the same
 // bits run to run (W1 is then bit-reproducible) and equals numpy's stable argsort of the oracle's buckets
 // (tests/test_gpu_steps.py::test_sorted_row_list_is_the_stable_sort).  The bucket of an entry is recomputed from its
@@ -111,31 +111,34 @@ k_sort_scan_tiles(uint32_t* __restrict__ counts, int C, uint32_t* __restrict__ t
 }
 
 // stable scatter of one tile: out[digit_base[d] + tile_off[d][tile] + rank within the tile] = entry.
-// Warp w owns the positions [w T/16, (w+1) T/16) of the tile and walks them 32 at a time, in order; the rank of an
-// element among the tile's elements with its digit = (count in earlier warps) + (count in earlier rounds of the warp)
-// + (lower lanes of the round with the same digit, match.any).
-__global__ void __launch_bounds__(SORT_THREADS)
+// Thread t owns the K = T / 256 consecutive positions [t K, (t + 1) K) of the tile and a private column cnt[d][t] of
+// 16-bit counters: it counts its digits, the counters of every digit are scanned over the threads (thread order =
+// position order), and a second walk over the same positions hands out the ranks in order.  No atomics and no vote /
+// match instructions (a match.any version spent 85% of its time in MATCH: ~28 distinct digits per warp).
+#define SCATTER_THREADS 256
+__global__ void __launch_bounds__(SCATTER_THREADS)
 k_sort_scatter(uint64_t seed, int64_t row0, int64_t m, uint32_t s1, const uint32_t* __restrict__ in,
                uint32_t* __restrict__ out, int shift, int bits, int T, int C, const uint32_t* __restrict__ tile_off,
                const uint32_t* __restrict__ total)
 {
     extern __shared__ uint32_t sm_sort[];
-    const int bins = 1 << bits;
-    uint32_t* ent = sm_sort;                                        // T
-    uint32_t* dbase = ent + T;                                      // bins
-    uint16_t* dig = reinterpret_cast<uint16_t*>(dbase + bins);      // T
-    uint16_t* cnt = dig + T;                                        // SORT_WARPS x bins
-    __shared__ uint32_t warp_tot[SORT_WARPS];
+    constexpr int NT = SCATTER_THREADS;
+    const int bins = 1 << bits, K = T / NT, KP = K + 2;             // K % 4 == 0: KP / 2 odd, conflict-free walks
+    uint32_t* ent = sm_sort;                                        // NT x (K + 1): odd row stride, conflict-free
+    uint32_t* dbase = ent + NT * (K + 1);                           // bins (<= 256)
+    uint16_t* dig = reinterpret_cast<uint16_t*>(dbase + bins);      // NT x KP
+    uint16_t* cnt = dig + (size_t)NT * KP;                          // bins x NT
+    __shared__ uint32_t warp_tot[NT / 32];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int64_t base = (int64_t)blockIdx.x * T;
-    for (int i = tid; i < T; i += SORT_THREADS) {
+    for (int i = tid; i < T; i += NT) {                             // coalesced: position i -> owner i / K, slot i % K
         uint32_t e = 0, d = 0xFFFFu;
         if (base + i < m) sort_load(in, base + i, seed, row0, s1, shift, (uint32_t)bins - 1, e, d);
-        ent[i] = e;
-        dig[i] = (uint16_t)d;
+        ent[(i / K) * (K + 1) + (i % K)] = e;
+        dig[(i / K) * KP + (i % K)] = (uint16_t)d;
     }
-    for (int i = tid; i < SORT_WARPS * bins; i += SORT_THREADS) cnt[i] = 0;
-    {   // dbase = exclusive scan of total[0..bins), bins <= 512 = one element per thread
+    for (int i = tid; i < bins * NT / 2; i += NT) reinterpret_cast<uint32_t*>(cnt)[i] = 0u;
+    {   // dbase = exclusive scan of total[0..bins), bins <= 256 = one element per thread
         const uint32_t v = tid < bins ? total[tid] : 0u;
         uint32_t x = v;
 #pragma unroll
@@ -147,38 +150,38 @@ k_sort_scatter(uint64_t seed, int64_t row0, int64_t m, uint32_t s1, const uint32
         __syncthreads();
         uint32_t before = 0;
         for (int w = 0; w < wid; ++w) before += warp_tot[w];
-        if (tid < bins) dbase[tid] = before + x - v;
+        // first output position of this tile's run of digit d: the digit's base + the earlier tiles' counts
+        if (tid < bins) dbase[tid] = before + x - v + tile_off[(size_t)tid * C + blockIdx.x];
     }
     __syncthreads();
-    const int per_warp = T / SORT_WARPS;                            // T is a multiple of 512
-    const uint32_t lt = (1u << lane) - 1u;
-    uint16_t* mycnt = cnt + wid * bins;
-    for (int r = 0; r < per_warp; r += 32) {
-        const uint32_t d = dig[wid * per_warp + r + lane];
-        const uint32_t peers = __match_any_sync(0xffffffffu, d);
-        if (d != 0xFFFFu && (peers & lt) == 0) mycnt[d] += (uint16_t)__popc(peers);
-        __syncwarp();
+    const uint16_t* mydig = dig + (size_t)tid * KP;
+    for (int j = 0; j < K; ++j) {
+        const uint32_t d = mydig[j];
+        if (d != 0xFFFFu) cnt[d * NT + tid] += 1;
     }
     __syncthreads();
-    for (int d = tid; d < bins; d += SORT_THREADS) {                // per digit: exclusive scan over the warps
-        uint32_t run = 0;
-        for (int w = 0; w < SORT_WARPS; ++w) {
-            const uint32_t t = cnt[w * bins + d];
-            cnt[w * bins + d] = (uint16_t)run;
-            run += t;
+    for (int d = wid; d < bins; d += NT / 32) {                     // per digit: exclusive scan over the 256 threads
+        uint16_t* row = cnt + (size_t)d * NT;
+        uint32_t v[8], sum = 0;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) { v[q] = row[lane * 8 + q]; sum += v[q]; }
+        uint32_t x = sum;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= o) x += y;
         }
+        uint32_t run = x - sum;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) { row[lane * 8 + q] = (uint16_t)run; run += v[q]; }
     }
     __syncthreads();
-    for (int r = 0; r < per_warp; r += 32) {
-        const int i = wid * per_warp + r + lane;
-        const uint32_t d = dig[i];
-        const uint32_t peers = __match_any_sync(0xffffffffu, d);
-        uint32_t rank = 0;
-        if (d != 0xFFFFu) rank = (uint32_t)mycnt[d] + __popc(peers & lt);
-        __syncwarp();
-        if (d != 0xFFFFu && (peers & lt) == 0) mycnt[d] += (uint16_t)__popc(peers);
-        __syncwarp();
-        if (d != 0xFFFFu) out[dbase[d] + tile_off[(size_t)d * C + blockIdx.x] + rank] = ent[i];
+    for (int j = 0; j < K; ++j) {
+        const uint32_t d = mydig[j];
+        if (d == 0xFFFFu) continue;
+        const uint32_t rank = cnt[d * NT + tid];
+        cnt[d * NT + tid] = (uint16_t)(rank + 1);
+        out[dbase[d] + rank] = ent[tid * (K + 1) + j];
     }
 }
 
@@ -187,14 +190,18 @@ __global__ void __launch_bounds__(256)
 k_bucket_bounds(uint64_t seed, int64_t row0, int64_t m, uint32_t s1, const uint32_t* __restrict__ entries,
                 uint32_t* __restrict__ off)
 {
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < m; i += (int64_t)gridDim.x * blockDim.x) {
-        uint32_t b, bp = 0, neg;
-        rqr_hash_sign(seed, (uint64_t)(row0 + (entries[i] & 0x7fffffffu)), s1, b, neg);
-        if (i > 0) {
-            rqr_hash_sign(seed, (uint64_t)(row0 + (entries[i - 1] & 0x7fffffffu)), s1, bp, neg);
-            bp += 1;
-        }
-        for (uint32_t bb = bp; bb <= b; ++bb) off[bb] = (uint32_t)i;          // empty buckets in between share the offset
+    const int lane = threadIdx.x & 31;
+    const int64_t nthreads = (int64_t)gridDim.x * blockDim.x;
+    const int64_t rounds = (m + nthreads - 1) / nthreads;
+    for (int64_t it = 0; it < rounds; ++it) {                                 // whole warps stay in the loop (shuffle)
+        const int64_t i = it * nthreads + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+        uint32_t b = 0, neg;
+        if (i < m) rqr_hash_sign(seed, (uint64_t)(row0 + (entries[i] & 0x7fffffffu)), s1, b, neg);
+        uint32_t bp = __shfl_up_sync(0xffffffffu, b, 1);                      // bucket of position i - 1
+        if (i >= m) continue;
+        if (lane == 0 && i > 0) rqr_hash_sign(seed, (uint64_t)(row0 + (entries[i - 1] & 0x7fffffffu)), s1, bp, neg);
+        const uint32_t first = i > 0 ? bp + 1 : 0;
+        for (uint32_t bb = first; bb <= b; ++bb) off[bb] = (uint32_t)i;       // empty buckets in between share the offset
         if (i == m - 1)
             for (uint32_t bb = b + 1; bb <= s1; ++bb) off[bb] = (uint32_t)m;
     }
@@ -219,7 +226,7 @@ static int launch_prepare_sorted(int64_t m, int64_t row0, int64_t s1, uint64_t s
 {
     int key_bits = 0;
     while (((int64_t)1 << key_bits) < s1) ++key_bits;
-    const int passes = key_bits <= 9 ? 1 : (key_bits + 8) / 9;
+    const int passes = key_bits <= 8 ? 1 : (key_bits + 7) / 8;     // digits of at most 8 bits (k_sort_scatter's table)
     int bits = (key_bits + passes - 1) / passes;
     if (bits < 1) bits = 1;
     const int bins = 1 << bits;
@@ -228,9 +235,10 @@ static int launch_prepare_sorted(int64_t m, int64_t row0, int64_t s1, uint64_t s
     uint32_t* other = scratch;
     uint32_t* counts = scratch + (((size_t)m + 63) & ~(size_t)63);
     uint32_t* total = counts + (size_t)RQR_SORT_MAX_BINS * C;
-    const size_t smem = (size_t)T * 4 + (size_t)bins * 4 + (size_t)T * 2 + (size_t)SORT_WARPS * bins * 2;
+    const int K = T / SCATTER_THREADS;
+    const size_t smem = (size_t)SCATTER_THREADS * (K + 1) * 4 + (size_t)bins * 4 + (size_t)SCATTER_THREADS * (K + 2) * 2 + (size_t)bins * SCATTER_THREADS * 2;
     RQR_ONCE_PER_DEVICE({
-        cudaFuncSetAttribute(k_sort_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
+        cudaFuncSetAttribute(k_sort_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     });
     // the last pass must land in `entries`: an odd number of passes starts by writing `entries`
     const uint32_t* in = nullptr;
@@ -241,7 +249,7 @@ static int launch_prepare_sorted(int64_t m, int64_t row0, int64_t s1, uint64_t s
         RQR_LAUNCH_CHECK();
         k_sort_scan_tiles<<<bins, 1024, 0, st>>>(counts, C, total);
         RQR_LAUNCH_CHECK();
-        k_sort_scatter<<<C, SORT_THREADS, smem, st>>>(seed, row0, m, (uint32_t)s1, in, out, shift, bits, T, C, counts, total);
+        k_sort_scatter<<<C, SCATTER_THREADS, smem, st>>>(seed, row0, m, (uint32_t)s1, in, out, shift, bits, T, C, counts, total);
         RQR_LAUNCH_CHECK();
         in = out;
         out = (out == entries) ? other : entries;
@@ -525,13 +533,13 @@ extern "C" int rqr_countsketch(const double* V, int64_t m, int n, int64_t ldv, i
     const int lpr = vec2 ? n / 2 : n;
     const int R = 256 / lpr > 1 ? 256 / lpr : 1;
     size_t smem = (size_t)R * n * sizeof(double);
-    // One CTA walks one bucket at a time, 148 x 8 CTAs are resident: with s1 buckets of equal expected length the
-    // pass takes ceil(s1 / 1184) rounds, i.e. it runs at (s1 / 1184) / ceil(s1 / 1184) of its speed (s1 = 2048:
-    // 1.73 / 2 = 86%; s1 = 200: 17%).  Every bucket's row list is therefore split into `split` segments, the smallest
-    // count that fills the last round to >= 95% (and the grid at all when s1 < 1184); the segment sums go to `split`
-    // partial sketches in region A of the workspace (free during A1) and are added in a fixed order.
+    // One CTA walks one bucket at a time and 148 x 8 CTAs are resident: with fewer buckets than half of that the grid
+    // is underfilled (s1 = 200: 17% of the CTA slots).  Every bucket's row list is then split into `split` segments,
+    // the smallest count that fills the last round of CTAs to >= 95%; the segment sums go to `split` partial sketches
+    // in region A of the workspace (free during A1) and are added in a fixed order.  With s1 >= 592 the pass is bound
+    // by DRAM, not by CTA slots (measured at s1 = 2048: 5.36 TB/s with or without a split), and is left alone.
     int64_t split = 1;
-    {
+    if (s1 * 2 <= 148 * 8) {
         const double slots = 148.0 * 8.0;
         const int64_t fit = (int64_t)rqr_gram_partial_cap(n) * n / s1;          // region A holds cap n^2 doubles
         const int64_t rows = m / (s1 * 4 * R);                                  // >= 4 R rows per segment
