@@ -4,7 +4,7 @@
 
 Prints one JSON line: CUDA-event time of every step called on its own (A0 sketch generation, A1 in both
 CountSketch variants, A2 with the Gaussian and with the on-the-fly Rademacher S2 (N4), A3, A4 with and without R0,
-A5, A6 stored / recomputed, A7, the one-shot with either S2), with the achieved
+A5, A6 stored / recomputed, A7, the dense Gaussian sketch of B'' and its draw alone, the one-shot with either S2), with the achieved
 GB/s or TFLOP/s of the m-sized passes against their algorithmic work.  The input is a
 plain Gaussian matrix: timings do not depend on the values.
 """
@@ -83,6 +83,11 @@ def main(argv=None):
     if n <= 64:
         t["A6_apply_recompute_V1"] = _time(lambda: rq.apply(V, R0, R1, Q, work), reps)
     t["A7_triu_mul"] = _time(lambda: rq.triu_mul(R1, R0, R), reps)
+    # B'': the single dense Gaussian sketch (s = s2 rows) and the draw of its s x m Gaussians alone
+    t["Bpp_dense_gauss_sketch"] = _time(lambda: rq.dense_gauss_sketch(V, s2, 42, W, work), max(1, reps // 3))
+    if n % 2 == 0:
+        t["Bpp_draw_only"] = _time(lambda: rq.debug_dense_gauss_draw_only(m, n, s2, 42, work), max(1, reps // 3))
+    t["Bpp_gauss_randcholqr"] = _time(lambda: rq.gauss_randcholqr(V, s2, 42, Q, R, work, info), max(1, reps // 3))
     # N4: Rademacher S2 generated on the fly (no S2 in the workspace), and the one-shot with either S2
     RAD = rq.S2_RADEMACHER
     t["one_shot_stream_variant"] = _time(lambda: rq.rand_cholqr(V, s1, s2, 42, Q, R, work, info, rq.VARIANT_STREAM, P), reps)
@@ -107,6 +112,7 @@ def main(argv=None):
         "A6_GBs": 16.0 * mn / t["A6_apply_in_place"] / 1e6,
         "A6_TFLOPs": mn * n / t["A6_apply_in_place"] / 1e9,
         "A2_TFLOPs": 2.0 * s2 * s1 * n / t["A2_gauss_sketch"] / 1e9,
+        "Bpp_sketch_TFLOPs": 2.0 * mn * s2 / t["Bpp_dense_gauss_sketch"] / 1e9,
     }
     out["info"] = int(info.item())
     print(json.dumps(out))
