@@ -154,7 +154,7 @@ def config_dict(args, c, name, v1_mode):
 def v1_mode_of(args, n):
     if args.v1 != "auto":
         return args.v1 + "d" if args.v1 == "store" else "recomputed"
-    return "recomputed (auto, n <= 16)" if n <= 16 else "stored (auto, n > 16)"
+    return "recomputed (auto, n <= 24)" if n <= 24 else "stored (auto, n > 24)"
 
 
 # ------------------------------------------------------------------------------------------
@@ -346,7 +346,7 @@ def run_config(torch, rq, name, args, peaks, p64, want_e2e=True, want_breakdown=
     bufs = rdist.alloc_bufs(rq, m, n, s1, s2, "cuda")
     work, info = bufs["work"], bufs["info"]
     v1f = {"auto": 0, "store": rq.FLAG_STORE_V1, "recompute": rq.FLAG_RECOMPUTE_V1}[args.v1]
-    recompute = (n <= 64) and (args.v1 == "recompute" or (args.v1 == "auto" and n <= 16))
+    recompute = (n <= 64) and (args.v1 == "recompute" or (args.v1 == "auto" and n <= 24))
     flags = rq.FLAG_PREPARED | v1f
 
     def prep():
@@ -528,6 +528,8 @@ def main():
     sharded = world > 1 or args.force_sharded
     if sharded:
         import torch.distributed as dist
+        if os.environ.get("NCCL_DEBUG", "").upper() in ("", "VERSION"):
+            os.environ["NCCL_DEBUG"] = "WARN"       # "NCCL version ..." goes to stdout: keep stdout to the one JSON line
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         os.environ.setdefault("MASTER_PORT", "29533")
         os.environ.setdefault("RANK", "0")

@@ -81,9 +81,9 @@ extern "C" {
                                  traffic instead of 40mn, 4mn^2 flops instead of 3mn^2).
                                  Honoured for n <= 64; for n > 64 V1 is always stored.       */
 #define RQR_FLAG_STORE_V1 4   /* one-shot drivers: store V1 into Q in A4 and transform it in place in A6.
-                                 With neither flag the drivers choose per n: recomputed for n <= 16 (the
+                                 With neither flag the drivers choose per n: recomputed for n <= 24 (the
                                  path is HBM-bound there and moves 32mn instead of 40mn bytes), stored above
-                                 (measured: from n = 24 up A4 is bound by the FP64 tensor pipe with or without
+                                 (measured: from n = 32 up A4 is bound by the FP64 tensor pipe with or without
                                  the store, and the extra mn^2 flops of A6 do not hide).  When V and
                                  Q would not take the same kernel family (Q not 16-byte aligned while V is,
                                  even n) V1 is stored whatever the flags say: a V1 re-formed by different

@@ -11,7 +11,7 @@ PROBE_DIR = os.path.join(HERE, "bench_probe")
 PROBE_LIB = os.path.join(HERE, "librqr_probe.so")       # bench-only FP64 peak probe, not part of librqr.so
 SOURCES = ["rqr_sketch.cu", "rqr_gauss_mma.cu", "rqr_dense_mma.cu", "rqr_small.cu", "rqr_tall.cu", "rqr_tall_mma.cu", "rqr_tall_panel.cu", "rqr_api.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
+              "-Xcompiler", "-fPIC", "-Xptxas", "-v"] + os.environ.get("RQR_EXTRA_NVCC_FLAGS", "").split()
 
 
 def _stale() -> bool:

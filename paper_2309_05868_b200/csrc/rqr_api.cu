@@ -46,14 +46,14 @@ static int check_common(const double* V, int64_t m, int n, double* Q, double* R,
 
 // V1 = V R0^-1 stored or recomputed (PAPER.md:220-222 flop terms; reading S20).  Stored: A4 writes V1
 // into Q and A6 transforms it in place: 40mn bytes, 3mn^2 flops.  Recomputed: A4 stores nothing and A6 re-forms V1
-// with the bit-identical routine: 32mn bytes, 4mn^2 flops.  Measured (profiles/r2_v1_mode.md): with 8 x 8 tiles A4
-// executes NB (NB + 1) DMMA per 8 rows for the substitution and as many for the Gram, so it is already bound by the
-// FP64 tensor pipe at n = 32 (0.36 ms at 2^22 x 32 with or without the store: the 8mn-byte write hides under it),
-// and the second substitution in A6 is not free from n = 24 up.  Recomputing wins only for n <= 16 (2^22 x 16: 0.542
-// vs 0.569 ms), ties at n = 24 and loses above (n = 32: 0.994 vs 0.972; n = 40: 1.43 vs 1.31; n = 64: 2.82 vs 2.41).
+// with the bit-identical routine: 32mn bytes, 4mn^2 flops.  Measured (profiles/r2_summary.md sections 3 and 9): with
+// 8 x 8 tiles A4 executes NB (NB + 1) DMMA per 8 rows for the substitution and as many for the Gram, so from n = 32 up
+// it is bound by the FP64 tensor pipe with or without the store (0.343 vs 0.348 ms at 2^22 x 32), and the second
+// substitution in A6 costs more than the store saves from n = 40 up.  Recomputing wins for n <= 24 (10^7 x 16: A4 + A6
+// 0.76 vs 0.90 ms; 10^7 x 24: 1.13 vs 1.23), ties at 32 and loses above (n = 40: 0.98 vs 0.91; n = 64: 2.82 vs 2.41).
 // Default: "recompute iff n <= RQR_AUTO_RECOMPUTE_MAX_N"; RQR_FLAG_RECOMPUTE_V1 / RQR_FLAG_STORE_V1 override it.
 // Every driver (CholeskyQR2 and sCholQR3 included) takes the same decision: the comparison stays on the same kernels.
-#define RQR_AUTO_RECOMPUTE_MAX_N 16
+#define RQR_AUTO_RECOMPUTE_MAX_N 24
 static bool use_recompute(const double* V, int n, const double* R0, const double* Q, int flags)
 {
     if (!R0 || n > 64) return false;      // n > 64: A4 is FP64-bound either way and V1 is always stored

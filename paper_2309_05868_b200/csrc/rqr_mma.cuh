@@ -320,15 +320,21 @@ struct WarpRing {
     const double* V;
     int64_t ldv, m;
     int n;
+    int ld = LD;          // landing row stride: LD (padded rows, one bulk copy per row) or n (BLOCK mode: ldv == n,
+                          // the 8 rows are contiguous in memory and land packed with ONE bulk copy; stage stride stays 8 LD)
 
     __device__ __forceinline__ void issue(int stage, int64_t rblk, int lane) const
     {
-        // rows 8*rblk .. 8*rblk+7; lane i < 8 copies row i (8n bytes) into its padded slot
+        // rows 8*rblk .. 8*rblk+7
         const int64_t row = rblk * 8 + lane;
         const int valid = (int)((m - rblk * 8) < 8 ? (m - rblk * 8) : 8);
         if (lane == 0) mbar_expect_tx(bar + stage, (uint32_t)(valid * n * 8));
         __syncwarp();
-        if (lane < valid) bulk_g2s(buf + (stage * 8 + lane) * LD, V + row * ldv, (uint32_t)(n * 8), bar + stage);
+        if (ld != LD) {       // BLOCK mode: narrow rows are bound by the NUMBER of bulk copies, not by their bytes
+            if (lane == 0) bulk_g2s(buf + stage * 8 * LD, V + rblk * 8 * ldv, (uint32_t)(valid * n * 8), bar + stage);
+        } else if (lane < valid) {                    // lane i < 8 copies row i (8n bytes) into its padded slot
+            bulk_g2s(buf + (stage * 8 + lane) * LD, V + row * ldv, (uint32_t)(n * 8), bar + stage);
+        }
     }
 };
 
@@ -356,15 +362,23 @@ struct SmemPlan {
     static constexpr size_t bytes = total_doubles * sizeof(double);
 };
 
-// load the C fragments of a landing row-block (row stride LDL)
+// load the C fragments of a landing row-block (row stride ld).  ld == LDL: rows are padded with zeros up to 8 NB
+// columns.  BLOCK mode (ld == n < LDL, rows packed): the columns past n of the last block hold the next row's data and
+// are masked with the lane's column mask (col_mask()).
 template <int NB, int LDL>
-__device__ __forceinline__ void load_acc(double (&acc)[NB][2], const double* __restrict__ rb, int lane)
+__device__ __forceinline__ void load_acc(double (&acc)[NB][2], const double* __restrict__ rb, int lane, int ld = LDL,
+                                         uint32_t colmask = 0xffffffffu)
 {
     const int r = lane >> 2, q = lane & 3;
+    const double* p = rb + r * ld + 2 * q;
 #pragma unroll
     for (int J = 0; J < NB; ++J) {
-        double2 v = *reinterpret_cast<const double2*>(rb + r * LDL + 8 * J + 2 * q);
+        double2 v = *reinterpret_cast<const double2*>(p + 8 * J);
         acc[J][0] = v.x; acc[J][1] = v.y;
+    }
+    if (ld != LDL && ld != 8 * NB) {                  // packed rows narrower than the column blocks: mask the last block
+        if (!((colmask >> (2 * (NB - 1) + 1)) & 1u)) acc[NB - 1][0] = 0.0;
+        if (!((colmask >> (2 * (NB - 1))) & 1u)) acc[NB - 1][1] = 0.0;
     }
 }
 

@@ -36,7 +36,7 @@ template <int NB, bool HAS_R, bool FULL>
 __global__ void __launch_bounds__(GramWarps<NB>::value * 32, 1)
 k_trsm_gram_mma(const double* V, int64_t m, int n, int64_t ldv,          // V1 == V allowed: no restrict on either
                 const double* __restrict__ R0, double* V1, int64_t ldq,
-                double* __restrict__ part)
+                double* __restrict__ part, int land_ld)
 {
     using Plan = SmemPlan<NB, GramWarps<NB>::value, GRAM_STAGES, 1, 2>;
     constexpr int LDL = Plan::LDL, N8 = Plan::N8;
@@ -60,7 +60,7 @@ k_trsm_gram_mma(const double* V, int64_t m, int n, int64_t ldv,          // V1 =
     fence_proxy_async();
     __syncthreads();
 
-    WarpRing<LDL> wr{ring + (size_t)warp * GRAM_STAGES * 8 * LDL, bars + warp * GRAM_STAGES, V, ldv, m, n};
+    WarpRing<LDL> wr{ring + (size_t)warp * GRAM_STAGES * 8 * LDL, bars + warp * GRAM_STAGES, V, ldv, m, n, land_ld};
     const XsAddr<N8> ad(lane);
     const int64_t nrb = (m + 7) / 8;
     const int64_t gw = (int64_t)blockIdx.x * GramWarps<NB>::value + warp;
@@ -84,10 +84,10 @@ k_trsm_gram_mma(const double* V, int64_t m, int n, int64_t ldv,          // V1 =
         double* rb = wr.buf + stage * 8 * LDL;
         const int valid = (int)((m - rblk * 8) < 8 ? (m - rblk * 8) : 8);
         if (valid < 8) {
-            for (int e = lane; e < (8 - valid) * LDL; e += 32) rb[valid * LDL + e] = 0.0;
+            for (int e = lane; e < (8 - valid) * wr.ld; e += 32) rb[valid * wr.ld + e] = 0.0;
             __syncwarp();
         }
-        load_acc<NB, LDL>(acc, rb, lane);
+        load_acc<NB, LDL>(acc, rb, lane, wr.ld, colmask);
         // refill of the landing block once its values have been consumed (registers -> DMMA / xs)
         auto refill = [&]() {
             const int64_t next = rblk + (int64_t)GRAM_STAGES * stride;
@@ -363,7 +363,7 @@ template <int NB, bool TWO, bool FULL>
 __global__ void __launch_bounds__(ApplyCfg<NB, TWO>::WARPS * 32, 1)
 k_apply_mma(const double* V, int64_t m, int n, int64_t ldv,              // Q == V allowed: no restrict on either
             const double* __restrict__ R0, const double* __restrict__ R1,
-            double* Q, int64_t ldq)
+            double* Q, int64_t ldq, int land_ld)
 {
     using Plan = SmemPlan<NB, ApplyCfg<NB, TWO>::WARPS, ApplyCfg<NB, TWO>::STAGES, 2, 0>;
     constexpr int LDL = Plan::LDL, N8 = Plan::N8;
@@ -388,7 +388,7 @@ k_apply_mma(const double* V, int64_t m, int n, int64_t ldv,              // Q ==
     fence_proxy_async();
     __syncthreads();
 
-    WarpRing<LDL> wr{ring + (size_t)warp * ApplyCfg<NB, TWO>::STAGES * 8 * LDL, bars + warp * ApplyCfg<NB, TWO>::STAGES, V, ldv, m, n};
+    WarpRing<LDL> wr{ring + (size_t)warp * ApplyCfg<NB, TWO>::STAGES * 8 * LDL, bars + warp * ApplyCfg<NB, TWO>::STAGES, V, ldv, m, n, land_ld};
     const XsAddr<N8> ad(lane);
     const int64_t nrb = (m + 7) / 8;
     const int64_t gw = (int64_t)blockIdx.x * ApplyCfg<NB, TWO>::WARPS + warp;
@@ -408,10 +408,10 @@ k_apply_mma(const double* V, int64_t m, int n, int64_t ldv,              // Q ==
         double* rb = wr.buf + stage * 8 * LDL;
         const int valid = (int)((m - rblk * 8) < 8 ? (m - rblk * 8) : 8);
         if (valid < 8) {
-            for (int e = lane; e < (8 - valid) * LDL; e += 32) rb[valid * LDL + e] = 0.0;
+            for (int e = lane; e < (8 - valid) * wr.ld; e += 32) rb[valid * wr.ld + e] = 0.0;
             __syncwarp();
         }
-        load_acc<NB, LDL>(acc, rb, lane);
+        load_acc<NB, LDL>(acc, rb, lane, wr.ld, colmask);
         auto refill = [&]() {
             const int64_t next = rblk + (int64_t)ApplyCfg<NB, TWO>::STAGES * stride;
             if (next < nrb) {
@@ -443,6 +443,27 @@ static bool fast_ok(const void* V, int n, int64_t ldv, const void* Q, int64_t ld
     return true;
 }
 
+#ifndef RQR_BLOCK_GRAM_MAX_NB
+#define RQR_BLOCK_GRAM_MAX_NB 8
+#endif
+// BLOCK mode of the landing ring (rqr_mma.cuh WarpRing): ONE bulk copy per 8-row block instead of one per row, when the
+// rows are contiguous (ldv == n).  Narrow rows are bound by the number of bulk copies, not by their bytes: measured
+// (profiles/r2_summary.md section 9, 10^7 x 10..24 and 2^22 x 32..56) the plain Gram gains 10-30% at every n, A4 with R0
+// 5-15% (not at 16 < n <= 24 when it also stores V1), the two-pass apply 5-20%, the in-place apply only for n <= 24 (it
+// loses 12-15% for n >= 40).  kind: 1 = plain Gram (no R0), 2 = A4 with R0, 4 = A6.
+#ifndef RQR_BLOCK_MODE
+#define RQR_BLOCK_MODE 7
+#endif
+template <int NB>
+static int landing_ld(int n, int64_t ldv, int kind, bool stores_v1_or_two_pass)
+{
+    bool block = ldv == n && (RQR_BLOCK_MODE & kind);
+    if (kind == 1) block = block && NB <= RQR_BLOCK_GRAM_MAX_NB;
+    if (kind == 2 && stores_v1_or_two_pass && NB == 3) block = false;
+    if (kind == 4 && !stores_v1_or_two_pass && NB > 3) block = false;
+    return block ? n : TallCfg<NB>::LDL;
+}
+
 static int grid_for(int64_t m, int warps)
 {
     int64_t nrb = (m + 7) / 8;
@@ -463,9 +484,10 @@ static int launch_trsm_gram(const double* V, int64_t m, int n, int64_t ldv, cons
     });
     const int grid = grid_for(m, GramWarps<NB>::value);
     *nparts = grid;
-    if (R0 && n == 8 * NB) k_trsm_gram_mma<NB, true, true><<<grid, GramWarps<NB>::value * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, V1, ldq, part);
-    else if (R0)           k_trsm_gram_mma<NB, true, false><<<grid, GramWarps<NB>::value * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, V1, ldq, part);
-    else                   k_trsm_gram_mma<NB, false, false><<<grid, GramWarps<NB>::value * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, nullptr, ldq, part);
+    const int lld = landing_ld<NB>(n, ldv, R0 ? 2 : 1, V1 != nullptr);
+    if (R0 && n == 8 * NB) k_trsm_gram_mma<NB, true, true><<<grid, GramWarps<NB>::value * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, V1, ldq, part, lld);
+    else if (R0)           k_trsm_gram_mma<NB, true, false><<<grid, GramWarps<NB>::value * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, V1, ldq, part, lld);
+    else                   k_trsm_gram_mma<NB, false, false><<<grid, GramWarps<NB>::value * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, nullptr, ldq, part, lld);
     RQR_LAUNCH_CHECK();
     return RQR_OK;
 }
@@ -522,8 +544,9 @@ static int launch_apply_mode(const double* V, int64_t m, int n, int64_t ldv, con
         cudaFuncSetAttribute(k_apply_mma<NB, TWO, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
     });
     const int grid = grid_for(m, W);
-    if (n == 8 * NB) k_apply_mma<NB, TWO, true><<<grid, W * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, R1, Q, ldq);
-    else             k_apply_mma<NB, TWO, false><<<grid, W * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, R1, Q, ldq);
+    const int lld = landing_ld<NB>(n, ldv, 4, TWO);
+    if (n == 8 * NB) k_apply_mma<NB, TWO, true><<<grid, W * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, R1, Q, ldq, lld);
+    else             k_apply_mma<NB, TWO, false><<<grid, W * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, R1, Q, ldq, lld);
     RQR_LAUNCH_CHECK();
     return RQR_OK;
 }
