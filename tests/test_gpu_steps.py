@@ -231,6 +231,36 @@ def test_apply_parity_and_bit_identical_recompute(rq, orc, m, n, generic):
         rq.force_generic(False)
 
 
+@pytest.mark.parametrize("m,n,pad", [(5003, 20, 4), (4099, 32, 2), (3001, 64, 8), (2500, 100, 6), (777, 10, 2)])
+def test_strided_V_and_Q_take_the_per_row_staging(rq, orc, m, n, pad):
+    """ld > n: the rows of an 8-row block are not contiguous, so the DMMA kernels stage them with one bulk copy per row
+    (ld = n takes the one-copy-per-block mode, covered by the shapes above); both must give the oracle's X and G, and
+    the same bits as the contiguous call."""
+    V = inputs.make_V(m, n, 1e3, 13)
+    R0 = inputs.make_upper(n, 5).cuda(); R1 = inputs.make_upper(n, 7).cuda()
+    big = torch.zeros(m, n + pad, dtype=torch.float64, device="cuda")
+    big[:, :n] = V.cuda()
+    Vs = big[:, :n]                                   # ldv = n + pad
+    qbig = torch.full((m, n + pad), float("nan"), dtype=torch.float64, device="cuda")
+    Qs = qbig[:, :n]
+    G = torch.empty(n, n, dtype=torch.float64, device="cuda")
+    Gc = torch.empty_like(G)
+    work = rq.alloc_workspace(m, n, max(n, 2), 2)
+    rq.trsm_gram(Vs, R0, G, Qs, work)
+    Vc = V.cuda(); X = torch.empty_like(Vc)
+    rq.trsm_gram(Vc, R0, Gc, X, work)
+    assert torch.equal(Qs, X) and torch.equal(G, Gc)
+    assert bool(torch.isnan(qbig[:, n:]).all())       # nothing written past the n columns
+    Xo = orc.trsm(V.numpy(), host(R0))
+    assert np.abs(host(X) - Xo).max() <= 1e-12 * np.abs(Xo).max()
+    rq.apply(Qs, None, R1, Qs, work)                  # in place, strided
+    Qc = torch.empty_like(Vc)
+    rq.apply(X, None, R1, Qc, work)
+    assert torch.equal(Qs, Qc)
+    rq.apply(Vs, R0, R1, Qs, work)                    # two-pass from the strided V
+    assert torch.equal(Qs, Qc)
+
+
 def test_trsm_rowwise_backward_error_with_graded_R(rq):
     # eq. (42), PAPER.md:449-453: each row solves x (R + dR) = v with |dR| <= c n u |R|.
     # R0 = R factor of a column-graded matrix (12 decades), as randQR meets at kappa = 1e12.
