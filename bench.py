@@ -528,8 +528,8 @@ def main():
     sharded = world > 1 or args.force_sharded
     if sharded:
         import torch.distributed as dist
-        if os.environ.get("NCCL_DEBUG", "").upper() in ("", "VERSION"):
-            os.environ["NCCL_DEBUG"] = "WARN"       # "NCCL version ..." goes to stdout: keep stdout to the one JSON line
+        # NCCL writes its "NCCL version ..." / debug lines to stdout: send them to stderr, stdout is the one JSON line
+        os.environ.setdefault("NCCL_DEBUG_FILE", "/dev/stderr")
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         os.environ.setdefault("MASTER_PORT", "29533")
         os.environ.setdefault("RANK", "0")
