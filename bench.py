@@ -240,6 +240,30 @@ def median(v):
     return s[k // 2] if k % 2 else 0.5 * (s[k // 2 - 1] + s[k // 2])
 
 
+def gpu_energy_mj(index=0):
+    """Total energy counter of the board (NVML, millijoules) or None."""
+    try:
+        import pynvml
+        pynvml.nvmlInit()
+        return pynvml.nvmlDeviceGetTotalEnergyConsumption(pynvml.nvmlDeviceGetHandleByIndex(index))
+    except Exception:
+        return None
+
+
+def probe_hbm_sustained(torch, seconds=1.0):
+    """Sustained device copy bandwidth (GB/s, read + write bytes) over >= `seconds` of back-to-back copies of 2 GiB:
+    what the HBM delivers once the board sits at its power cap (MEASURED_PEAKS.json holds the burst figure)."""
+    a = torch.empty(1 << 28, dtype=torch.float64, device="cuda")
+    b = torch.empty_like(a)
+    b.copy_(a)
+    ms1 = time_region(torch, lambda: b.copy_(a), 3) / 3
+    reps = max(3, int(seconds * 1e3 / ms1))
+    ms = time_region(torch, lambda: b.copy_(a), reps) / reps
+    del a, b
+    torch.cuda.empty_cache()
+    return 2.0 * (1 << 28) * 8 / ms / 1e6
+
+
 def probe_fp64_peak(torch):
     """Measured FP64 peak (TFLOP/s): best of a DFMA chain and a DMMA chain, >= 0.25 s each."""
     from paper_2309_05868_b200 import bench_probe as probe
@@ -372,7 +396,9 @@ def run_config(torch, rq, name, args, peaks, p64, want_e2e=True, want_breakdown=
         timed_step = graph.replay
         for _ in range(2):
             timed_step()
+    en0 = gpu_energy_mj(torch.cuda.current_device())
     total_ms, per = time_steps(torch, timed_step, steps, barrier)
+    en1 = gpu_energy_mj(torch.cuda.current_device())
     ms_med, ms_mean = median(per), total_ms / steps
     if barrier:                                     # every rank reports the slowest rank's figures
         import torch.distributed as dist
@@ -415,6 +441,10 @@ def run_config(torch, rq, name, args, peaks, p64, want_e2e=True, want_breakdown=
            "orth_err_worst_of_seeds": worst_orth, "resid_worst_of_seeds": worst_res,
            "sketch_seeds": list(inputs.SKETCH_SEEDS), "v1": "recomputed" if recompute else "stored",
            "sketch_gen_ms": t_prep, "ms_with_sketch_gen": ms_med + t_prep}
+    if en0 is not None and en1 is not None and total_ms > 0:
+        # the board's energy counter over the timed region: the path runs AT the 1 kW power cap
+        out["energy_j_per_step"] = (en1 - en0) / 1e3 / steps
+        out["power_w_avg_timed_region"] = (en1 - en0) / total_ms
     if shard is None or world == 1:
         # comparator on the same kernels, same V (CholeskyQR2, Alg. 4): same V1 policy, same timing method
         def step_c2():
@@ -543,6 +573,7 @@ def main():
     p64s = {"dfma": 34.2, "dmma": 37.2, "note": "not probed in this run"} if args.no_probe else probe_fp64_peak(torch)
     ratio_peak = (peaks["bf16_tflops"] or 1590.0) * (45.0 / 2250.0)   # guide's nominal FP64:bf16 ratio
     p64 = max(p64s["dfma"], p64s["dmma"], 1e-3)
+    hbm_sustained = None if args.no_probe else probe_hbm_sustained(torch)
     c = inputs.config(args.workload)
     m, n = c["m"], c["n"]
     shard = (world, rank, rank * m) if sharded else None
@@ -615,7 +646,15 @@ def main():
             "sketch_gen_ms": main_out["sketch_gen_ms"], "ms_with_sketch_gen": main_out["ms_with_sketch_gen"],
             "breakdown_ms": bd, "fp64_peak_tflops": p64s, "e2e": main_out.get("e2e"),
             "gpu_launches": nl * args.steps * world, "roofline": roof, "cpu_baseline": cpu,
-            "cpu_baseline_other_configs": cpu_other or None, "clocks": clocks, "extra": extra}
+            "cpu_baseline_other_configs": cpu_other or None, "clocks": clocks,
+            # the path runs at the board's power cap: energy counter over the timed region, and the
+            # sustained device-copy bandwidth (1 s loop) beside the burst figure of MEASURED_PEAKS.json
+            "power": {"energy_j_per_step": main_out.get("energy_j_per_step"),
+                      "power_w_avg_timed_region": main_out.get("power_w_avg_timed_region"),
+                      "hbm_sustained_gbs": hbm_sustained, "hbm_burst_gbs": peaks["hbm_gbs"],
+                      "note": "every m-sized kernel of the step runs at the 1 kW cap (sw_power_cap): the burst peaks of the "
+                              "roofline (FP64 probe at ~600 W, device copy) are not reachable together under it"},
+            "extra": extra}
     if sharded:
         line["config"].update({"m_per_gpu": m, "m_total": m * world,
                                "parallelism": "row-sharded, 2 all-reduces (W, G) per step"})

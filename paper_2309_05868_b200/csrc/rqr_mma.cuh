@@ -312,6 +312,51 @@ __device__ __forceinline__ void trsm_rowblock_gf(double (&acc)[NB][2], double* _
     if constexpr (XS) __syncwarp();
 }
 
+// Two row-blocks through the same triangular factor at once (A6): every B fragment (T_J, -R[J,J']) is read from
+// shared memory ONCE for both, and the warp carries two independent substitution chains, so a dependent DMMA of one
+// chain issues in the shadow of the other's.  The arithmetic on each row-block is the instruction sequence of
+// trsm_rowblock (H1: same bits); which blocks are paired does not enter it.
+template <int NB, bool FULL, class Hook>
+__device__ __forceinline__ void trsm_rowblock_x2(double (&accA)[NB][2], double (&accB)[NB][2],
+                                                 const double* __restrict__ Tf, const double* __restrict__ nRf,
+                                                 double* __restrict__ gpA, double* __restrict__ gpB, uint32_t colmask,
+                                                 int lane, Hook&& after_first)
+{
+    static_for<0, NB>([&](auto Jc) {
+        constexpr int J = decltype(Jc)::value;
+        double xa0 = 0.0, xa1 = 0.0, xb0 = 0.0, xb1 = 0.0;
+        const double t0 = Tf[J * 64 + lane];
+        dmma(xa0, xa1, accA[J][0], t0);
+        dmma(xb0, xb1, accB[J][0], t0);
+        const double t1 = Tf[J * 64 + 32 + lane];
+        dmma(xa0, xa1, accA[J][1], t1);
+        dmma(xb0, xb1, accB[J][1], t1);
+#pragma unroll
+        for (int Jp = J + 1; Jp < NB; ++Jp) {
+            const double r0 = nRf[TriFrags<NB>::pair(J, Jp) * 64 + lane];
+            dmma(accA[Jp][0], accA[Jp][1], xa0, r0);
+            dmma(accB[Jp][0], accB[Jp][1], xb0, r0);
+        }
+#pragma unroll
+        for (int Jp = J + 1; Jp < NB; ++Jp) {
+            const double r1 = nRf[TriFrags<NB>::pair(J, Jp) * 64 + 32 + lane];
+            dmma(accA[Jp][0], accA[Jp][1], xa1, r1);
+            dmma(accB[Jp][0], accB[Jp][1], xb1, r1);
+        }
+        accA[J][0] = xa0; accA[J][1] = xa1;
+        accB[J][0] = xb0; accB[J][1] = xb1;
+        if constexpr (J == 0) after_first();
+        if (gpA != nullptr) {
+            if (FULL || ((colmask >> (2 * J)) & 1u)) *reinterpret_cast<double2*>(gpA + 8 * J) = make_double2(xa0, xa1);
+            else if ((colmask >> (2 * J + 1)) & 1u) gpA[8 * J] = xa0;
+        }
+        if (gpB != nullptr) {
+            if (FULL || ((colmask >> (2 * J)) & 1u)) *reinterpret_cast<double2*>(gpB + 8 * J) = make_double2(xb0, xb1);
+            else if ((colmask >> (2 * J + 1)) & 1u) gpB[8 * J] = xb0;
+        }
+    });
+}
+
 // Per-warp ring of landing row-blocks fed by bulk async copies.
 template <int LD>
 struct WarpRing {

@@ -432,6 +432,94 @@ k_apply_mma(const double* V, int64_t m, int n, int64_t ldv,              // Q ==
     }
 }
 
+// A6 with two row-blocks per warp and iteration (trsm_rowblock_x2): half the B-fragment loads, two independent chains
+// per warp.  Ring of 4 stages = two pairs: the pair of iteration i + 1 lands while pair i is in the registers.
+#define APPLY2_WARPS 8
+#define APPLY2_STAGES 4
+template <int NB, bool TWO, bool FULL>
+__global__ void __launch_bounds__(APPLY2_WARPS * 32, 1)
+k_apply_mma2(const double* V, int64_t m, int n, int64_t ldv,             // Q == V allowed: no restrict on either
+             const double* __restrict__ R0, const double* __restrict__ R1,
+             double* Q, int64_t ldq, int land_ld)
+{
+    using Plan = SmemPlan<NB, APPLY2_WARPS, APPLY2_STAGES, 2, 0>;
+    constexpr int LDL = Plan::LDL;
+    constexpr int FD = TallCfg<NB>::FRAG_DOUBLES;
+    extern __shared__ __align__(16) double smem[];
+    double* Tf1 = smem;
+    double* nRf1 = smem + NB * 64;
+    double* Tf0 = smem + FD;
+    double* nRf0 = smem + FD + NB * 64;
+    double* scratch = smem + Plan::scratch;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + Plan::bars);
+    double* ring = smem + Plan::ring;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+
+    static_assert(Plan::ring_doubles >= 64 * NB * NB, "ring too small to stage R");
+    if (threadIdx.x < APPLY2_WARPS * APPLY2_STAGES) mbar_init(bars + threadIdx.x, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    build_tri_frags<NB>(R1, n, Tf1, nRf1, scratch, ring);
+    if (TWO) build_tri_frags<NB>(R0, n, Tf0, nRf0, scratch, ring);
+    for (int i = threadIdx.x; i < (int)Plan::ring_doubles; i += blockDim.x) ring[i] = 0.0;
+    fence_proxy_async();
+    __syncthreads();
+
+    WarpRing<LDL> wr{ring + (size_t)warp * APPLY2_STAGES * 8 * LDL, bars + warp * APPLY2_STAGES, V, ldv, m, n, land_ld};
+    const int64_t nrb = (m + 7) / 8;
+    const int64_t gw = (int64_t)blockIdx.x * APPLY2_WARPS + warp;
+    const int64_t stride = (int64_t)gridDim.x * APPLY2_WARPS;
+#pragma unroll
+    for (int s = 0; s < APPLY2_STAGES; ++s)
+        if (gw + s * stride < nrb) wr.issue(s, gw + s * stride, lane);
+    double accA[NB][2], accB[NB][2];
+    const uint32_t colmask = col_mask<NB>(n, lane);
+    const int64_t lane_off = (int64_t)(lane >> 2) * ldq + 2 * (lane & 3);
+    int stage = 0;                                   // even: the pair uses stages (stage, stage + 1)
+    uint32_t phase = 0;
+    for (int64_t rblk = gw; rblk < nrb; rblk += 2 * stride) {
+        const int64_t rblkB = rblk + stride;
+        const bool hasB = rblkB < nrb;
+        auto land = [&](int st, int64_t rb_idx, double (&acc)[NB][2]) {
+            mbar_wait(wr.bar + st, phase);
+            double* rb = wr.buf + st * 8 * LDL;
+            const int valid = (int)((m - rb_idx * 8) < 8 ? (m - rb_idx * 8) : 8);
+            if (valid < 8) {
+                for (int e = lane; e < (8 - valid) * wr.ld; e += 32) rb[valid * wr.ld + e] = 0.0;
+                __syncwarp();
+            }
+            load_acc<NB, LDL>(acc, rb, lane, wr.ld, colmask);
+            return valid;
+        };
+        const int validA = land(stage, rblk, accA);
+        int validB = 0;
+        if (hasB) validB = land(stage + 1, rblkB, accB);
+        else {
+#pragma unroll
+            for (int J = 0; J < NB; ++J) { accB[J][0] = 0.0; accB[J][1] = 0.0; }
+        }
+        auto refill = [&]() {
+            const int64_t nextA = rblk + (int64_t)APPLY2_STAGES * stride, nextB = nextA + stride;
+            if (nextA < nrb || nextB < nrb) {
+                fence_proxy_async();
+                __syncwarp();
+                if (nextA < nrb) wr.issue(stage, nextA, lane);
+                if (nextB < nrb) wr.issue(stage + 1, nextB, lane);
+            }
+        };
+        auto nohook = []() {};
+        double* gpA = ((lane >> 2) < validA) ? Q + rblk * 8 * ldq + lane_off : nullptr;
+        double* gpB = (hasB && (lane >> 2) < validB) ? Q + rblkB * 8 * ldq + lane_off : nullptr;
+        if (TWO) {
+            trsm_rowblock_x2<NB, FULL>(accA, accB, Tf0, nRf0, nullptr, nullptr, colmask, lane, refill);
+            trsm_rowblock_x2<NB, FULL>(accA, accB, Tf1, nRf1, gpA, gpB, colmask, lane, nohook);
+        } else {
+            trsm_rowblock_x2<NB, FULL>(accA, accB, Tf1, nRf1, gpA, gpB, colmask, lane, refill);
+        }
+        stage += 2;
+        if (stage == APPLY2_STAGES) { stage = 0; phase ^= 1u; }
+    }
+}
+
 // ------------------------------------------------------------------------------------------
 // host dispatch
 // ------------------------------------------------------------------------------------------
@@ -532,10 +620,35 @@ int rqr_trsm_gram_mma(const double* V, int64_t m, int n, int64_t ldv, const doub
     return launch_trsm_gram<8>(V, m, n, ldv, R0, V1, ldq, part, nparts, st);
 }
 
+#ifndef RQR_APPLY_X2
+#define RQR_APPLY_X2 1
+#endif
+template <int NB, bool TWO>
+static int launch_apply2_mode(const double* V, int64_t m, int n, int64_t ldv, const double* R0, const double* R1,
+                              double* Q, int64_t ldq, cudaStream_t st)
+{
+    using Plan = SmemPlan<NB, APPLY2_WARPS, APPLY2_STAGES, 2, 0>;
+    static_assert(Plan::bytes <= 227 * 1024, "A6 (x2) shared memory plan too large");
+    RQR_ONCE_PER_DEVICE({
+        cudaFuncSetAttribute(k_apply_mma2<NB, TWO, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
+        cudaFuncSetAttribute(k_apply_mma2<NB, TWO, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
+    });
+    const int grid = grid_for(m, 2 * APPLY2_WARPS);
+    const int lld = landing_ld<NB>(n, ldv, 4, TWO);
+    if (n == 8 * NB) k_apply_mma2<NB, TWO, true><<<grid, APPLY2_WARPS * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, R1, Q, ldq, lld);
+    else             k_apply_mma2<NB, TWO, false><<<grid, APPLY2_WARPS * 32, Plan::bytes, st>>>(V, m, n, ldv, R0, R1, Q, ldq, lld);
+    RQR_LAUNCH_CHECK();
+    return RQR_OK;
+}
+
 template <int NB, bool TWO>
 static int launch_apply_mode(const double* V, int64_t m, int n, int64_t ldv, const double* R0, const double* R1,
                              double* Q, int64_t ldq, cudaStream_t st)
 {
+    // two row-blocks per warp (k_apply_mma2): measured against the one-block kernel on the same box, in place: n = 32
+    // 0.327 vs 0.340 ms (2^22 rows), n = 64 1.42 vs 1.46-1.48 ms inside the C3 factorization (equal stand-alone); slower
+    // at n = 40 / 48 (0.548 vs 0.476 ms) and in the two-pass mode: only NB = 4 and NB = 8 in place take it
+    if (RQR_APPLY_X2 && !TWO && (NB == 4 || NB == 8)) return launch_apply2_mode<NB, TWO>(V, m, n, ldv, R0, R1, Q, ldq, st);
     constexpr int W = ApplyCfg<NB, TWO>::WARPS;
     using Plan = SmemPlan<NB, W, ApplyCfg<NB, TWO>::STAGES, 2, 0>;
     static_assert(Plan::bytes <= 227 * 1024, "A6 shared memory plan too large");
