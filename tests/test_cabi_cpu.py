@@ -73,6 +73,12 @@ def test_argument_validation_without_gpu(lib):
     assert lib.rqr_rand_cholqr_batched(one, 100, 8, 0, 800, 64, 16, 1, one, 800, one, one, z, 0, 1, z) == -4     # batch < 1
     assert lib.rqr_rand_cholqr_batched(one, 100, 8, 2, 799, 64, 16, 1, one, 800, one, one, z, 0, 1, z) == -5     # stride < m n
     assert lib.rqr_rand_cholqr_batched(z, 100, 8, 2, 800, 64, 16, 1, one, 800, one, one, z, 0, 1, z) == -1
+    # row-sharded one-shot: V m row0 m_total n s1 s2 seed Q R work info variant flags allreduce ctx stream
+    assert lib.rqr_rand_cholqr_sharded(one, 100, -1, 200, 8, 64, 16, 1, one, one, one, z, 0, 0, z, z, z) == -3      # row0 < 0
+    assert lib.rqr_rand_cholqr_sharded(one, 100, 150, 200, 8, 64, 16, 1, one, one, one, z, 0, 0, z, z, z) == -4     # past m_total
+    assert lib.rqr_rand_cholqr_sharded(one, 100, 0, 200, 8, 300, 16, 1, one, one, one, z, 0, 0, z, z, z) == -6      # s1 > m_total
+    assert lib.rqr_rand_cholqr_sharded(one, 4, 0, 200, 8, 64, 4, 1, one, one, one, z, 0, 0, z, z, z) == -7          # s2 < n (a 4-row shard is fine)
+    assert lib.rqr_rand_cholqr_sharded(z, 100, 0, 200, 8, 64, 16, 1, one, one, one, z, 0, 0, z, z, z) == -1
     assert lib.rqr_debug_rademacher(1, 100, 2000, 0, 10, one, z) == -3                                          # row
     assert lib.rqr_debug_rademacher(1, 100, 3, 95, 10, one, z) == -4                                            # past s1
     # the Rademacher S2 needs no S2 slot: 8 * 1024 * ld bytes less
