@@ -648,7 +648,7 @@ static int launch_apply_mode(const double* V, int64_t m, int n, int64_t ldv, con
     // two row-blocks per warp (k_apply_mma2): measured against the one-block kernel on the same box, in place: n = 32
     // 0.327 vs 0.340 ms (2^22 rows), n = 64 1.42 vs 1.46-1.48 ms inside the C3 factorization (equal stand-alone); slower
     // at n = 40 / 48 (0.548 vs 0.476 ms) and in the two-pass mode: only NB = 4 and NB = 8 in place take it
-    if (RQR_APPLY_X2 && !TWO && (NB == 4 || NB == 8)) return launch_apply2_mode<NB, TWO>(V, m, n, ldv, R0, R1, Q, ldq, st);
+    if constexpr (RQR_APPLY_X2 && !TWO && (NB == 4 || NB == 8)) return launch_apply2_mode<NB, TWO>(V, m, n, ldv, R0, R1, Q, ldq, st);
     constexpr int W = ApplyCfg<NB, TWO>::WARPS;
     using Plan = SmemPlan<NB, W, ApplyCfg<NB, TWO>::STAGES, 2, 0>;
     static_assert(Plan::bytes <= 227 * 1024, "A6 shared memory plan too large");
