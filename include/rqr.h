@@ -138,6 +138,32 @@ int rqr_small_geqrf(double* W, int s2, int n, double* R0, int* d_info, void* str
 int rqr_trsm_gram(const double* V, int64_t m, int n, int64_t ldv, const double* R0, double* G,
                   double* V1, int64_t ldq, void* work, void* stream);
 
+/* A4 for callers that cannot allocate or carry a workspace (code under CUDA-graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): the same operation and the same kernels as rqr_trsm_gram (Alg. 1 step 3 +
+ * Alg. 2 step 1), with NO `work` argument.  The per-CTA Gram partials (the only scratch A4
+ * needs for n <= 64) live in a file-scope `static __device__` array inside the library:
+ *     RQR_NOALLOC_MAX_PARTIALS x RQR_NOALLOC_MAX_N^2 doubles = 148 x 64 x 64 x 8 = 4 849 664 bytes,
+ * held by every GPU that loads librqr.so until the process exits.  The call performs no cudaMalloc / cudaFree and
+ * calls no allocating routine; the first call on each device looks the array's device address up once
+ * (cudaGetSymbolAddress, with that device current) and sets the kernels' shared-memory attributes -- make that
+ * first call outside stream capture.
+ *  - Limits: 2 <= n <= RQR_NOALLOC_MAX_N (64) and 1 <= m <= RQR_NOALLOC_MAX_M (2^23 rows, one accumulation chunk).
+ *    A shape beyond either returns RQR_ERR_SCRATCH_LIMIT and launches nothing.  Other arguments as rqr_trsm_gram
+ *    (return -k for argument k of THIS signature).
+ *  - Results: on the DMMA path (even n, even ld, 16-byte aligned bases) G and V1 are bit-identical to
+ *    rqr_trsm_gram's; on the generic path the partial count is capped at 148 (rqr_trsm_gram: 304), so G agrees to
+ *    rounding (1e-13 relative), V1 bit for bit.
+ *  - The array is SHARED by every call on a device and keeps the last call's contents.  Nothing in it has to
+ *    start at zero: each launch overwrites the partials it reads back (CTA p writes partial p in full before the
+ *    reduction reads partials 0 .. grid-1).  Two calls that overlap on the GPU (different streams, or concurrent
+ *    graph branches) RACE on it: serialise them, or use rqr_trsm_gram with one workspace per stream.            */
+#define RQR_ERR_SCRATCH_LIMIT (-1002)
+#define RQR_NOALLOC_MAX_N 64
+#define RQR_NOALLOC_MAX_M ((int64_t)1 << 23)
+#define RQR_NOALLOC_MAX_PARTIALS 148
+int rqr_trsm_gram_noalloc(const double* V, int64_t m, int n, int64_t ldv, const double* R0, double* G,
+                          double* V1, int64_t ldq, void* stream);
+
 /* A5 -- upper Cholesky factor, G + shift I = R1^T R1 (Alg. 2 step 2).  R1 is n x n
  * upper triangular with diag > 0 and exact zeros below; it must not alias G (for n > 128 the part
  * of R1 that ends up zero is scratch during the call: inverse diagonal blocks and the Schur

@@ -26,6 +26,9 @@ FLAG_STORE_V1 = 4
 S2_RADEMACHER = 16          # OR into `variant` (workspace, prepare, countsketch, rand_cholqr) / `flags` (gauss_sketch)
 MAX_N = 256                 # argument limits of include/rqr.h
 MAX_S2 = 1024
+ERR_SCRATCH_LIMIT = -1002   # rqr_trsm_gram_noalloc: shape beyond its built-in scratch
+NOALLOC_MAX_N = 64
+NOALLOC_MAX_M = 1 << 23
 
 _i64, _u64, _u32, _int, _dbl, _vp, _sz = (ctypes.c_int64, ctypes.c_uint64, ctypes.c_uint32, ctypes.c_int,
                                           ctypes.c_double, ctypes.c_void_p, ctypes.c_size_t)
@@ -38,6 +41,7 @@ SIGNATURES = {
     "rqr_gauss_sketch": (_int, [_vp, _i64, _int, _int, _u64, _vp, _vp, _int, _vp]),
     "rqr_small_geqrf": (_int, [_vp, _int, _int, _vp, _vp, _vp]),
     "rqr_trsm_gram": (_int, [_vp, _i64, _int, _i64, _vp, _vp, _vp, _i64, _vp, _vp]),
+    "rqr_trsm_gram_noalloc": (_int, [_vp, _i64, _int, _i64, _vp, _vp, _vp, _i64, _vp]),
     "rqr_chol": (_int, [_vp, _int, _dbl, _vp, _vp, _vp]),
     "rqr_apply": (_int, [_vp, _i64, _int, _i64, _vp, _vp, _vp, _i64, _vp, _vp]),
     "rqr_triu_mul": (_int, [_vp, _vp, _int, _vp, _vp]),
@@ -158,6 +162,19 @@ def trsm_gram(V, R0, G, V1, work):
     ldq = V1.stride(0) if V1 is not None else n
     f = lib().rqr_debug_trsm_gram_generic if _force_generic else lib().rqr_trsm_gram
     _chk(f(_ptr(V), m, n, V.stride(0), _ptr(R0), _ptr(G), _ptr(V1), ldq, _ptr(work), _stream()), "rqr_trsm_gram")
+
+
+def trsm_gram_noalloc(V, R0, G, V1):
+    """rqr_trsm_gram without a workspace: the Gram partials live in the library's own static device array
+    (n <= 64, m <= 2^23; calls that overlap on the GPU race on it).  Allocates nothing."""
+    _f64(V, "V"); _f64(G, "G")
+    m, n = V.shape
+    ldq = V1.stride(0) if V1 is not None else n
+    rc = lib().rqr_trsm_gram_noalloc(_ptr(V), m, n, V.stride(0), _ptr(R0), _ptr(G), _ptr(V1), ldq, _stream())
+    if rc == ERR_SCRATCH_LIMIT:
+        raise RqrError("rqr_trsm_gram_noalloc: shape %d x %d is beyond the built-in scratch (n <= %d, m <= %d); "
+                       "use rqr_trsm_gram with a workspace" % (m, n, NOALLOC_MAX_N, NOALLOC_MAX_M))
+    _chk(rc, "rqr_trsm_gram_noalloc")
 
 
 def chol(G, R1, info=None, shift=0.0):

@@ -232,3 +232,61 @@ extern "C" int rqr_debug_apply_generic(const double* V, int64_t m, int n, int64_
 {
     return apply_impl(V, m, n, ldv, R0, R1, Q, ldq, work, stream, true);
 }
+
+// ---------------------------------------------------------------------------------------
+// rqr_trsm_gram_noalloc: A4 with the Gram partials in a file-scope device array instead of the caller's workspace
+// (include/rqr.h).  One array per device that loads the library, shared by every call: calls that overlap on the
+// GPU race on it.  Nothing in it must start at zero: CTA p overwrites partial p before k_gram_reduce reads it.
+// ---------------------------------------------------------------------------------------
+static __device__ __align__(256) double d_noalloc_gram_part[(size_t)RQR_NOALLOC_MAX_PARTIALS * RQR_NOALLOC_MAX_N * RQR_NOALLOC_MAX_N];
+
+// Device address of the array on the CURRENT device.  In host code `d_noalloc_gram_part` is only a stand-in for the
+// symbol, not an address a kernel may use; cudaGetSymbolAddress resolves it per device.  Looked up once per device.
+static double* noalloc_gram_part()
+{
+    static std::atomic<double*> addr[RQR_MAX_DEVICES];
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) return nullptr;
+    const bool keep = dev >= 0 && dev < RQR_MAX_DEVICES;
+    if (keep) {
+        double* p = addr[dev].load(std::memory_order_acquire);
+        if (p) return p;
+    }
+    double* p = nullptr;
+    if (cudaGetSymbolAddress((void**)&p, d_noalloc_gram_part) != cudaSuccess || !p) {
+        cudaGetLastError();
+        return nullptr;
+    }
+    if (keep) addr[dev].store(p, std::memory_order_release);
+    return p;
+}
+
+extern "C" int rqr_trsm_gram_noalloc(const double* V, int64_t m, int n, int64_t ldv, const double* R0,
+                                     double* G, double* V1, int64_t ldq, void* stream)
+{
+    if (!V) return -1;
+    if (m < 1) return -2;
+    if (n < 2) return -3;
+    if (n > RQR_NOALLOC_MAX_N || m > RQR_NOALLOC_MAX_M) return RQR_ERR_SCRATCH_LIMIT;
+    if (ldv < n) return -4;
+    if (!G) return -6;
+    if (V1 && ldq < n) return -8;
+    double* part = noalloc_gram_part();
+    if (!part) return RQR_ERR_LAUNCH;
+    cudaStream_t st = (cudaStream_t)stream;
+    int nparts = 0;
+    // n <= 64 and one chunk of rows: the DMMA kernels run at most 148 CTAs, one partial each
+    int rc = rqr_trsm_gram_mma(V, m, n, ldv, R0, V1, ldq, part, &nparts, st);
+    if (rc == RQR_TALL_NOT_HANDLED) {
+        generic_attrs();
+        nparts = generic_grid(m);
+        if (nparts > RQR_NOALLOC_MAX_PARTIALS) nparts = RQR_NOALLOC_MAX_PARTIALS;
+        size_t smem = (size_t)GEN_TR * (n + 1) * sizeof(double);
+        k_trsm_gram_generic<<<nparts, 256, smem, st>>>(V, m, n, ldv, R0, V1, ldq, part);
+        RQR_LAUNCH_CHECK();
+    } else if (rc != RQR_OK) return rc;
+    dim3 rgrid((n + 63) / 64, n);
+    k_gram_reduce<<<rgrid, 256, 0, st>>>(part, nparts, n, G);
+    RQR_LAUNCH_CHECK();
+    return RQR_OK;
+}
