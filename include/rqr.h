@@ -68,7 +68,10 @@ extern "C" {
                                  atomics: no stored S1 at all ("storage of only O(n) values"; :947
                                  "adding/subtracting subsets of rows"), nothing to prepare in A0; the order of
                                  the reductions is not fixed.  Needs even n and ld and 16-byte aligned bases
-                                 (else it runs as RQR_VARIANT_SCATTER).                                  */
+                                 (else it runs as RQR_VARIANT_SCATTER).  When the whole sketch fits shared
+                                 memory (n <= 20 and 8 s1 n <= 224 KB; any ld, any alignment) every CTA
+                                 accumulates its rows in a shared-memory bucket tile with shared-memory
+                                 atomics and flushes it once (north_star's "shared-memory bucket tiles").  */
 
 /* flags */
 #define RQR_FLAG_PREPARED 1   /* `work` already holds the sketch state written by

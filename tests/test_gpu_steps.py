@@ -109,6 +109,24 @@ def test_countsketch_strided_and_row_offset(rq, orc):
         assert np.array_equal(host(W1), ref)
 
 
+@pytest.mark.parametrize("m,n,ld,s1,row0", [(70001, 12, 15, 300, 1000), (50000, 19, 19, 700, (1 << 33) + 3),
+                                            (33, 20, 22, 1400, 5), (100000, 3, 3, 9333, 0)])
+def test_countsketch_stream_tile_form(rq, orc, m, n, ld, s1, row0):
+    """RQR_VARIANT_STREAM with a sketch that fits shared memory (n <= 20, 8 s1 n <= 224 KB): the shared-memory
+    bucket-tile kernel (k_countsketch_tile): strided V, odd n, row offsets, odd s1 n (element-wise flush), a tile at the
+    size limit (1400 x 20) and a ragged last group."""
+    big = inputs.make_integer_V(m, ld, 6).cuda()
+    V = big[:, :n]
+    W1 = torch.full((s1, n), float("nan"), dtype=torch.float64, device="cuda")
+    work = rq.alloc_workspace(m, n, s1, min(2 * n, s1))
+    rq.countsketch(V, s1, 11, W1, work, variant=2, row0=row0)
+    assert np.array_equal(host(W1), orc.countsketch(host(V), s1, 11, row0=row0))
+    Vr = inputs.make_V(m, n, 1e6, 8) if m >= n else inputs.make_graded_V(m, n, 1, 8)
+    rq.countsketch(Vr.cuda(), s1, 11, W1, work, variant=2, row0=row0)
+    W1o = orc.countsketch(Vr.numpy(), s1, 11, row0=row0)
+    assert np.abs(host(W1) - W1o).max() <= 1e-13 * np.abs(W1o).max()
+
+
 @pytest.mark.parametrize("s1,n,s2", [(512, 16, 32), (8192, 64, 128), (9940, 70, 140), (300, 5, 7),
                                      (4096, 256, 512), (32768, 128, 256), (9984, 200, 401), (40000, 98, 130),
                                      (65536, 256, 512), (40953, 70, 789)])
