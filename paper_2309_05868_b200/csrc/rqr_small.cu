@@ -125,16 +125,29 @@ __device__ __forceinline__ double group8_sum(double x)
     return x;
 }
 
+// A/B switch of the single-factorization kernel, compile time only (-DRQR_GEQRF_G8X=0: eight columns per warp)
+#ifndef RQR_GEQRF_G8X
+#define RQR_GEQRF_G8X 1
+#endif
+
+// timing hooks of a working experiment (compiled out unless RQR_G8_TRACE is defined by the including file)
+#ifndef RQR_G8_MARK
+#define RQR_G8_MARK(k)
+#endif
+
 // One Householder step of k_geqrf_g8 with the row-slot index of the pivot, P = j / 8, known at
 // compile time: slots p < P hold finished (zeroed) rows and are skipped, the pivot element is
-// col[P] of lane t == j % 8 without a select, and the owner warp is w == P.
-template <int P>
-__device__ __forceinline__ void geqrf_g8_step(double (&a)[2][16], int j, int n, int w, int lane,
+// col[P] of lane t == j % 8 without a select.  QQ = column quads per warp: QQ = 2 (8 warps, warp w holds columns
+// 8 w + 4 qq + g, owner of column j is w == P) or QQ = 1 (16 warps, columns 4 w + g, owner w == j / 4): the same
+// arithmetic column by column (bit-identical results), half the instructions per warp and step on the chain.
+template <int P, int QQ>
+__device__ __forceinline__ void geqrf_g8_step(double (&a)[QQ][16], int j, int n, int w, int lane,
                                               double (*vbuf)[128], double* den_s, double* sgn_s,
                                               double* __restrict__ R0, int* d_info)
 {
     const int g = lane >> 3, t = lane & 7, tj = j & 7;
-    if (w == P) {                                          // warp-uniform: the warp that owns column j
+    RQR_G8_MARK(0);
+    if (w == (QQ == 2 ? P : (j >> 2))) {                   // warp-uniform: the warp that owns column j
         auto reflect = [&](double (&col)[16]) {
             double s0 = 0.0, s1 = 0.0;
 #pragma unroll
@@ -161,17 +174,21 @@ __device__ __forceinline__ void geqrf_g8_step(double (&a)[2][16], int j, int n, 
                 for (int p = P; p < 16; ++p) col[p] = 0.0;                           // column j is done
             }
         };
-        if ((j >> 2) & 1) reflect(a[1]); else reflect(a[0]);
+        if (QQ == 2 && ((j >> 2) & 1)) reflect(a[QQ - 1]); else reflect(a[0]);
     }
+    RQR_G8_MARK(1);
     __syncthreads();
+    RQR_G8_MARK(2);
+    if (4 * QQ * w + 4 * QQ - 1 <= j) return;        // warp-uniform: every column of this warp is finished (all zero);
+                                                     // it only keeps the barriers
     double v[16];
 #pragma unroll
     for (int p = P; p < 16; ++p) v[p] = vbuf[j & 1][t + 8 * p];
     const double den = den_s[j & 1], sg = sgn_s[j & 1];
     const double beta = (den > 0.0) ? 1.0 / den : 0.0;
-    double dot[2];
+    double dot[QQ];
 #pragma unroll
-    for (int qq = 0; qq < 2; ++qq) {
+    for (int qq = 0; qq < QQ; ++qq) {
         double s0 = 0.0, s1 = 0.0;
 #pragma unroll
         for (int p = P; p < 16; p += 2) {
@@ -182,37 +199,40 @@ __device__ __forceinline__ void geqrf_g8_step(double (&a)[2][16], int j, int n, 
     }
 #pragma unroll
     for (int o = 1; o < 8; o <<= 1) {
-        dot[0] += __shfl_xor_sync(0xffffffffu, dot[0], o);
-        dot[1] += __shfl_xor_sync(0xffffffffu, dot[1], o);
-    }
 #pragma unroll
-    for (int qq = 0; qq < 2; ++qq) {
+        for (int qq = 0; qq < QQ; ++qq) dot[qq] += __shfl_xor_sync(0xffffffffu, dot[qq], o);
+    }
+    RQR_G8_MARK(3);
+#pragma unroll
+    for (int qq = 0; qq < QQ; ++qq) {
         const double ws = beta * dot[qq];            // finished and padding columns are all zero: ws = 0
 #pragma unroll
         for (int p = P; p < 16; ++p) a[qq][p] = fma(-ws, v[p], a[qq][p]);
     }
     if (t == tj) {                                   // row j is final: move it out of the tile
 #pragma unroll
-        for (int qq = 0; qq < 2; ++qq) {
-            const int c = 8 * w + 4 * qq + g;
+        for (int qq = 0; qq < QQ; ++qq) {
+            const int c = 4 * QQ * w + 4 * qq + g;
             const double val = a[qq][P];
             a[qq][P] = 0.0;
             if (c > j && c < n) R0[(int64_t)j * n + c] = (sg > 0.0) ? -val : val;
         }
     }
+    RQR_G8_MARK(4);
 }
 
-template <int P>
-__device__ __forceinline__ void geqrf_g8_steps(double (&a)[2][16], int n, int w, int lane, double (*vbuf)[128],
+template <int P, int QQ>
+__device__ __forceinline__ void geqrf_g8_steps(double (&a)[QQ][16], int n, int w, int lane, double (*vbuf)[128],
                                                double* den_s, double* sgn_s, double* __restrict__ R0, int* d_info)
 {
     if constexpr (P < 8) {
         const int jend = (8 * P + 8 < n) ? 8 * P + 8 : n;
-        for (int j = 8 * P; j < jend; ++j) geqrf_g8_step<P>(a, j, n, w, lane, vbuf, den_s, sgn_s, R0, d_info);
-        if (8 * P + 8 < n) geqrf_g8_steps<P + 1>(a, n, w, lane, vbuf, den_s, sgn_s, R0, d_info);
+        for (int j = 8 * P; j < jend; ++j) geqrf_g8_step<P, QQ>(a, j, n, w, lane, vbuf, den_s, sgn_s, R0, d_info);
+        if (8 * P + 8 < n) geqrf_g8_steps<P + 1, QQ>(a, n, w, lane, vbuf, den_s, sgn_s, R0, d_info);
     }
 }
 
+template <int QQ>
 __device__ __forceinline__ void geqrf_g8_body(const double* __restrict__ W, int s2, int n, double* __restrict__ R0,
                                               int* d_info)
 {
@@ -220,25 +240,32 @@ __device__ __forceinline__ void geqrf_g8_body(const double* __restrict__ W, int 
     __shared__ double den_s[2], sgn_s[2];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int g = lane >> 3, t = lane & 7;
-    double a[2][16];
+    double a[QQ][16];
 #pragma unroll
-    for (int qq = 0; qq < 2; ++qq)
+    for (int qq = 0; qq < QQ; ++qq)
 #pragma unroll
         for (int p = 0; p < 16; ++p) {
-            const int c = 8 * w + 4 * qq + g, i = t + 8 * p;
+            const int c = 4 * QQ * w + 4 * qq + g, i = t + 8 * p;
             a[qq][p] = (c < n && i < s2) ? W[(int64_t)i * n + c] : 0.0;
         }
-    for (int e = threadIdx.x; e < n * n; e += 256) {      // exact zeros below the diagonal
+    for (int e = threadIdx.x; e < n * n; e += blockDim.x) {      // exact zeros below the diagonal
         const int i = e / n, c = e - i * n;
         if (c < i) R0[e] = 0.0;
     }
-    geqrf_g8_steps<0>(a, n, w, lane, vbuf, den_s, sgn_s, R0, d_info);
+    geqrf_g8_steps<0, QQ>(a, n, w, lane, vbuf, den_s, sgn_s, R0, d_info);
 }
 
 __global__ void __launch_bounds__(256, 1)
 k_geqrf_g8(const double* __restrict__ W, int s2, int n, double* __restrict__ R0, int* d_info)
 {
-    geqrf_g8_body(W, s2, n, R0, d_info);
+    geqrf_g8_body<2>(W, s2, n, R0, d_info);
+}
+
+// four columns per warp (QQ = 1), ceil(n / 4) <= 8 warps: the single factorization of A3 at n <= 32
+__global__ void __launch_bounds__(256, 1)
+k_geqrf_g8x(const double* __restrict__ W, int s2, int n, double* __restrict__ R0, int* d_info)
+{
+    geqrf_g8_body<1>(W, s2, n, R0, d_info);
 }
 
 // One level of a TSQR tree: block b = rows [b rows/nb, (b+1) rows/nb) of A (at most 128 each), its R
@@ -248,7 +275,7 @@ __global__ void __launch_bounds__(256, 1)
 k_geqrf_g8_batched(const double* __restrict__ A, int64_t rows, int nb, int n, double* __restrict__ Rout)
 {
     const int64_t r0 = (int64_t)blockIdx.x * rows / nb, r1 = (int64_t)(blockIdx.x + 1) * rows / nb;
-    geqrf_g8_body(A + r0 * n, (int)(r1 - r0), n, Rout + (int64_t)blockIdx.x * n * n, nullptr);
+    geqrf_g8_body<2>(A + r0 * n, (int)(r1 - r0), n, Rout + (int64_t)blockIdx.x * n * n, nullptr);
 }
 
 // R factor of the Householder QR of a TALL matrix A (rows x n, n <= 64, any rows >= n) by a TSQR tree of
@@ -264,7 +291,8 @@ int rqr_tsqr_r_dev(const double* A, int64_t rows, int n, double* R, double* scra
     for (;;) {
         const int64_t nb = (rows_in + 127) / 128;
         if (nb <= 1) {
-            k_geqrf_g8<<<1, 256, 0, st>>>(in, (int)rows_in, n, R, d_info);
+            if (RQR_GEQRF_G8X && n <= 32) k_geqrf_g8x<<<1, 32 * ((n + 3) / 4), 0, st>>>(in, (int)rows_in, n, R, d_info);
+            else                          k_geqrf_g8<<<1, 256, 0, st>>>(in, (int)rows_in, n, R, d_info);
             RQR_LAUNCH_CHECK();
             return RQR_OK;
         }
@@ -666,7 +694,13 @@ extern "C" int rqr_small_geqrf(double* W, int s2, int n, double* R0, int* d_info
     cudaStream_t st = (cudaStream_t)stream;
     const int rpl = (s2 + 31) / 32, cpw = (n + 31) / 32;
     if (s2 <= 128 && n <= 64) {
-        k_geqrf_g8<<<1, 256, 0, st>>>(W, s2, n, R0, d_info);
+        // four columns per warp: 8 warps cover n <= 32, 16 warps n <= 64 (k_geqrf_g8, eight columns per warp, remains
+        // the block kernel of the TSQR tree)
+        // n <= 32: four columns per warp, ceil(n / 4) warps (measured A/B in one run: 64 x 32 26.7 against 31.4 us,
+        // 32 x 16 15.4 against 17.9); above, eight columns per warp on 8 warps (128 x 64: 55.4 against 57.4 us
+        // with 16 warps: twice the warps reload the reflector from shared memory)
+        if (RQR_GEQRF_G8X && n <= 32) k_geqrf_g8x<<<1, 32 * ((n + 3) / 4), 0, st>>>(W, s2, n, R0, d_info);
+        else                          k_geqrf_g8<<<1, 256, 0, st>>>(W, s2, n, R0, d_info);
         RQR_LAUNCH_CHECK();
         return RQR_OK;
     }
