@@ -347,7 +347,7 @@ def make_step(torch, rq, rdist, Vd, c, seed, Q, R, bufs, flags, shard):
 
 
 def run_config(torch, rq, name, args, peaks, p64, want_e2e=True, want_breakdown=True, steps=None, shard=None,
-               shape=None):
+               shape=None, want_comparators=False):
     """Measures one workload.  shard = (world, rank, row0): this rank's block rows of the row-sharded job (weak
     scaling: `m` rows per rank); timings are then the max over ranks.  shape = (m, n, kappa): a sweep point."""
     from paper_2309_05868_b200 import dist as rdist, flops, inputs
@@ -456,6 +456,26 @@ def run_config(torch, rq, name, args, peaks, p64, want_e2e=True, want_breakdown=
         out["cholqr2_ms"] = median(pc)
         out["cholqr2_info"] = int(info.item())
         out["no_slower_than_cholqr2"] = bool(ms_med <= out["cholqr2_ms"])
+        if want_comparators:
+            # the other in-run comparators of BASELINE.json configs 2, 3 and 5 on the same V and the same kernels:
+            # shifted CholeskyQR3 (6 m n^2 flops, 48 m n bytes) and rand_cholQR with ONE dense Gaussian sketch
+            # (2 m n s2 + 3 m n^2 flops, 32 m n bytes), each against its own FP64 / HBM roofline (models of sweep.py)
+            comp = {"cholqr2": {"ms": out["cholqr2_ms"], "info": out["cholqr2_info"],
+                                "roofline_frac": max(flops.cholqr2_flops(m, n) / (p64 * 1e12), 32.0 * m * n / (peaks["hbm_gbs"] * 1e9))
+                                / (out["cholqr2_ms"] * 1e-3)}}
+            for cname, fn, Fc, Bc, reps_c in (
+                    ("scholqr3", lambda: rq.scholqr3(Vd, Q, R, work, info), 6.0 * m * n * n, 48.0 * m * n, 5),
+                    ("gauss_rand_cholqr", lambda: rq.gauss_randcholqr(Vd, s2, seed, Q, R, work, info),
+                     2.0 * m * n * s2 + 3.0 * m * n * n, 32.0 * m * n, 3)):
+                fn()
+                _, pcc = time_steps(torch, fn, reps_c)
+                st = int(info.item())
+                e = {"ms": median(pcc), "info": st,
+                     "roofline_frac": max(Fc / (p64 * 1e12), Bc / (peaks["hbm_gbs"] * 1e9)) / (median(pcc) * 1e-3)}
+                if st == 0:
+                    e["orth_err"], e["resid"] = checks()
+                comp[cname] = e
+            out["comparators"] = comp
     if want_breakdown:
         out["breakdown_ms"] = breakdown(torch, rq, Vd, c, seed, Q, R, bufs, max(5, steps // 3), recompute, row0)
     if want_e2e:
@@ -577,7 +597,8 @@ def main():
     c = inputs.config(args.workload)
     m, n = c["m"], c["n"]
     shard = (world, rank, rank * m) if sharded else None
-    main_out, F = run_config(torch, rq, args.workload, args, peaks, p64, want_e2e=not args.no_e2e, shard=shard)
+    main_out, F = run_config(torch, rq, args.workload, args, peaks, p64, want_e2e=not args.no_e2e, shard=shard,
+                             want_comparators=not args.no_extra)
     sampler.stop()
     sampler.join(timeout=1.0)
     clocks = sampler.summary()
@@ -589,7 +610,8 @@ def main():
         for nm, st in (("C2", 20), ("C4", 10)):
             if nm == args.workload:
                 continue
-            o, _ = run_config(torch, rq, nm, args, peaks, p64, want_e2e=False, want_breakdown=True, steps=st)
+            o, _ = run_config(torch, rq, nm, args, peaks, p64, want_e2e=False, want_breakdown=True, steps=st,
+                              want_comparators=(nm == "C2"))
             o.pop("_V_host_sample", None)
             extra["configs"][nm] = o
         for nn in (32, 64, 128):
@@ -643,6 +665,7 @@ def main():
             "resid_worst_of_seeds": main_out["resid_worst_of_seeds"], "sketch_seeds": main_out["sketch_seeds"],
             "cholqr2_ms": main_out.get("cholqr2_ms"), "cholqr2_info": main_out.get("cholqr2_info"),
             "no_slower_than_cholqr2": main_out.get("no_slower_than_cholqr2"),
+            "comparators": main_out.get("comparators"),
             "sketch_gen_ms": main_out["sketch_gen_ms"], "ms_with_sketch_gen": main_out["ms_with_sketch_gen"],
             "breakdown_ms": bd, "fp64_peak_tflops": p64s, "e2e": main_out.get("e2e"),
             "gpu_launches": nl * args.steps * world, "roofline": roof, "cpu_baseline": cpu,
