@@ -89,6 +89,28 @@ def test_argument_validation_without_gpu(lib):
     assert lib.rqr_rand_cholqr(one, 100, 8, 64, 16, 1, one, one, one, z, 32, 0, z) == -11
 
 
+def test_noalloc_entry_point_limits_without_gpu(lib):
+    """rqr_trsm_gram_noalloc: the limits of its built-in scratch are checked from the sizes alone, before the device
+    is touched, and the header's constants are the binding's."""
+    from paper_2309_05868_b200 import binding
+    hdr = open(os.path.join(ROOT, "include", "rqr.h")).read()
+    assert int(re.search(r"#define RQR_NOALLOC_MAX_N (\d+)", hdr).group(1)) == binding.NOALLOC_MAX_N == 64
+    assert re.search(r"#define RQR_NOALLOC_MAX_M \(\(int64_t\)1 << (\d+)\)", hdr).group(1) == "23"
+    assert binding.NOALLOC_MAX_M == 1 << 23
+    assert int(re.search(r"#define RQR_ERR_SCRATCH_LIMIT \((-\d+)\)", hdr).group(1)) == binding.ERR_SCRATCH_LIMIT
+    one = ctypes.c_void_p(16)
+    z = ctypes.c_void_p(0)
+    f = lib.rqr_trsm_gram_noalloc
+    assert f(one, 100, 66, 66, z, one, z, 66, z) == binding.ERR_SCRATCH_LIMIT
+    assert f(one, (1 << 23) + 1, 64, 64, z, one, z, 64, z) == binding.ERR_SCRATCH_LIMIT
+    assert f(z, 100, 64, 64, z, one, z, 64, z) == -1
+    assert f(one, 0, 64, 64, z, one, z, 64, z) == -2
+    assert f(one, 100, 1, 64, z, one, z, 64, z) == -3
+    assert f(one, 100, 64, 63, z, one, z, 64, z) == -4
+    assert f(one, 100, 64, 64, z, z, z, 64, z) == -6
+    assert f(one, 100, 64, 64, z, one, one, 63, z) == -8
+
+
 def test_binding_refuses_cpu_tensors(lib):
     import torch
     from paper_2309_05868_b200 import binding
