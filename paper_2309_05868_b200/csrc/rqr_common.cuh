@@ -12,7 +12,7 @@
 #define RQR_MAX_S2 1024
 #define RQR_MAX_GRAM_PARTIALS 304        // >= 2 CTAs per SM on 148 SMs (one chunk of rows)
 #define RQR_GRAM_CHUNK_ROWS ((int64_t)1 << 23)   // A4 accumulates at most this many rows per partial set
-#define RQR_GAUSS_PARTIAL_ROWS 16384     // ksplit * s2 <= this
+#define RQR_GAUSS_PARTIAL_ROWS 32768     // ksplit * s2 <= this (3 resident CTAs per SM at s2 = 767 ... 842: 37 ... 31 splits)
 #define RQR_PANEL_FRAG_BYTES (2 * 10 * 4096 * sizeof(double))   // rqr_tall_panel.cu
 
 #define RQR_PHILOX_STREAM_COUNT 0u

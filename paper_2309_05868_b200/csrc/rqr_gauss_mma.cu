@@ -133,11 +133,22 @@ static int launch_gauss_mma(const double* S2, const double* W1, int64_t s1, int 
         cudaFuncSetAttribute(k_gauss_gemm_mma<NBN, RAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Plan::bytes);
     });
     const int tiles_m = (s2 + 63) / 64;
-    int64_t ks = 296 / tiles_m;
-    if (ks > ks_cap) ks = ks_cap;
     const int64_t kblocks = (s1 + GM_KB - 1) / GM_KB;
-    if (ks > kblocks) ks = kblocks;
-    if (ks < 1) ks = 1;
+    // Resident CTAs: one per SM at NBN >= 24 (141 / 174 KB of shared memory), two at NBN = 16 (108 KB).  The K split
+    // that fills whole waves of those slots best, at most 296 CTAs, the larger split on a tie (C4: 8 row tiles x 18 =
+    // 144 CTAs in one wave of 148 instead of 8 x 32 = 256 in 1.73 waves: 1.29 -> 1.14 ms).
+    const int64_t slots = 148 * (Plan::bytes * 3 <= 227 * 1024 ? 3 : (Plan::bytes * 2 <= 227 * 1024 ? 2 : 1));
+    int64_t kmax = 2 * slots / tiles_m;
+    if (kmax > ks_cap) kmax = ks_cap;
+    if (kmax > kblocks) kmax = kblocks;
+    if (kmax < 1) kmax = 1;
+    int64_t ks = 1;
+    double best = 0.0;
+    for (int64_t k = 1; k <= kmax; ++k) {
+        const int64_t ctas = tiles_m * k, waves = (ctas + slots - 1) / slots;
+        const double eff = (double)ctas / (double)(waves * slots);
+        if (eff >= best - 1e-12) { best = eff; ks = k; }
+    }
     const int64_t kchunk = ((kblocks + ks - 1) / ks) * GM_KB;
     ks = (s1 + kchunk - 1) / kchunk;
     dim3 grid(1, tiles_m, (unsigned)ks);
@@ -147,18 +158,33 @@ static int launch_gauss_mma(const double* S2, const double* W1, int64_t s1, int 
     return RQR_OK;
 }
 
-// returns RQR_TALL_NOT_HANDLED when the shape is left to the DFMA kernel; S2 == NULL: Rademacher S2 from `seed`
+// returns RQR_TALL_NOT_HANDLED when the shape is left to the DFMA kernel; S2 == NULL: Rademacher S2 from `seed`.
+// n >= 96: always.  32 <= n < 96: only for a product large enough to fill the machine with 64-row tiles (the
+// paper-grid sketches, s2 = 600 ... 840 rows by s1 = 7 000 ... 67 000: measured 2-3x the DFMA kernel); the BASELINE
+// sketches at n <= 64 (s2 = 2n <= 128 rows: two row tiles) stay on the DFMA split-K kernel, which was measured faster
+// there.
+#ifndef RQR_GAUSS_MMA_MIN_WORK
+#define RQR_GAUSS_MMA_MIN_WORK 2.0e8      // s2 * s1 * n
+#endif
+template <bool RAD>
+static int gauss_mma_dispatch(const double* S2, const double* W1, int64_t s1, int n, int s2, double* part,
+                              int64_t ks_cap, int* ks_out, cudaStream_t st, uint64_t seed)
+{
+    if (n <= 64) return launch_gauss_mma<8, RAD>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st, seed);
+    if (n <= 80) return launch_gauss_mma<10, RAD>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st, seed);
+    if (n <= 96) return launch_gauss_mma<12, RAD>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st, seed);
+    if (n <= 112) return launch_gauss_mma<14, RAD>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st, seed);
+    if (n <= 128) return launch_gauss_mma<16, RAD>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st, seed);
+    if (n <= 192) return launch_gauss_mma<24, RAD>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st, seed);
+    return launch_gauss_mma<32, RAD>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st, seed);
+}
+
 int rqr_gauss_gemm_mma(const double* S2, const double* W1, int64_t s1, int n, int s2, double* part,
                        int64_t ks_cap, int* ks_out, cudaStream_t st, uint64_t seed)
 {
-    if (n < 96 || n > 256 || (n & 1)) return RQR_TALL_NOT_HANDLED;
+    if (n < 32 || n > 256 || (n & 1)) return RQR_TALL_NOT_HANDLED;
+    if (n < 96 && ((double)s2 * (double)s1 * n < RQR_GAUSS_MMA_MIN_WORK || s2 < 192)) return RQR_TALL_NOT_HANDLED;
     if ((((uintptr_t)S2 | (uintptr_t)W1) & 15) != 0) return RQR_TALL_NOT_HANDLED;
-    if (S2) {
-        if (n <= 128) return launch_gauss_mma<16, false>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st, seed);
-        if (n <= 192) return launch_gauss_mma<24, false>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st, seed);
-        return launch_gauss_mma<32, false>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st, seed);
-    }
-    if (n <= 128) return launch_gauss_mma<16, true>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st, seed);
-    if (n <= 192) return launch_gauss_mma<24, true>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st, seed);
-    return launch_gauss_mma<32, true>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st, seed);
+    if (S2) return gauss_mma_dispatch<false>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st, seed);
+    return gauss_mma_dispatch<true>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st, seed);
 }

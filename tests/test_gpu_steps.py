@@ -129,7 +129,9 @@ def test_countsketch_stream_tile_form(rq, orc, m, n, ld, s1, row0):
 
 @pytest.mark.parametrize("s1,n,s2", [(512, 16, 32), (8192, 64, 128), (9940, 70, 140), (300, 5, 7),
                                      (4096, 256, 512), (32768, 128, 256), (9984, 200, 401), (40000, 98, 130),
-                                     (65536, 256, 512), (40953, 70, 789)])
+                                     (65536, 256, 512), (40953, 70, 789),
+                                     # 32 <= n < 96 with a large product: the DMMA GEMM with 8 / 10 / 12 column blocks
+                                     (13514, 40, 707), (30159, 60, 767), (9001, 34, 900), (12000, 88, 333)])
 def test_gauss_sketch_parity(rq, orc, s1, n, s2):
     rng = np.random.default_rng(s1 + n)
     W1 = rng.standard_normal((s1, n))
