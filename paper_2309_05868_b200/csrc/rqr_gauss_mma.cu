@@ -1,11 +1,12 @@
-// rqr_gauss_mma.cu -- A2 for n >= 128: W = S2 W1 as a split-K FP64 DMMA GEMM.
-// At n = 256 this step is 34 GFLOP over 0.8 GB (C4): FP64-bound, 8% of the path's flops.
+// rqr_gauss_mma.cu -- A2 for n >= 96 (and large products from n = 32): W = S2 W1 as a split-K FP64
+// DMMA GEMM.  At n = 256 this step is 34 GFLOP over 0.8 GB (C4): FP64-bound, 8% of the path's flops.
 // CTA (y = 64-row tile of S2, z = K chunk): 8 consumer warps, warp w owns rows 8w..8w+7 of the tile and
-// all n columns (NBN accumulator blocks in registers); a producer warp stages 16-deep K slices of the S2
-// tile (64 x 16) and of W1 (16 x n) with per-row bulk async copies into padded rows (strides 20 and
-// n+4 doubles: the A- and B-fragment reads are bank-conflict free); 4 stages, full/empty mbarriers.
-// Partials go to the caller's buffer and are reduced in fixed order by k_reduce_partials.
-// RAD (N4): S2 is the dense Rademacher matrix of reading S21; nothing of S2 is staged, every lane
+// all n columns (NBN accumulator blocks in registers); a producer warp stages 16-deep K slices of W1 (16 x n) with
+// per-row bulk async copies into padded rows (stride n+4 doubles: the B-fragment reads are bank-conflict free), 4 stages,
+// full/empty mbarriers; the A fragments (S2) come straight from global memory, one slice ahead in registers: every entry
+// of S2 is used by exactly one warp.  Partials go to the caller's buffer and are reduced in fixed order by
+// k_reduce_partials.
+// RAD (N4): S2 is the dense Rademacher matrix of reading S21; nothing of S2 is read, every lane
 // forms its A-fragment entries +-1/sqrt(s2) from the Philox words of its row (one call per 128 columns).
 #include "rqr_mma.cuh"
 
@@ -20,9 +21,9 @@ __device__ __forceinline__ void gm_arrive(uint64_t* bar)
 
 template <int NBN>
 struct GaussPlan {
-    static constexpr int LDA = GM_KB + 4, LDB = 8 * NBN + 4;
-    static constexpr size_t a_doubles = 64 * LDA, b_doubles = (size_t)GM_KB * LDB;
-    static constexpr size_t stage = a_doubles + b_doubles;
+    static constexpr int LDB = 8 * NBN + 4;
+    static constexpr size_t b_doubles = (size_t)GM_KB * LDB;
+    static constexpr size_t stage = b_doubles;          // only W1 is staged: every entry of S2 is used by ONE warp
     static constexpr size_t bars = GM_STAGES * stage;
     static constexpr size_t bytes = (bars + 2 * GM_STAGES) * sizeof(double);
 };
@@ -33,7 +34,7 @@ k_gauss_gemm_mma(const double* __restrict__ S2, const double* __restrict__ W1, i
                  int64_t kchunk, double* __restrict__ part, uint64_t seed)
 {
     using Plan = GaussPlan<NBN>;
-    constexpr int LDA = Plan::LDA, LDB = Plan::LDB;
+    constexpr int LDB = Plan::LDB;
     extern __shared__ __align__(16) double smem[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smem + Plan::bars);
     uint64_t* empty = full + GM_STAGES;
@@ -50,24 +51,19 @@ k_gauss_gemm_mma(const double* __restrict__ S2, const double* __restrict__ W1, i
     const int64_t k1 = (k0 + kchunk < s1) ? k0 + kchunk : s1;
     const int nsteps = (int)((k1 - k0 + GM_KB - 1) / GM_KB);
     const int64_t lds2 = rqr_s2_ld(s1);                 // rows of S2 are padded with zeros to a multiple of 16
-    const int rows_a = (s2 - m0) < 64 ? (s2 - m0) : 64;
 
     if (warp == GM_WARPS) {
         int stage = 0;
         uint32_t ph = 0;
         for (int s = 0; s < nsteps; ++s) {
             const int64_t k = k0 + (int64_t)s * GM_KB;
-            double* A = smem + (size_t)stage * Plan::stage;
-            double* B = A + Plan::a_doubles;
+            double* B = smem + (size_t)stage * Plan::stage;
             mbar_wait(empty + stage, ph ^ 1u);
             // the last slice may run past s1: S2's pad columns are zero, the matching rows of the B stage
             // keep finite data of an earlier slice (0 x finite = 0), so only the existing rows of W1 are copied
             const int rows_b = (int)((s1 - k) < GM_KB ? (s1 - k) : GM_KB);
-            if (lane == 0) mbar_expect_tx(full + stage, (uint32_t)((RAD ? 0 : rows_a * GM_KB * 8) + rows_b * n * 8));
+            if (lane == 0) mbar_expect_tx(full + stage, (uint32_t)(rows_b * n * 8));
             __syncwarp();
-            if (!RAD)
-                for (int r = lane; r < rows_a; r += 32)
-                    bulk_g2s(A + r * LDA, S2 + (int64_t)(m0 + r) * lds2 + k, GM_KB * 8, full + stage);
             if (lane < rows_b) bulk_g2s(B + lane * LDB, W1 + (k + lane) * n, (uint32_t)(n * 8), full + stage);
             if (++stage == GM_STAGES) { stage = 0; ph ^= 1u; }
         }
@@ -83,9 +79,22 @@ k_gauss_gemm_mma(const double* __restrict__ S2, const double* __restrict__ W1, i
     const double inv = 1.0 / sqrt((double)s2);
     uint32_t o[4] = {0u, 0u, 0u, 0u};
     int64_t gcur = -1;
+    // A fragments straight from global memory: lane (r, q) needs S2[m0 + 8 warp + r][k + 4 j + q], j < 4, of every
+    // K slice -- one 32-byte sector per row and load, each entry of S2 read by exactly one lane of the grid, so
+    // staging it in shared memory bought nothing and cost 64 bulk copies of 128 bytes per slice (measured: the
+    // Rademacher form, which stages no A, ran the same product in 0.52 against 0.83 ms).  One slice ahead in registers.
+    const int arow = m0 + 8 * warp + r;
+    const double* Ag = RAD ? nullptr : S2 + (int64_t)(arow < s2 ? arow : 0) * lds2 + k0 + q;
+    const bool aok = !RAD && arow < s2;
+    double acur[GM_KB / 4], anext[GM_KB / 4];
+#pragma unroll
+    for (int j = 0; j < GM_KB / 4; ++j) { acur[j] = (aok && nsteps > 0) ? __ldg(Ag + 4 * j) : 0.0; anext[j] = 0.0; }
     for (int s = 0; s < nsteps; ++s) {
-        const double* A = smem + (size_t)stage * Plan::stage + (8 * warp + r) * LDA + q;
-        const double* B = smem + (size_t)stage * Plan::stage + Plan::a_doubles + q * LDB + r;
+        const double* B = smem + (size_t)stage * Plan::stage + q * LDB + r;
+        if (aok && s + 1 < nsteps) {
+#pragma unroll
+            for (int j = 0; j < GM_KB / 4; ++j) anext[j] = __ldg(Ag + (int64_t)(s + 1) * GM_KB + 4 * j);
+        }
         uint32_t bits = 0;
         const int64_t kcol = k0 + (int64_t)s * GM_KB;
         if (RAD) {
@@ -103,13 +112,15 @@ k_gauss_gemm_mma(const double* __restrict__ S2, const double* __restrict__ W1, i
         for (int kk = 0; kk < GM_KB; kk += 4) {
             double a;
             if (RAD) a = (kcol + kk + q < s1) ? (((bits >> kk) & 1u) ? -inv : inv) : 0.0;
-            else a = A[kk];
+            else a = acur[kk / 4];
 #pragma unroll
             for (int b = 0; b < NBN; ++b) dmma(acc[b][0], acc[b][1], a, B[kk * LDB + 8 * b]);
         }
         __syncwarp();
         if (lane == 0) gm_arrive(empty + stage);
         if (++stage == GM_STAGES) { stage = 0; ph ^= 1u; }
+#pragma unroll
+        for (int j = 0; j < GM_KB / 4; ++j) acur[j] = anext[j];
     }
     double* P = part + (int64_t)blockIdx.z * s2 * n;
     const int row = m0 + 8 * warp + r;
@@ -166,6 +177,9 @@ static int launch_gauss_mma(const double* S2, const double* W1, int64_t s1, int 
 #ifndef RQR_GAUSS_MMA_MIN_WORK
 #define RQR_GAUSS_MMA_MIN_WORK 2.0e8      // s2 * s1 * n
 #endif
+#ifndef RQR_GAUSS_MMA_MIN_S2
+#define RQR_GAUSS_MMA_MIN_S2 192
+#endif
 template <bool RAD>
 static int gauss_mma_dispatch(const double* S2, const double* W1, int64_t s1, int n, int s2, double* part,
                               int64_t ks_cap, int* ks_out, cudaStream_t st, uint64_t seed)
@@ -183,7 +197,7 @@ int rqr_gauss_gemm_mma(const double* S2, const double* W1, int64_t s1, int n, in
                        int64_t ks_cap, int* ks_out, cudaStream_t st, uint64_t seed)
 {
     if (n < 32 || n > 256 || (n & 1)) return RQR_TALL_NOT_HANDLED;
-    if (n < 96 && ((double)s2 * (double)s1 * n < RQR_GAUSS_MMA_MIN_WORK || s2 < 192)) return RQR_TALL_NOT_HANDLED;
+    if (n < 96 && ((double)s2 * (double)s1 * n < RQR_GAUSS_MMA_MIN_WORK || s2 < RQR_GAUSS_MMA_MIN_S2)) return RQR_TALL_NOT_HANDLED;
     if ((((uintptr_t)S2 | (uintptr_t)W1) & 15) != 0) return RQR_TALL_NOT_HANDLED;
     if (S2) return gauss_mma_dispatch<false>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st, seed);
     return gauss_mma_dispatch<true>(S2, W1, s1, n, s2, part, ks_cap, ks_out, st, seed);
