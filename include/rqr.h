@@ -32,7 +32,7 @@
  *  - Fast paths: the FP64 DMMA kernels of rqr_trsm_gram / rqr_apply need an even n, even leading
  *    dimensions and 16-byte aligned bases (2 <= n <= 64: fused kernels; 64 < n <= 256: panel
  *    kernels); rqr_gauss_sketch uses its DMMA GEMM for even n >= 96, and for even 32 <= n < 96 when the product is
- *    large (s2 >= 192 and s2 s1 n >= 2e8: the paper-grid sketch sizes).  Any other
+ *    large (s2 >= 128 and s2 s1 n >= 5e7).  Any other
  *    shape runs the generic kernels: same results to rounding, much slower.
  *  - Thread safety: calls on different streams with different buffers are independent, from any host thread and on
  *    any device.  The library keeps no state besides the per-device "kernel attributes set" flags (atomic; the

@@ -134,6 +134,9 @@ k_gauss_gemm_mma(const double* __restrict__ S2, const double* __restrict__ W1, i
     }
 }
 
+#ifndef RQR_GAUSS_MMA_MIN_STEPS
+#define RQR_GAUSS_MMA_MIN_STEPS 8
+#endif
 template <int NBN, bool RAD>
 static int launch_gauss_mma(const double* S2, const double* W1, int64_t s1, int n, int s2, double* part,
                             int64_t ks_cap, int* ks_out, cudaStream_t st, uint64_t seed)
@@ -151,7 +154,7 @@ static int launch_gauss_mma(const double* S2, const double* W1, int64_t s1, int 
     const int64_t slots = 148 * (Plan::bytes * 3 <= 227 * 1024 ? 3 : (Plan::bytes * 2 <= 227 * 1024 ? 2 : 1));
     int64_t kmax = 2 * slots / tiles_m;
     if (kmax > ks_cap) kmax = ks_cap;
-    if (kmax > kblocks) kmax = kblocks;
+    if (kmax > kblocks / RQR_GAUSS_MMA_MIN_STEPS) kmax = kblocks / RQR_GAUSS_MMA_MIN_STEPS;   // >= that many K slices per CTA
     if (kmax < 1) kmax = 1;
     int64_t ks = 1;
     double best = 0.0;
@@ -170,15 +173,15 @@ static int launch_gauss_mma(const double* S2, const double* W1, int64_t s1, int 
 }
 
 // returns RQR_TALL_NOT_HANDLED when the shape is left to the DFMA kernel; S2 == NULL: Rademacher S2 from `seed`.
-// n >= 96: always.  32 <= n < 96: only for a product large enough to fill the machine with 64-row tiles (the
-// paper-grid sketches, s2 = 600 ... 840 rows by s1 = 7 000 ... 67 000: measured 2-3x the DFMA kernel); the BASELINE
-// sketches at n <= 64 (s2 = 2n <= 128 rows: two row tiles) stay on the DFMA split-K kernel, which was measured faster
-// there.
+// n >= 96: always.  32 <= n < 96: for s2 >= 128 rows and s2 s1 n >= 5e7: the paper-grid sketches (s2 = 600 ... 840 rows
+// by s1 = 7 000 ... 67 000: 2-3x the DFMA kernel) and the BASELINE sketch at n = 64 (128 x 8192: 19.7 -> 14.5 us with at
+// least 8 K slices per CTA, i.e. 64 partials instead of 148 for the reduction); smaller ones stay on the DFMA split-K
+// kernel (same time on either: launch + reduction).
 #ifndef RQR_GAUSS_MMA_MIN_WORK
-#define RQR_GAUSS_MMA_MIN_WORK 2.0e8      // s2 * s1 * n
+#define RQR_GAUSS_MMA_MIN_WORK 5.0e7      // s2 * s1 * n
 #endif
 #ifndef RQR_GAUSS_MMA_MIN_S2
-#define RQR_GAUSS_MMA_MIN_S2 192
+#define RQR_GAUSS_MMA_MIN_S2 128
 #endif
 template <bool RAD>
 static int gauss_mma_dispatch(const double* S2, const double* W1, int64_t s1, int n, int s2, double* part,
