@@ -127,6 +127,46 @@ def test_countsketch_stream_tile_form(rq, orc, m, n, ld, s1, row0):
     assert np.abs(host(W1) - W1o).max() <= 1e-13 * np.abs(W1o).max()
 
 
+def test_new_kernels_write_only_their_outputs(rq, orc):
+    """Guard bands around the outputs of the kernels added in round 2 (compute-sanitizer is not available on the pool):
+    the shared-memory-tile CountSketch (bulk-reduction flush and element-wise flush), the DMMA sketch GEMM below
+    n = 96 and the four-columns-per-warp Householder kernel must leave every sentinel outside their output intact."""
+    SENT = 1234.5
+    def guarded(rows, cols, g=64):
+        buf = torch.full(((rows + 2 * g) * cols,), SENT, dtype=torch.float64, device="cuda")
+        return buf, buf[g * cols:(g + rows) * cols].view(rows, cols)
+    def intact(buf, rows, cols, g=64):
+        return bool((buf[:g * cols] == SENT).all()) and bool((buf[(g + rows) * cols:] == SENT).all())
+    for m, n, s1 in [(50000, 20, 1400), (70001, 7, 37), (33, 12, 5)]:
+        V = inputs.make_integer_V(m, n, 9).cuda()
+        buf, W1 = guarded(s1, n)
+        work = rq.alloc_workspace(m, n, s1, min(2 * n, s1))
+        rq.countsketch(V, s1, 3, W1, work, variant=2)
+        torch.cuda.synchronize()
+        assert intact(buf, s1, n)
+        assert np.array_equal(host(W1), orc.countsketch(host(V), s1, 3))
+    for s1, n, s2 in [(13514, 40, 707), (9001, 34, 900), (8192, 64, 128)]:
+        rng = np.random.default_rng(s1)
+        W1 = dev(rng.standard_normal((s1, n)))
+        buf, W = guarded(s2, n)
+        work = rq.alloc_workspace(s1, n, s1, s2)
+        rq.gauss_sketch(W1, s2, 42, W, work)
+        torch.cuda.synchronize()
+        assert intact(buf, s2, n)
+        Wo = orc.gauss_sketch(host(W1), s2, 42)
+        assert np.abs(host(W) - Wo).max() <= 1e-13 * np.abs(Wo).max()
+    for s2, n in [(64, 32), (20, 10), (128, 30), (37, 13)]:
+        rng = np.random.default_rng(s2 + n)
+        Wm = rng.standard_normal((s2, n))
+        buf, R0 = guarded(n, n)
+        info = rq.new_info()
+        rq.small_geqrf(dev(Wm), R0, info)
+        torch.cuda.synchronize()
+        assert intact(buf, n, n) and int(info.item()) == 0
+        Ro, _ = orc.hhqr_r(Wm)
+        assert np.linalg.norm(host(R0) - Ro) <= 1e-13 * np.linalg.norm(Ro)
+
+
 @pytest.mark.parametrize("s1,n,s2", [(512, 16, 32), (8192, 64, 128), (9940, 70, 140), (300, 5, 7),
                                      (4096, 256, 512), (32768, 128, 256), (9984, 200, 401), (40000, 98, 130),
                                      (65536, 256, 512), (40953, 70, 789),
