@@ -201,7 +201,7 @@ def run_reference(args):
             "data": "synthetic", "config": config_dict(args, c, args.workload, v1_mode_of(args, n)),
             "cpu_baseline": r,
             "e2e": {"value": r["value"], "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
-    print(json.dumps(line))
+    _emit(line)
 
 
 # ------------------------------------------------------------------------------------------
@@ -561,8 +561,32 @@ def run_config(torch, rq, name, args, peaks, p64, want_e2e=True, want_breakdown=
     return out, F
 
 
+_JSON_FD = None
+
+
+def _claim_stdout():
+    """stdout carries exactly ONE line, the JSON record.  Libraries loaded below write to file descriptor 1 on their
+    own (NCCL prints "NCCL version ..." there on the first communicator, whatever NCCL_DEBUG_FILE says): keep a
+    private duplicate of the real stdout for the record and point descriptor 1 at stderr for everything else."""
+    global _JSON_FD
+    if _JSON_FD is None:
+        sys.stdout.flush()
+        _JSON_FD = os.dup(1)
+        os.dup2(2, 1)
+
+
+def _emit(line):
+    sys.stdout.flush()
+    data = (json.dumps(line) + "\n").encode()
+    if _JSON_FD is None:
+        os.write(1, data)
+    else:
+        os.write(_JSON_FD, data)
+
+
 def main():
     args = parse()
+    _claim_stdout()
     if args.impl == "reference":
         run_reference(args)
         return
@@ -681,7 +705,7 @@ def main():
     if sharded:
         line["config"].update({"m_per_gpu": m, "m_total": m * world,
                                "parallelism": "row-sharded, 2 all-reduces (W, G) per step"})
-    print(json.dumps(line))
+    _emit(line)
     if sharded:
         import torch.distributed as dist
         dist.destroy_process_group()
