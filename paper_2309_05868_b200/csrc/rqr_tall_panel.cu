@@ -23,7 +23,7 @@
 
 #define PANEL_WARPS 8        // consumer warps of k_syrk_fold; warp PANEL_WARPS is the producer
 #ifndef PANEL_CW_WIDE
-#define PANEL_CW_WIDE 11     // consumer warps of k_trsm_panel for NP = 2 (PanelPlan)
+#define PANEL_CW_WIDE 15     // consumer warps of k_trsm_panel for NP = 2 (PanelPlan): 16 warps = 4 per sub-partition
 #endif
 #define PANEL_SLOT 4096      // doubles per fragment slot (32 KB)
 #define PANEL_DIAG 2304      // doubles used by a diagonal slot: Tf (8*64) + nRf (28*64)
@@ -72,9 +72,10 @@ k_build_panel_frags(const double* __restrict__ R, int n, double* __restrict__ fr
 
 template <int NP>
 struct PanelPlan {
-    // consumer warps of k_trsm_panel: 11 (+ the producer = 3 per SM sub-partition, 170 registers each) at NP = 2
-    // (measured at 2^21 rows: n = 128 A6 1.196 -> 1.157 ms, n = 96 0.755 -> 0.706 ms), 8 above (NP = 3: 2.46 vs
-    // 2.49 ms with 11; NP = 4: one 8 x 264-double landing block per warp is 17 KB)
+    // consumer warps of k_trsm_panel: 15 (+ the producer = 4 per SM sub-partition, 128 registers each; the kernel
+    // needs 116) at NP = 2 (measured A/B in one process at 2^22 rows: n = 128 A6 2.283 ms with 11 warps, 2.522 with 13
+    // -- an odd number of warps per sub-partition pair --, 2.207 with 15; n = 96 1.385 / 1.551 / 1.327), 8 above
+    // (NP = 3: 2.46 vs 2.49 ms with 11; NP = 4: one 8 x 264-double landing block per warp is 17 KB)
     static constexpr int CW = (NP == 2) ? PANEL_CW_WIDE : 8;
     static constexpr int N8 = 64 * NP;
     static constexpr int LDL = N8 + LDL_PAD;
