@@ -291,8 +291,11 @@ extern "C" int rqr_sketch_prepare(int64_t m, int n, int64_t row0, int64_t s1, in
 // bucket's rows r, r+R, r+2R, ... (4 loads in flight per thread), then the R slot sums are
 // added in slot order through shared memory.  Fixed mapping => bit-reproducible W1.
 // HBM-bound: every row of V is read exactly once, 8n contiguous bytes.
-template <int VEC>
-__global__ void __launch_bounds__(256)
+#ifndef RQR_GATHER_PREFETCH_MAX_N
+#define RQR_GATHER_PREFETCH_MAX_N 40
+#endif
+template <int VEC, bool PREFETCH>
+__global__ void __launch_bounds__(256, 8)
 k_countsketch_gather(const double* __restrict__ V, int64_t ldv, int n,
                      const uint32_t* __restrict__ off, const uint32_t* __restrict__ entries,
                      uint32_t s1, double* __restrict__ W1, uint32_t split)
@@ -314,12 +317,23 @@ k_countsketch_gather(const double* __restrict__ V, int64_t ldv, int n,
         double a0 = 0.0, a1 = 0.0;
         if (active) {
             uint32_t k = beg + slot;
-            // 4 rows in flight
-            for (; k + 3u * R < end; k += 4u * R) {
-                uint32_t e[4];
-                double x[4][2];
+            // 4 rows in flight; PREFETCH: the row-list entries of the NEXT four are loaded while these are in flight
+            uint32_t e[4] = {0u, 0u, 0u, 0u}, en[4] = {0u, 0u, 0u, 0u};
+            if (PREFETCH && k + 3u * R < end) {
 #pragma unroll
                 for (int u = 0; u < 4; ++u) e[u] = entries[k + u * R];
+            }
+            for (; k + 3u * R < end; k += 4u * R) {
+                double x[4][2];
+                if (!PREFETCH) {
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) e[u] = entries[k + u * R];
+                }
+                const bool more = PREFETCH && k + 7u * R < end;
+                if (more) {
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) en[u] = entries[k + (4 + u) * R];
+                }
 #pragma unroll
                 for (int u = 0; u < 4; ++u) {
                     const double* p = V + (int64_t)(e[u] & 0x7fffffffu) * ldv + col;
@@ -334,6 +348,10 @@ k_countsketch_gather(const double* __restrict__ V, int64_t ldv, int n,
                 for (int u = 0; u < 4; ++u) {
                     if (e[u] >> 31) { a0 -= x[u][0]; a1 -= x[u][1]; }
                     else            { a0 += x[u][0]; a1 += x[u][1]; }
+                }
+                if (PREFETCH) {
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) e[u] = en[u];
                 }
             }
             for (; k < end; k += R) {
@@ -669,8 +687,15 @@ extern "C" int rqr_countsketch(const double* V, int64_t m, int n, int64_t ldv, i
     double* dst = split > 1 ? (double*)(w + L.A) : W1;
     const int64_t items = s1 * split;
     int blocks = (int)(items < 148 * 8 ? items : 148 * 8);
-    if (vec2) k_countsketch_gather<2><<<blocks, 256, smem, st>>>(V, ldv, n, off, ent, (uint32_t)s1, dst, (uint32_t)split);
-    else      k_countsketch_gather<1><<<blocks, 256, smem, st>>>(V, ldv, n, off, ent, (uint32_t)s1, dst, (uint32_t)split);
+    // PREFETCH: the next four row-list entries are loaded while four rows are in flight (the entry load and the row load
+    // it feeds are two dependent memory latencies).  Measured A/B in one process, both forms at 8 resident CTAs per SM
+    // (__launch_bounds__(256, 8): 32 registers either way): it pays for even n <= 40 without a bucket split (2^22 x 32
+    // 193 -> 184 us, 2^25 x 32 1457 -> 1361, 10^7 x 20 309 -> 292) and loses for odd n (scalar loads: 173 -> 238 us
+    // at n = 33), with split buckets and from n = 48 up.
+    const bool pf = vec2 && n <= RQR_GATHER_PREFETCH_MAX_N && split == 1;
+    if (vec2 && pf)  k_countsketch_gather<2, true><<<blocks, 256, smem, st>>>(V, ldv, n, off, ent, (uint32_t)s1, dst, (uint32_t)split);
+    else if (vec2)   k_countsketch_gather<2, false><<<blocks, 256, smem, st>>>(V, ldv, n, off, ent, (uint32_t)s1, dst, (uint32_t)split);
+    else             k_countsketch_gather<1, false><<<blocks, 256, smem, st>>>(V, ldv, n, off, ent, (uint32_t)s1, dst, (uint32_t)split);
     RQR_LAUNCH_CHECK();
     if (split > 1) {
         const int64_t elems = s1 * n;
