@@ -794,7 +794,13 @@ __device__ __forceinline__ double* chol2_tslot(double* base, int ld, int K)
     return (K < 15) ? base + (int64_t)(8 * (K + 1)) * ld + 8 * K : base + (int64_t)(8 * 15) * ld;
 }
 
-__global__ void __launch_bounds__(256, 1)
+// threads of k_chol_blocked: 8 warps up to n = 48 (at most 15 trailing blocks), 16 warps above (A/B: RQR_CHOL_WIDE)
+#ifndef RQR_CHOL_WIDE
+#define RQR_CHOL_WIDE 1
+#endif
+#define RQR_CHOL_THREADS(nn) ((RQR_CHOL_WIDE && (nn) > 48) ? 512 : 256)
+template <int THREADS>
+__global__ void __launch_bounds__(THREADS, 1)
 k_chol_blocked(const double* G, int ldg, int n, double shift_h, const double* __restrict__ d_shift,
                double* R1, int ldr, int* d_info, int info_off, const double* __restrict__ Rprev,
                double* __restrict__ Rprod, double* Tsave, int ldt, double* zero_src, int zero_cols)
@@ -811,7 +817,8 @@ k_chol_blocked(const double* G, int ldg, int n, double shift_h, const double* __
     __shared__ int fail_s;
     const double shift = shift_h + (d_shift ? *d_shift : 0.0);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    for (int e = tid; e < np * np; e += 256) {
+    const int nthr = blockDim.x, nwarps = nthr >> 5;             // 8 or 16 warps (CHOL_THREADS_OF)
+    for (int e = tid; e < np * np; e += nthr) {
         const int i = e / np, c = e - i * np;
         double v = (i == c) ? 1.0 : 0.0;
         if (i < n && c < n) v = G[(int64_t)i * ldg + c] + ((i == c) ? shift : 0.0);
@@ -819,12 +826,12 @@ k_chol_blocked(const double* G, int ldg, int n, double shift_h, const double* __
     }
     if (zero_src != nullptr) {
         __syncthreads();                                  // every thread has read its part of the scratch input
-        for (int e = tid; e < n * zero_cols; e += 256) {
+        for (int e = tid; e < n * zero_cols; e += nthr) {
             const int i = e / zero_cols, c = e - i * zero_cols;
             zero_src[(int64_t)i * ldg + c] = 0.0;
         }
     }
-    for (int e = tid; e < n * n; e += 256) {              // exact zeros below the diagonal
+    for (int e = tid; e < n * n; e += nthr) {              // exact zeros below the diagonal
         const int i = e / n, c = e - i * n;
         if (c < i) R1[(int64_t)i * ldr + c] = 0.0;
     }
@@ -882,7 +889,7 @@ k_chol_blocked(const double* G, int ldg, int n, double shift_h, const double* __
         }
         __syncthreads();
         if (fail_s) break;
-        if (warp == 7) {                                      // R_KK to global
+        if (warp == nwarps - 1) {                                      // R_KK to global
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
                 const int i = (lane + 32 * h) >> 3, c = (lane + 32 * h) & 7;
@@ -891,7 +898,7 @@ k_chol_blocked(const double* G, int ldg, int n, double shift_h, const double* __
             }
         }
         // (2) row panel: R[K,J] = T^T A[K,J], J > K
-        for (int J = K + 1 + warp; J < NB; J += 8) {
+        for (int J = K + 1 + warp; J < NB; J += nwarps) {
             double c0 = 0.0, c1 = 0.0;
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
@@ -908,7 +915,7 @@ k_chol_blocked(const double* G, int ldg, int n, double shift_h, const double* __
         __syncthreads();
         // (3) trailing update: A[I,J] -= R[K,I]^T R[K,J], K < I <= J
         const int nt = NB - K - 1;
-        for (int pidx = warp; pidx < nt * (nt + 1) / 2; pidx += 8) {
+        for (int pidx = warp; pidx < nt * (nt + 1) / 2; pidx += nwarps) {
             int I = 0, rem = pidx;
             while (rem >= nt - I) { rem -= nt - I; ++I; }
             const int J = K + 1 + I + rem;
@@ -932,14 +939,14 @@ k_chol_blocked(const double* G, int ldg, int n, double shift_h, const double* __
         // fused A7 of the one-shot drivers: Rprod = R1 Rprev (upper x upper, Alg. 3 step 3 PAPER.md:206).  R1 is the
         // upper triangle of A; Rprev^T is staged into the (now free) strict lower triangle, its diagonal into the
         // first pad column; the product runs block-wise on mma.sync like the trailing update.
-        for (int e = tid; e < n * n; e += 256) {
+        for (int e = tid; e < n * n; e += nthr) {
             const int k = e / n, c = e - k * n;
             if (k < c) A[c * LD + k] = __ldg(Rprev + e);
             else if (k == c) A[k * LD + np] = __ldg(Rprev + e);
             else if ((c >> 3) < (k >> 3)) Rprod[e] = 0.0;
         }
         __syncthreads();
-        for (int blk = warp; blk < NB * (NB + 1) / 2; blk += 8) {
+        for (int blk = warp; blk < NB * (NB + 1) / 2; blk += nwarps) {
             int I = 0, rem = blk;
             while (rem >= NB - I) { rem -= NB - I; ++I; }
             const int J = I + rem;
@@ -1075,24 +1082,30 @@ int rqr_chol_dev(const double* G, int n, double shift, const double* d_shift, do
     if (!R1) return -4;
     if (G == R1) return -4;
     RQR_ONCE_PER_DEVICE({
-        cudaFuncSetAttribute(k_chol_blocked, cudaFuncAttributeMaxDynamicSharedMemorySize, 144 * 1024);
+        cudaFuncSetAttribute(k_chol_blocked<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, 144 * 1024);
+        cudaFuncSetAttribute(k_chol_blocked<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, 144 * 1024);
     });
     auto smem_of = [](int nn) { const int np = (nn + 7) & ~7; return (size_t)np * (np + 8 + (np & 8)) * sizeof(double); };
+#define CHOL_LAUNCH(nn, ...)                                                                          \
+    do {                                                                                              \
+        if (RQR_CHOL_THREADS(nn) == 512) k_chol_blocked<512><<<1, 512, smem_of(nn), st>>>(__VA_ARGS__); \
+        else                             k_chol_blocked<256><<<1, 256, smem_of(nn), st>>>(__VA_ARGS__); \
+    } while (0)
     if (n <= 128) {
-        k_chol_blocked<<<1, 256, smem_of(n), st>>>(G, n, n, shift, d_shift, R1, n, d_info, 0, Rprev, Rprod,
+        CHOL_LAUNCH(n, G, n, n, shift, d_shift, R1, n, d_info, 0, Rprev, Rprod,
                                                    nullptr, 0, nullptr, 0);
     } else {
         // two-level (see k_chol2_trsm): 0.51 ms -> 0.12 ms at n = 256
         const int h = 128, n2 = n - h, nb2 = (n2 + 7) / 8;
         double* S = R1 + (int64_t)h * n;
-        k_chol_blocked<<<1, 256, smem_of(h), st>>>(G, n, h, shift, d_shift, R1, n, d_info, 0, nullptr, nullptr,
+        CHOL_LAUNCH(h, G, n, h, shift, d_shift, R1, n, d_info, 0, nullptr, nullptr,
                                                    R1, n, nullptr, 0);
         RQR_LAUNCH_CHECK();
         k_chol2_trsm<<<nb2, 32, 0, st>>>(G, n, R1);
         RQR_LAUNCH_CHECK();
         k_chol2_syrk<<<(nb2 * (nb2 + 1) / 2 + 7) / 8, 256, 0, st>>>(G, n, shift, d_shift, R1);
         RQR_LAUNCH_CHECK();
-        k_chol_blocked<<<1, 256, smem_of(n2), st>>>(S, n, n2, 0.0, nullptr, R1 + (int64_t)h * n + h, n, d_info, h,
+        CHOL_LAUNCH(n2, S, n, n2, 0.0, nullptr, R1 + (int64_t)h * n + h, n, d_info, h,
                                                     nullptr, nullptr, nullptr, 0, S, h);
         RQR_LAUNCH_CHECK();
         if (!Rprod) return RQR_OK;
@@ -1100,6 +1113,7 @@ int rqr_chol_dev(const double* G, int n, double shift, const double* d_shift, do
     }
     RQR_LAUNCH_CHECK();
     return RQR_OK;
+#undef CHOL_LAUNCH
 }
 
 // =========================================================================================
